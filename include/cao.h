@@ -1,0 +1,158 @@
+/* cao.h -- C ABI of libcao: constraint-aware evolutionary auto-tuning steps on one B200 (sm_100a).
+ *
+ * The operations follow the problem statement of "Constraint-aware Optimization in Auto-Tuning"
+ * (arxiv/paper_2606_28372; "Lnnn" = line of PAPER.md, "Ox"/"Ax" = readings listed in DESIGN.md):
+ *   P = (X, D, C): parameters, finite domains, predicate constraints           L129-135 (sec. IV-A)
+ *   the search space is fully resolved before tuning                            L137
+ *   Search Space queries: is-valid, valid samples, valid neighbours             L139-143, L215
+ *   strategies DE / PSO / Firefly / GA with repair to the nearest valid config  Alg.1-3
+ *   memoisation of evaluated configs, budget interruption                       L268, L125
+ *
+ * Conventions
+ *   - Every function returns 0 (CAO_OK) or a negative cao_status; cao_last_error() gives a
+ *     thread-local message for the last failure.  No exceptions cross this boundary.
+ *   - Pointers named h_* are HOST memory, d_* are DEVICE memory.  ALL device memory is owned by the
+ *     caller: the library reports the bytes it needs, is handed 256-byte aligned base pointers and
+ *     never allocates device memory itself.  Buffers must stay alive while the handle that was
+ *     given them is alive.  Handles (cao_space, cao_runs) are host objects owned by the library.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Launching
+ *     calls are asynchronous on it unless stated otherwise.
+ *   - There is no CPU fallback: without a CUDA device every launching call returns CAO_E_CUDA.
+ *
+ * Layouts
+ *   - Index row: one byte per parameter, idx_d in [0, m_d), parameter 0 first.  In HBM a row
+ *     occupies row_bytes = 16 (n <= 16) or 32 (n <= 32) bytes, the padding bytes are zero.
+ *   - Linear index L = sum_d idx_d * stride_d, the FIRST declared parameter is the most
+ *     significant digit (itertools.product order, A1).
+ *   - Bitmap: bit (L & 63) of 64-bit little-endian word (L >> 6) is 1 iff config L is valid.
+ *   - rank of a valid config = its position in the valid table, which is sorted by L.
+ */
+#ifndef CAO_H_
+#define CAO_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cao_space cao_space;
+typedef struct cao_runs cao_runs;
+
+typedef enum {
+    CAO_OK = 0,
+    CAO_E_INVALID_ARG = -1,  /* null pointer, bad enum, malformed constraint program, ...        */
+    CAO_E_STATE = -2,        /* call order violated (e.g. fill before count)                      */
+    CAO_E_TOO_LARGE = -3,    /* n > 32, m_d > 256, N >= 2^40, V >= 2^32, pop > 1024               */
+    CAO_E_EMPTY_SPACE = -4,  /* V == 0                                                            */
+    CAO_E_POP_GT_VALID = -5, /* population larger than the number of valid configs               */
+    CAO_E_WORKSPACE = -6,    /* misaligned / missing workspace                                    */
+    CAO_E_CUDA = -7          /* a CUDA runtime call failed (message holds cudaGetErrorString)     */
+} cao_status;
+
+typedef enum { CAO_DE = 0, CAO_PSO = 1, CAO_FIREFLY = 2, CAO_GA = 3 } cao_algo;
+
+/* Hyperparameters, defaults from Table IV (L368-393). */
+typedef struct {
+    float de_F, de_CR;               /* 0.7, 0.6 (best1bin)                          L372-375 */
+    float pso_w, pso_c1, pso_c2;     /* 0.5, 3.0, 0.5                                L378-380 */
+    float ff_B0, ff_gamma, ff_alpha; /* 1.0, 1.0, 0.2                                L383-385 */
+    int32_t ga_mutation_chance;      /* 5 => mutate 1 child in 5                     L389, L393 */
+    int32_t ga_beta_b;               /* 3: Beta(1,b) parent selection over the sorted rank (A18) */
+} cao_hparams;
+
+/* Constraint programs: postfix (RPN) over int64, one int32 word per token (O1, A2, A3).
+ * PUSH_PARAM is followed by the parameter number, PUSH_CONST by the low and the high 32 bits.
+ * DIV/MOD truncate toward zero; a zero divisor makes the whole constraint false; ADD/SUB/MUL/NEG
+ * saturate to +-2^62.  A constraint holds iff its result is non-zero. */
+enum {
+    CAO_OP_PUSH_PARAM = 1, CAO_OP_PUSH_CONST = 2,
+    CAO_OP_ADD = 3, CAO_OP_SUB = 4, CAO_OP_MUL = 5, CAO_OP_DIV = 6, CAO_OP_MOD = 7, CAO_OP_NEG = 8,
+    CAO_OP_MIN = 9, CAO_OP_MAX = 10,
+    CAO_OP_LT = 11, CAO_OP_LE = 12, CAO_OP_GT = 13, CAO_OP_GE = 14, CAO_OP_EQ = 15, CAO_OP_NE = 16,
+    CAO_OP_AND = 17, CAO_OP_OR = 18, CAO_OP_NOT = 19
+};
+
+/* ---------------------------------------------------------------- define P = (X, D, C), L129-135 */
+int cao_space_create(cao_space** out);
+void cao_space_destroy(cao_space* s);
+/* Appends a parameter with n_values (1..256) int64 values (copied).  Call order = digit order. */
+int cao_space_add_param(cao_space* s, const char* name, const int64_t* h_values, int32_t n_values);
+/* Appends a constraint program (copied, validated: known opcodes, stack depth 1 at the end, <= 32). */
+int cao_space_add_constraint(cao_space* s, const int32_t* h_rpn, int32_t n_words);
+
+/* ---------------------------------------------------------------- build the space (S1; L137)
+ * build_mode: 0 = word-parallel (constraints with a small scope become bit tables, the bitmap is
+ * the AND of table words), 1 = plain (every constraint is interpreted for every config).  Both
+ * give identical results.  Set before build_workspace_bytes. */
+int cao_space_set_build_mode(cao_space* s, int32_t mode);
+int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64_t* scratch_bytes);
+/* Pass 1: validity bitmap + per-512-config counts, then the exclusive scan of the counts.
+ * Synchronises `stream` once to return V in *h_V.  d_scratch may be released after build_fill. */
+int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V);
+int cao_space_table_bytes(const cao_space* s, uint64_t* bytes);
+/* Pass 2: valid rows (V x row_bytes), Ltab (V x u64) and the rank directory, into d_table. */
+int cao_space_build_fill(cao_space* s, void* d_table, void* stream);
+int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes);
+/* Borrowed device views into the caller's buffers; rank_dir[i] = number of valid L < 512*i. */
+int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t** d_rows,
+                    const uint64_t** d_Ltab, const uint32_t** d_rank_dir);
+
+/* ---------------------------------------------------------------- Search Space queries (L139), batched
+ * d_idx_rows: count rows of row_bytes bytes each (padding ignored). */
+int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint8_t* d_out,
+                       void* stream);
+/* S5 standalone: d_rank_out[i] = rank of argmin (Hamming, sum |didx|, L) over the valid table; the
+ * identity for valid rows (L143, L215, L270; O9).  d_key_out (optional, may be NULL) receives
+ * ham << 45 | sad << 32 | rank.  use_probe: 1 = bitmap probes of the Hamming-1 neighbours first,
+ * 0 = table scan only.  d_scratch: cao_space_repair_scratch_bytes(count) bytes. */
+int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
+int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
+                     uint64_t* d_key_out, int32_t use_probe, void* d_scratch, void* stream);
+/* Objective table by rank: V floats, > 0 and finite (borrowed; L268: the evaluation is a lookup). */
+int cao_space_set_objective(cao_space* s, const float* d_obj);
+
+/* ---------------------------------------------------------------- runs (S2-S7)
+ * n_runs independent simulated tuning runs of `algo`; run k uses RNG run index first_run + k, so
+ * any partition of the run indices gives the same per-run results. */
+int cao_runs_workspace_bytes(const cao_space* s, int32_t algo, int32_t pop, uint32_t n_runs,
+                             uint32_t max_gens, uint64_t* bytes);
+/* Creates the runs and executes generation 0 (S2; O4) on `stream`.  budget_unique: unique
+ * evaluations per run, 0 = unlimited (L125, A20).  max_gens: generation cap = trajectory rows - 1. */
+int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uint32_t n_runs,
+                    uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens,
+                    uint64_t seed, void* d_workspace, void* stream, cao_runs** out);
+void cao_runs_destroy(cao_runs* r);
+/* S3-S7, n_generations times (stops recording at max_gens).  Asynchronous. */
+int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream);
+/* Copies per-run results to DEVICE arrays of n_runs elements each (any may be NULL). */
+int cao_runs_best(const cao_runs* r, float* d_best_f, uint32_t* d_best_rank, uint32_t* d_uniq,
+                  uint32_t* d_gens_done, void* stream);
+/* Borrowed: trajectory [gen][run] of packed {f32 best_f, u32 best_rank, u32 uniq}, gens 0..generation. */
+int cao_runs_trajectory(const cao_runs* r, const void** d_traj, uint32_t* gens_recorded);
+/* Parity taps of the last stepped generation, [run][ind]: post-snap pre-repair rows (row_bytes each),
+ * validity flag, rank after repair, rank evaluated, f, accept flag, and [run] active flag. */
+int cao_runs_debug_last(const cao_runs* r, const uint8_t** d_postsnap_rows, const uint8_t** d_valid,
+                        const uint32_t** d_repaired_rank, const uint32_t** d_eval_rank, const float** d_f,
+                        const uint8_t** d_accept, const uint8_t** d_active);
+/* Raw population state, borrowed.  which: 0 idx rows [run][ind][row_bytes] u8, 1 rank [run][ind] u32,
+ * 2 f [run][ind] f32, 3 x, 4 v, 5 pbest [run][dim][ind] f32 (dimension-major), 6 pbest_f [run][ind]. */
+int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, uint64_t* bytes);
+/* Counters since create (synchronises `stream`): candidates whose post-snap row was invalid,
+ * candidates that needed the table scan, candidates evaluated. */
+int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uint64_t* n_scanned,
+                      uint64_t* n_evaluated);
+/* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
+uint64_t cao_launch_count(void);
+
+/* Device self-tests for the parity of the arithmetic primitives (O3, O5-O7): out[i] from in[i]. */
+int cao_test_philox(const uint32_t* d_ctr_key /* count x 6 */, uint32_t* d_out /* count x 4 */,
+                    uint64_t count, void* stream);
+int cao_test_exp_neg(const float* d_z, float* d_out, uint64_t count, void* stream);
+
+const char* cao_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAO_H_ */

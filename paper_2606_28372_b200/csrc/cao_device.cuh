@@ -1,0 +1,179 @@
+// cao_device.cuh -- device-side primitives shared by the libcao kernels (sm_100a).
+// Citations: "Lnnn" = PAPER.md line, "Ox"/"Ax" = readings in DESIGN.md.  Nothing here is shared
+// with oracle/ (the CPU oracle has its own copies of every formula).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#define CAO_MAX_DIMS 32
+#define CAO_MAX_STACK 32
+#define CAO_DIR_SHIFT 9          // rank directory granularity: one u32 per 512 configs (8 bitmap words)
+
+// ---------------------------------------------------------------------------------------------
+// Space description handed to every kernel BY VALUE (__grid_constant__), so several spaces can be
+// in flight on different streams without sharing a __constant__ symbol.
+struct SpaceMeta {
+    uint64_t N;                         // Cartesian size
+    uint64_t stride[CAO_MAX_DIMS];      // stride[n-1] = 1 (A1: first param most significant)
+    uint64_t magic[CAO_MAX_DIMS];       // ceil(2^64 / m_d) for m_d >= 2 (exact division of any L < 2^56)
+    const uint64_t* bitmap;             // ceil(N/64) words
+    const uint8_t* rows;                // V x rowB, ascending L, padding bytes zero
+    const uint64_t* Ltab;               // V
+    const uint32_t* dir;                // ceil(N/512)+1 exclusive counts
+    const float* obj;                   // V
+    uint32_t V;
+    int32_t n, rowB, M;                 // M = max_d m_d (O6)
+    uint16_t m[CAO_MAX_DIMS];
+};
+
+// ---------------------------------------------------------------------------------------------
+// O3: Philox4x32-10 (Salmon et al., SC'11).
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t h0 = __umulhi(0xD2511F53u, c.x), l0 = 0xD2511F53u * c.x;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c.z), l1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(h1 ^ c.y ^ k0, l1, h0 ^ c.w ^ k1, l0);
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return c;
+}
+
+enum : uint32_t { S_INIT = 0, S_OP = 1, S_MUT = 2, S_REINIT = 3 };
+
+// Slot-addressed draws for one (seed, run, generation, individual, stream): counter =
+// (run, gen, ind, stream<<24 | slot>>2), word slot&3.  The last block is cached, so walking
+// the slots in ascending order costs one Philox call per four draws.
+struct Draws {
+    uint32_t k0, k1, run, gen, ind, stream, cur;
+    uint4 blk;
+    __device__ __forceinline__ Draws(uint64_t seed, uint32_t run_, uint32_t gen_, uint32_t ind_, uint32_t stream_)
+        : k0((uint32_t)seed), k1((uint32_t)(seed >> 32)), run(run_), gen(gen_), ind(ind_), stream(stream_),
+          cur(0xFFFFFFFFu) {}
+    __device__ __forceinline__ uint32_t operator()(uint32_t slot) {
+        uint32_t b = slot >> 2;
+        if (b != cur) { blk = philox4x32_10(make_uint4(run, gen, ind, (stream << 24) | b), k0, k1); cur = b; }
+        uint32_t s = slot & 3;
+        return s == 0 ? blk.x : s == 1 ? blk.y : s == 2 ? blk.z : blk.w;
+    }
+};
+
+__device__ __forceinline__ float u01(uint32_t w) { return __fmul_rn((float)(w >> 8), 5.9604644775390625e-08f); }
+__device__ __forceinline__ uint32_t below(uint32_t w, uint32_t k) { return __umulhi(w, k); }
+
+// ---------------------------------------------------------------------------------------------
+// fp32 helpers: every operation is one IEEE rounding (__f*_rn never contracts into an FMA).
+// O7: exp(-z) for z >= 0, add/mul only.
+__device__ __forceinline__ float exp_neg_spec(float z) {
+    const float LOG2E = 0x1.715476p+0f, RSQRT2 = 0x1.6a09e6p-1f;
+    const float c0 = 1.0f, c1 = -0x1.62e430p-1f, c2 = 0x1.ebfbe0p-3f, c3 = -0x1.c6b08ep-5f,
+                c4 = 0x1.3b2ab6p-7f, c5 = -0x1.5d87fep-10f, c6 = 0x1.430912p-13f, c7 = -0x1.ffcbfcp-17f;
+    float t = __fmul_rn(z, LOG2E);
+    float kf = floorf(t);
+    if (!(kf < 126.0f)) return 0.0f;
+    float fr = __fsub_rn(t, kf);
+    float u = __fsub_rn(fr, 0.5f);
+    float p = c7;
+    p = __fadd_rn(__fmul_rn(p, u), c6);
+    p = __fadd_rn(__fmul_rn(p, u), c5);
+    p = __fadd_rn(__fmul_rn(p, u), c4);
+    p = __fadd_rn(__fmul_rn(p, u), c3);
+    p = __fadd_rn(__fmul_rn(p, u), c2);
+    p = __fadd_rn(__fmul_rn(p, u), c1);
+    p = __fadd_rn(__fmul_rn(p, u), c0);
+    p = __fmul_rn(p, RSQRT2);
+    float scale = __uint_as_float((uint32_t)(127 - (int)kf) << 23);
+    return __fmul_rn(p, scale);
+}
+
+__device__ __forceinline__ float clamp_pos(float x, float hi) {   // NaN -> 0, -0 -> +0
+    x = (x > 0.0f) ? x : 0.0f;
+    x = (x < hi) ? x : hi;
+    return x;
+}
+// O6: coord(k) = k / (M-1) (IEEE division), snap = rint(x*(M-1)) half-to-even, clamped (A10, A11).
+__device__ __forceinline__ float coord_M(int M, int k) { return M > 1 ? __fdiv_rn((float)k, (float)(M - 1)) : 0.0f; }
+__device__ __forceinline__ int snap_M(int M, int m_d, float x) {
+    float g = __fmul_rn(x, (float)(M - 1));
+    int k = __float2int_rn(g);
+    k = max(k, 0);
+    k = min(k, m_d - 1);
+    return k;
+}
+// O5: round_and_clip(i_best + F*(i_a - i_b)), two fp32 roundings, half-to-even (Alg.1, A8).
+__device__ __forceinline__ int de_mutate_index(float F, int ibest, int ia, int ib, int top) {
+    float t = __fmul_rn(F, (float)(ia - ib));
+    float mf = __fadd_rn((float)ibest, t);
+    int v = __float2int_rn(mf);
+    v = max(v, 0);
+    v = min(v, top);
+    return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Bitmap / rank directory.
+__device__ __forceinline__ bool bit_test(const uint64_t* __restrict__ bitmap, uint64_t L) {
+    return (__ldg(&bitmap[L >> 6]) >> (L & 63)) & 1ull;
+}
+// rank of a VALID L: directory entry of its 512-block + popcount of the bits below it in the block.
+__device__ __forceinline__ uint32_t rank_of(const SpaceMeta& sm, uint64_t L) {
+    uint64_t w = L >> 6, w0 = w & ~7ull;
+    uint32_t r = __ldg(&sm.dir[L >> CAO_DIR_SHIFT]);
+    for (uint64_t q = w0; q < w; ++q) r += __popcll(__ldg(&sm.bitmap[q]));
+    r += __popcll(__ldg(&sm.bitmap[w]) & ((1ull << (L & 63)) - 1ull));
+    return r;
+}
+
+// Exact L / m and L % m through the precomputed reciprocal (m >= 2, L < 2^56).
+__device__ __forceinline__ uint64_t div_magic(uint64_t L, uint64_t magic) { return __umul64hi(L, magic); }
+
+// Row bytes live in uint32 words (4 index bytes per word, byte d&3 of word d>>2).
+__device__ __forceinline__ uint32_t row_byte(const uint32_t* w, int d) { return (w[d >> 2] >> ((d & 3) * 8)) & 0xFFu; }
+
+// Saturating int64 arithmetic of the constraint programs (A3): clamp to +-2^62.
+#define CAO_SAT (1ll << 62)
+__device__ __forceinline__ int64_t sat64(int64_t v) { return v > CAO_SAT ? CAO_SAT : (v < -CAO_SAT ? -CAO_SAT : v); }
+__device__ __forceinline__ int64_t sat_add(int64_t a, int64_t b) {      // |a|,|b| <= 2^62
+    if (b > 0 && a > CAO_SAT - b) return CAO_SAT;
+    if (b < 0 && a < -CAO_SAT - b) return -CAO_SAT;
+    return a + b;
+}
+__device__ __forceinline__ int64_t sat_mul(int64_t a, int64_t b) {
+    int64_t hi = __mul64hi(a, b);
+    int64_t lo = (int64_t)((uint64_t)a * (uint64_t)b);
+    if (hi != (lo >> 63)) return ((a < 0) != (b < 0)) ? -CAO_SAT : CAO_SAT;
+    return sat64(lo);
+}
+
+// O1: postfix interpreter over the VALUES x[d]; returns 1/0; a zero divisor makes the constraint false.
+__device__ __noinline__ int eval_program(const int32_t* __restrict__ w, int nw, const int64_t* __restrict__ x) {
+    int64_t st[CAO_MAX_STACK];
+    int sp = 0;
+    for (int pc = 0; pc < nw; ++pc) {
+        int op = w[pc];
+        if (op == 1) { st[sp++] = sat64(x[w[++pc]]); continue; }
+        if (op == 2) {
+            uint64_t lo = (uint32_t)w[pc + 1], hi = (uint32_t)w[pc + 2]; pc += 2;
+            st[sp++] = sat64((int64_t)(lo | (hi << 32))); continue;
+        }
+        if (op == 8) { st[sp - 1] = -st[sp - 1]; continue; }
+        if (op == 19) { st[sp - 1] = (st[sp - 1] == 0); continue; }
+        int64_t b = st[--sp], a = st[sp - 1], r = 0;
+        switch (op) {
+            case 3: r = sat_add(a, b); break;
+            case 4: r = sat_add(a, -b); break;
+            case 5: r = sat_mul(a, b); break;
+            case 6: if (b == 0) return 0; r = a / b; break;
+            case 7: if (b == 0) return 0; r = a % b; break;
+            case 9: r = a < b ? a : b; break;
+            case 10: r = a > b ? a : b; break;
+            case 11: r = a < b; break;  case 12: r = a <= b; break;
+            case 13: r = a > b; break;  case 14: r = a >= b; break;
+            case 15: r = a == b; break; case 16: r = a != b; break;
+            case 17: r = (a != 0) && (b != 0); break;
+            case 18: r = (a != 0) || (b != 0); break;
+        }
+        st[sp - 1] = r;
+    }
+    return st[0] != 0;
+}

@@ -1,0 +1,185 @@
+// cao_enum_kernels.cuh -- S1: search-space construction (O1).
+//
+// The Cartesian index range is cut into blocks of B consecutive configs (B = product of the trailing
+// digits t..n-1).  A constraint whose scope is small is turned into a bit table indexed by its outer
+// scope digits; each row holds the B-bit validity pattern over the inner digits.  The bitmap of a block
+// is the AND of one row per constraint; constraints too wide for a table ("residual") are interpreted
+// only for the configs that survive the AND.  In plain mode every constraint is residual.
+#pragma once
+#include "cao_host.h"
+
+struct TableBuildArgs {
+    const int64_t* dom; const int32_t* prog; uint64_t* out;
+    uint64_t rows, B;
+    uint32_t Wb; int32_t nw, t, n_outer;
+    uint8_t dig[CAO_MAX_DIMS]; uint32_t cstride[CAO_MAX_DIMS];
+};
+
+// One thread per (row, 64-bit word of the row): evaluates the program for up to 64 inner patterns.
+__global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ SpaceMeta sm,
+                                                     const __grid_constant__ TableBuildArgs a) {
+    uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= a.rows * a.Wb) return;
+    uint64_t row = gid / a.Wb; uint32_t j = (uint32_t)(gid - row * a.Wb);
+    int64_t x[CAO_MAX_DIMS];
+    for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
+    for (int k = 0; k < a.n_outer; ++k) {
+        int d = a.dig[k];
+        uint32_t idx = (uint32_t)((row / a.cstride[k]) % sm.m[d]);
+        x[d] = a.dom[d * 256 + idx];
+    }
+    uint64_t word = 0;
+    for (int b = 0; b < 64; ++b) {
+        uint64_t p = (uint64_t)j * 64 + b;
+        if (p >= a.B) break;
+        uint64_t q = p;
+        for (int d = sm.n - 1; d >= a.t; --d) {
+            uint32_t m = sm.m[d];
+            uint32_t idx = (uint32_t)(q % m); q /= m;
+            x[d] = a.dom[d * 256 + idx];
+        }
+        if (eval_program(a.prog, a.nw, x)) word |= 1ull << b;
+    }
+    a.out[gid] = word;
+}
+
+__device__ __forceinline__ uint64_t get64(const uint64_t* mk, uint32_t r, uint32_t Wb) {
+    uint32_t j = r >> 6, s = r & 63;
+    if (j >= Wb) return 0;
+    uint64_t v = mk[j] >> s;
+    if (s && j + 1 < Wb) v |= mk[j + 1] << (64 - s);
+    return v;
+}
+
+// Pass 1.  desc layout: [0..n_tab) offsets of tabled descriptors {toff_lo, toff_hi, n_outer, (digit, cstride)*},
+// [n_tab..n_tab+n_res) offsets of residual descriptors {nw, words*}.
+__global__ void __launch_bounds__(256) k_enum_pass1(const __grid_constant__ SpaceMeta sm,
+                                                    const __grid_constant__ EnumArgs a) {
+    extern __shared__ uint64_t smem64[];
+    uint64_t* masks = smem64;
+    uint8_t* od = (uint8_t*)(masks + (size_t)(a.nb + 1) * a.Wb);
+    const uint32_t tid = threadIdx.x, bd = blockDim.x;
+    const uint64_t o0 = (uint64_t)blockIdx.x * a.nb;
+    const uint32_t tail_bits = (uint32_t)(a.B - (uint64_t)(a.Wb - 1) * 64);      // 1..64 bits in the last word
+    for (uint32_t i = tid; i <= a.nb; i += bd) {
+        uint64_t o = o0 + i;
+        uint64_t* mk = masks + (size_t)i * a.Wb;
+        if (o >= a.n_blocks) { for (uint32_t j = 0; j < a.Wb; ++j) mk[j] = 0; continue; }
+        uint64_t q = o;
+        for (int d = a.t - 1; d >= 0; --d) {
+            uint32_t m = sm.m[d];
+            uint32_t idx = 0;
+            if (m > 1) { uint64_t q2 = div_magic(q, sm.magic[d]); idx = (uint32_t)(q - q2 * m); q = q2; }
+            od[d * bd + tid] = (uint8_t)idx;
+        }
+        for (uint32_t j = 0; j + 1 < a.Wb; ++j) mk[j] = ~0ull;
+        mk[a.Wb - 1] = tail_bits == 64 ? ~0ull : ((1ull << tail_bits) - 1ull);
+        uint64_t any = 1;
+        for (int c = 0; c < a.n_tab && any; ++c) {
+            const int32_t* ds = a.desc + __ldg(&a.desc[c]);
+            uint64_t toff = (uint32_t)__ldg(&ds[0]) | ((uint64_t)(uint32_t)__ldg(&ds[1]) << 32);
+            int no = __ldg(&ds[2]);
+            uint64_t k = 0;
+            for (int e = 0; e < no; ++e) k += (uint64_t)od[__ldg(&ds[3 + 2 * e]) * bd + tid] * (uint32_t)__ldg(&ds[4 + 2 * e]);
+            const uint64_t* tab = a.tables + toff + k * a.Wb;
+            any = 0;
+            for (uint32_t j = 0; j < a.Wb; ++j) { uint64_t v = mk[j] & __ldg(&tab[j]); mk[j] = v; any |= v; }
+        }
+        if (a.n_res && any) {
+            int64_t x[CAO_MAX_DIMS];
+            for (int d = 0; d < a.t; ++d) x[d] = a.dom[d * 256 + od[d * bd + tid]];
+            for (uint32_t j = 0; j < a.Wb; ++j) {
+                uint64_t v = mk[j], keep = v;
+                while (v) {
+                    int b = __ffsll((long long)v) - 1; v &= v - 1;
+                    uint64_t p = (uint64_t)j * 64 + b;
+                    for (int d = sm.n - 1; d >= a.t; --d) {
+                        uint32_t m = sm.m[d]; uint32_t idx = 0;
+                        if (m > 1) { uint64_t p2 = div_magic(p, sm.magic[d]); idx = (uint32_t)(p - p2 * m); p = p2; }
+                        x[d] = a.dom[d * 256 + idx];
+                    }
+                    bool ok = true;
+                    for (int r = 0; r < a.n_res && ok; ++r) {
+                        const int32_t* ds = a.desc + __ldg(&a.desc[a.n_tab + r]);
+                        ok = eval_program(ds + 1, __ldg(&ds[0]), x);
+                    }
+                    if (!ok) keep &= ~(1ull << b);
+                }
+                mk[j] = keep;
+            }
+        }
+    }
+    __syncthreads();
+    // Phase 2: re-align the block masks to 64-bit words of the global bitmap (coalesced stores).
+    const uint64_t g0 = o0 * a.B;
+    uint64_t o1 = o0 + a.nb; if (o1 > a.n_blocks) o1 = a.n_blocks;
+    const uint64_t g1 = o1 * a.B;                       // == N for the last CTA
+    const uint64_t w_first = (g0 + 63) >> 6, w_end = (g1 + 63) >> 6;
+    for (uint64_t w = w_first + tid; w < w_end; w += bd) {
+        uint64_t rel = (w << 6) - g0;
+        uint64_t i = a.B > 1 ? div_magic(rel, a.magicB) : rel;
+        uint32_t r = (uint32_t)(rel - i * a.B);
+        uint64_t val = get64(masks + i * a.Wb, r, a.Wb);
+        uint64_t avail = a.B - r;
+        // B >= 64 whenever there is more than one block, so at most one following block contributes
+        if (avail < 64) val |= get64(masks + (i + 1) * a.Wb, 0, a.Wb) << avail;
+        a.bitmap[w] = val;
+        if (val) atomicAdd(&a.cnt[w >> 3], (uint32_t)__popcll(val));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Exclusive scan of the per-512 counts (three small launches; the data is N/128 bytes).
+#define SCAN_CHUNK 4096                                  // entries per CTA (256 threads x 16)
+__global__ void __launch_bounds__(256) k_scan_reduce(const uint32_t* __restrict__ cnt, uint64_t nd, uint32_t* part) {
+    __shared__ uint32_t ws[8];
+    uint64_t base = (uint64_t)blockIdx.x * SCAN_CHUNK + threadIdx.x * 16;
+    uint32_t s = 0;
+    for (int k = 0; k < 16; ++k) if (base + k < nd) s += cnt[base + k];
+    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) { uint32_t t = 0; for (int k = 0; k < 8; ++k) t += ws[k]; part[blockIdx.x] = t; }
+}
+// One CTA: exclusive scan of the partials in place; total (= V) to *V_out as u64 (overflow of u32 is detected on the host).
+__global__ void __launch_bounds__(1024) k_scan_partials(uint32_t* part, uint64_t n_part, uint64_t* V_out) {
+    __shared__ uint64_t ws[32];
+    __shared__ uint64_t carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (uint64_t base = 0; base < n_part; base += 1024) {
+        uint64_t i = base + threadIdx.x;
+        uint64_t v = i < n_part ? part[i] : 0, s = v;
+        for (int o = 1; o < 32; o <<= 1) { uint64_t t = __shfl_up_sync(0xFFFFFFFFu, s, o); if ((threadIdx.x & 31) >= o) s += t; }
+        if ((threadIdx.x & 31) == 31) ws[threadIdx.x >> 5] = s;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            uint64_t t = ws[threadIdx.x], u = t;
+            for (int o = 1; o < 32; o <<= 1) { uint64_t z = __shfl_up_sync(0xFFFFFFFFu, u, o); if (threadIdx.x >= o) u += z; }
+            ws[threadIdx.x] = u - t;
+        }
+        __syncthreads();
+        uint64_t excl = carry_s + ws[threadIdx.x >> 5] + s - v;
+        if (i < n_part) part[i] = (uint32_t)excl;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = excl + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *V_out = carry_s;
+}
+// In-place exclusive scan of each chunk plus the chunk offset.  nd here counts the trailing zero entry
+// too, so the last entry receives the total.
+__global__ void __launch_bounds__(256) k_scan_apply(uint32_t* cnt, uint64_t nd, const uint32_t* __restrict__ part) {
+    __shared__ uint32_t ws[8];
+    uint64_t base = (uint64_t)blockIdx.x * SCAN_CHUNK + threadIdx.x * 16;
+    uint32_t v[16], s = 0;
+    for (int k = 0; k < 16; ++k) { v[k] = (base + k < nd) ? cnt[base + k] : 0; s += v[k]; }
+    uint32_t inc = s;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o); if ((threadIdx.x & 31) >= o) inc += t; }
+    if ((threadIdx.x & 31) == 31) ws[threadIdx.x >> 5] = inc;
+    __syncthreads();
+    uint32_t off = part[blockIdx.x];
+    for (uint32_t k = 0; k < (threadIdx.x >> 5); ++k) off += ws[k];
+    off += inc - s;
+    for (int k = 0; k < 16; ++k) { if (base + k < nd) cnt[base + k] = off; off += v[k]; }
+}

@@ -1,0 +1,82 @@
+// cao_fill_kernels.cuh -- S1 pass 2 (valid table from the bitmap) and the batched is-valid query.
+#pragma once
+#include "cao_host.h"
+
+// Decode L into index bytes packed in ROWW uint32 words (4 bytes per word, padding zero).
+template <int ROWW>
+__device__ __forceinline__ void decode_row(const SpaceMeta& sm, uint64_t L, uint32_t (&w)[ROWW]) {
+#pragma unroll
+    for (int k = 0; k < ROWW; ++k) w[k] = 0;
+#pragma unroll
+    for (int d = ROWW * 4 - 1; d >= 0; --d) {
+        if (d < sm.n) {
+            uint32_t m = sm.m[d];
+            if (m > 1) {
+                uint64_t q = div_magic(L, sm.magic[d]);
+                uint32_t idx = (uint32_t)(L - q * m);
+                L = q;
+                w[d >> 2] |= idx << ((d & 3) * 8);
+            }
+        }
+    }
+}
+
+// L of a packed row.
+template <int ROWW>
+__device__ __forceinline__ uint64_t row_lin(const SpaceMeta& sm, const uint32_t (&w)[ROWW]) {
+    uint64_t L = 0;
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d)
+        if (d < sm.n) L += (uint64_t)((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) * sm.stride[d];
+    return L;
+}
+
+// One thread per 32-bit half word of the bitmap; the 16 lanes of a 512-config group share a directory
+// entry and find their row offsets with a 16-lane shuffle scan.  Rows are written in ascending L.
+template <int ROWW>
+__global__ void __launch_bounds__(256) k_fill(const __grid_constant__ SpaceMeta sm, uint64_t n_words,
+                                              uint8_t* rows, uint64_t* Ltab, uint32_t* dir_out,
+                                              const uint32_t* __restrict__ dir, uint64_t nd) {
+    uint64_t hw = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint64_t g = hw >> 4;
+    uint32_t base = 0, cnt = 0;
+    if (g < nd) {
+        base = dir[g]; cnt = dir[g + 1] - base;
+        if ((hw & 15) == 0) { dir_out[g] = base; if (g + 1 == nd) dir_out[nd] = base + cnt; }
+    }
+    uint32_t bits = 0;
+    if (cnt && hw < 2 * n_words) bits = ((const uint32_t*)sm.bitmap)[hw];
+    uint32_t pc = __popc(bits), inc = pc;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o, 16); if ((threadIdx.x & 15) >= o) inc += t; }
+    uint32_t r = base + inc - pc;
+    while (bits) {
+        int b = __ffs(bits) - 1; bits &= bits - 1;
+        uint64_t L = hw * 32 + b;
+        uint32_t w[ROWW];
+        decode_row<ROWW>(sm, L, w);
+        uint4* dst = (uint4*)(rows + (uint64_t)r * (ROWW * 4));
+        dst[0] = make_uint4(w[0], w[1], w[2], w[3]);
+        if (ROWW == 8) dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
+        Ltab[r] = L;
+        ++r;
+    }
+}
+
+// Batched Search Space query "is valid" (L139): out[i] = bitmap[L(row_i)]; rows with an index out of its
+// domain are invalid.
+template <int ROWW>
+__global__ void __launch_bounds__(256) k_is_valid(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ rows_in,
+                                                  uint64_t count, uint8_t* out) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const uint4* src = (const uint4*)(rows_in + i * (ROWW * 4));
+    uint32_t w[ROWW];
+    uint4 a = __ldg(&src[0]); w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
+    if (ROWW == 8) { uint4 b = __ldg(&src[1]); w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w; }
+    bool ok = true;
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d)
+        if (d < sm.n && ((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) >= sm.m[d]) ok = false;
+    out[i] = ok ? (uint8_t)bit_test(sm.bitmap, row_lin<ROWW>(sm, w)) : (uint8_t)0;
+}

@@ -1,0 +1,289 @@
+// cao_space.cu -- host side of the search-space half of include/cao.h (S1, is-valid; L129-143).
+#include <algorithm>
+#include <cstring>
+#include "cao_enum_kernels.cuh"
+#include "cao_fill_kernels.cuh"
+
+thread_local std::string g_cao_err;
+std::atomic<uint64_t> g_cao_launches{0};
+int cao_fail(int code, const std::string& msg) { g_cao_err = msg; return code; }
+int cao_cuda_check(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return 0;
+    return cao_fail(CAO_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+static bool program_ok(const int32_t* w, int nw, int n_params) {
+    int sp = 0;
+    for (int pc = 0; pc < nw; ++pc) {
+        int32_t op = w[pc];
+        if (op == CAO_OP_PUSH_PARAM) { if (pc + 1 >= nw || w[pc + 1] < 0 || w[pc + 1] >= n_params) return false; ++pc; ++sp; }
+        else if (op == CAO_OP_PUSH_CONST) { if (pc + 2 >= nw) return false; pc += 2; ++sp; }
+        else if (op == CAO_OP_NEG || op == CAO_OP_NOT) { if (sp < 1) return false; }
+        else if (op >= CAO_OP_ADD && op <= CAO_OP_OR) { if (sp < 2) return false; --sp; }
+        else return false;
+        if (sp > CAO_MAX_STACK) return false;
+    }
+    return sp == 1;
+}
+
+extern "C" {
+
+const char* cao_last_error(void) { return g_cao_err.c_str(); }
+uint64_t cao_launch_count(void) { return g_cao_launches.load(); }
+
+int cao_space_create(cao_space** out) {
+    if (!out) return cao_fail(CAO_E_INVALID_ARG, "cao_space_create: out is NULL");
+    *out = new cao_space();
+    return CAO_OK;
+}
+void cao_space_destroy(cao_space* s) { delete s; }
+
+int cao_space_add_param(cao_space* s, const char*, const int64_t* h_values, int32_t n_values) {
+    if (!s || !h_values) return cao_fail(CAO_E_INVALID_ARG, "cao_space_add_param: NULL argument");
+    if (s->planned) return cao_fail(CAO_E_STATE, "cao_space_add_param: space already planned/built");
+    if (n_values < 1) return cao_fail(CAO_E_INVALID_ARG, "cao_space_add_param: n_values < 1");
+    if (n_values > 256 || s->dom.size() >= CAO_MAX_DIMS) return cao_fail(CAO_E_TOO_LARGE, "cao_space_add_param: more than 32 params or 256 values");
+    s->dom.emplace_back(h_values, h_values + n_values);
+    return CAO_OK;
+}
+
+int cao_space_add_constraint(cao_space* s, const int32_t* h_rpn, int32_t n_words) {
+    if (!s || !h_rpn || n_words < 1) return cao_fail(CAO_E_INVALID_ARG, "cao_space_add_constraint: NULL/empty program");
+    if (s->planned) return cao_fail(CAO_E_STATE, "cao_space_add_constraint: space already planned/built");
+    if (!program_ok(h_rpn, n_words, (int)s->dom.size())) return cao_fail(CAO_E_INVALID_ARG, "cao_space_add_constraint: malformed program");
+    s->cons.emplace_back(h_rpn, h_rpn + n_words);
+    return CAO_OK;
+}
+
+int cao_space_set_build_mode(cao_space* s, int32_t mode) {
+    if (!s || (mode != 0 && mode != 1)) return cao_fail(CAO_E_INVALID_ARG, "cao_space_set_build_mode: mode must be 0 or 1");
+    if (s->planned) return cao_fail(CAO_E_STATE, "cao_space_set_build_mode: after build_workspace_bytes");
+    s->mode = mode;
+    return CAO_OK;
+}
+
+static int plan_space(cao_space* s) {
+    const int n = (int)s->dom.size();
+    if (n < 1) return cao_fail(CAO_E_INVALID_ARG, "space has no parameters");
+    SpaceMeta& M = s->meta;
+    std::memset(&M, 0, sizeof(M));
+    M.n = n; M.rowB = n <= 16 ? 16 : 32; M.M = 1;
+    unsigned __int128 N = 1;
+    for (int d = n - 1; d >= 0; --d) {
+        M.stride[d] = (uint64_t)N;
+        uint32_t m = (uint32_t)s->dom[d].size();
+        M.m[d] = (uint16_t)m;
+        M.M = std::max<int>(M.M, (int)m);
+        M.magic[d] = m > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + m - 1) / m) : 0;
+        N *= m;
+        if (N >= ((unsigned __int128)1 << 40)) return cao_fail(CAO_E_TOO_LARGE, "Cartesian size N >= 2^40");
+    }
+    M.N = (uint64_t)N;
+    // inner block: smallest trailing product >= 256 (or the whole space)
+    uint64_t B = 1; int t = n;
+    while (t > 0 && B < 256) { --t; B *= M.m[t]; }
+    s->t = t; s->B = B; s->Wb = (uint32_t)((B + 63) / 64); s->n_blocks = M.N / B;
+    s->n_words = (M.N + 63) / 64; s->nd = (M.N + 511) / 512;
+    int64_t nb = (int64_t)(40960 / ((uint64_t)s->Wb * 8)) - 1;
+    s->nb = (uint32_t)std::min<int64_t>(256, std::max<int64_t>(1, nb));
+    // per-constraint plan
+    s->plan.assign(s->cons.size(), ConsPlan());
+    uint64_t total_words = 0;
+    for (size_t c = 0; c < s->cons.size(); ++c) {
+        ConsPlan& p = s->plan[c];
+        const auto& w = s->cons[c];
+        bool used[CAO_MAX_DIMS] = {false};
+        for (size_t pc = 0; pc < w.size(); ++pc) {
+            if (w[pc] == CAO_OP_PUSH_PARAM) { used[w[pc + 1]] = true; ++pc; }
+            else if (w[pc] == CAO_OP_PUSH_CONST) pc += 2;
+        }
+        uint64_t rows = 1; bool ok = true;
+        for (int d = n - 1; d >= 0; --d) if (used[d]) {
+            p.scope.push_back(d);
+            if (d < t) {
+                p.outer.push_back(d); p.cstride.push_back((uint32_t)rows);
+                rows *= M.m[d];
+                if (rows > (1ull << 24)) { ok = false; rows = 1ull << 24; }
+            }
+        }
+        p.rows = rows;
+        uint64_t words = rows * s->Wb;
+        p.tabled = s->mode == 0 && ok && words * 8 <= (8ull << 20) && (total_words + words) * 8 <= (128ull << 20);
+        if (p.tabled) { p.table_off = total_words; total_words += words; }
+    }
+    s->tables_words = total_words;
+    // descriptors: small tables first, then residual programs
+    std::vector<int> tab, res;
+    for (size_t c = 0; c < s->cons.size(); ++c) (s->plan[c].tabled ? tab : res).push_back((int)c);
+    std::stable_sort(tab.begin(), tab.end(), [&](int a, int b) { return s->plan[a].rows < s->plan[b].rows; });
+    s->n_tab = (int)tab.size(); s->n_res = (int)res.size();
+    std::vector<int32_t>& D = s->desc;
+    D.assign(tab.size() + res.size() + s->cons.size(), 0);       // [tab offs][res offs][program offs of every constraint]
+    for (size_t k = 0; k < tab.size(); ++k) {
+        const ConsPlan& p = s->plan[tab[k]];
+        D[k] = (int32_t)D.size();
+        D.push_back((int32_t)(uint32_t)p.table_off); D.push_back((int32_t)(uint32_t)(p.table_off >> 32));
+        D.push_back((int32_t)p.outer.size());
+        for (size_t e = 0; e < p.outer.size(); ++e) { D.push_back(p.outer[e]); D.push_back((int32_t)p.cstride[e]); }
+    }
+    for (size_t k = 0; k < res.size(); ++k) {
+        D[tab.size() + k] = (int32_t)D.size();
+        D.push_back((int32_t)s->cons[res[k]].size());
+        D.insert(D.end(), s->cons[res[k]].begin(), s->cons[res[k]].end());
+    }
+    for (size_t c = 0; c < s->cons.size(); ++c) {
+        D[tab.size() + res.size() + c] = (int32_t)D.size();
+        D.insert(D.end(), s->cons[c].begin(), s->cons[c].end());
+    }
+    // scratch layout
+    uint64_t off = 0;
+    s->off_dom = off; off = align256(off + (uint64_t)n * 256 * 8);
+    s->off_desc = off; off = align256(off + D.size() * 4);
+    s->off_tables = off; off = align256(off + std::max<uint64_t>(1, total_words) * 8);
+    s->off_cnt = off; off = align256(off + (s->nd + 1) * 4);
+    s->n_part = (s->nd + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    s->off_part = off; off = align256(off + s->n_part * 4);
+    s->off_V = off; off = align256(off + 8);
+    s->scratch_bytes = off;
+    s->bitmap_bytes = align256(s->n_words * 8);
+    s->planned = true;
+    return CAO_OK;
+}
+
+int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64_t* scratch_bytes) {
+    if (!s || !bitmap_bytes || !scratch_bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_build_workspace_bytes: NULL argument");
+    if (!s->planned) { int rc = plan_space(s); if (rc) return rc; }
+    *bitmap_bytes = s->bitmap_bytes; *scratch_bytes = s->scratch_bytes;
+    return CAO_OK;
+}
+
+int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V) {
+    if (!s || !h_V) return cao_fail(CAO_E_INVALID_ARG, "cao_space_build_count: NULL argument");
+    if (!s->planned) return cao_fail(CAO_E_STATE, "cao_space_build_count: call cao_space_build_workspace_bytes first");
+    if (!d_bitmap || !d_scratch || ((uintptr_t)d_bitmap & 255) || ((uintptr_t)d_scratch & 255))
+        return cao_fail(CAO_E_WORKSPACE, "cao_space_build_count: bitmap/scratch must be non-NULL and 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n = s->meta.n;
+    uint8_t* sc = (uint8_t*)d_scratch;
+    std::vector<int64_t> hdom((size_t)n * 256, 0);
+    for (int d = 0; d < n; ++d) std::copy(s->dom[d].begin(), s->dom[d].end(), hdom.begin() + (size_t)d * 256);
+    CAO_CUDA(cudaMemcpyAsync(sc + s->off_dom, hdom.data(), hdom.size() * 8, cudaMemcpyHostToDevice, st));
+    CAO_CUDA(cudaMemcpyAsync(sc + s->off_desc, s->desc.data(), s->desc.size() * 4, cudaMemcpyHostToDevice, st));
+    CAO_CUDA(cudaMemsetAsync(sc + s->off_cnt, 0, (s->nd + 1) * 4, st));
+    s->meta.bitmap = (const uint64_t*)d_bitmap;
+    const int64_t* d_dom = (const int64_t*)(sc + s->off_dom);
+    const int32_t* d_desc = (const int32_t*)(sc + s->off_desc);
+    uint64_t* d_tables = (uint64_t*)(sc + s->off_tables);
+    const size_t prog_base = (size_t)s->n_tab + s->n_res;
+    for (size_t c = 0; c < s->cons.size(); ++c) {
+        const ConsPlan& p = s->plan[c];
+        if (!p.tabled) continue;
+        TableBuildArgs a{};
+        a.dom = d_dom; a.prog = d_desc + s->desc[prog_base + c]; a.out = d_tables + p.table_off;
+        a.rows = p.rows; a.B = s->B; a.Wb = s->Wb; a.nw = (int32_t)s->cons[c].size(); a.t = s->t;
+        a.n_outer = (int32_t)p.outer.size();
+        for (size_t e = 0; e < p.outer.size(); ++e) { a.dig[e] = (uint8_t)p.outer[e]; a.cstride[e] = p.cstride[e]; }
+        uint64_t threads = p.rows * s->Wb;
+        k_build_table<<<(unsigned)((threads + 127) / 128), 128, 0, st>>>(s->meta, a);
+        CAO_LAUNCHED("k_build_table");
+    }
+    EnumArgs ea{};
+    ea.B = s->B; ea.magicB = s->B > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + s->B - 1) / s->B) : 0;
+    ea.n_blocks = s->n_blocks; ea.n_words = s->n_words; ea.dom = d_dom; ea.desc = d_desc; ea.tables = d_tables;
+    ea.bitmap = (uint64_t*)d_bitmap; ea.cnt = (uint32_t*)(sc + s->off_cnt);
+    ea.Wb = s->Wb; ea.nb = s->nb; ea.t = s->t; ea.n_tab = s->n_tab; ea.n_res = s->n_res;
+    size_t smem = (size_t)(s->nb + 1) * s->Wb * 8 + (size_t)CAO_MAX_DIMS * 256;
+    if (smem > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_enum_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    uint64_t grid = (s->n_blocks + s->nb - 1) / s->nb;
+    k_enum_pass1<<<(unsigned)grid, 256, smem, st>>>(s->meta, ea);
+    CAO_LAUNCHED("k_enum_pass1");
+    uint32_t* d_cnt = (uint32_t*)(sc + s->off_cnt);
+    uint32_t* d_part = (uint32_t*)(sc + s->off_part);
+    uint64_t* d_V = (uint64_t*)(sc + s->off_V);
+    k_scan_reduce<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
+    CAO_LAUNCHED("k_scan_reduce");
+    k_scan_partials<<<1, 1024, 0, st>>>(d_part, s->n_part, d_V);
+    CAO_LAUNCHED("k_scan_partials");
+    k_scan_apply<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
+    CAO_LAUNCHED("k_scan_apply");
+    uint64_t V = 0;
+    CAO_CUDA(cudaMemcpyAsync(&V, d_V, 8, cudaMemcpyDeviceToHost, st));
+    CAO_CUDA(cudaStreamSynchronize(st));
+    if (V >= (1ull << 32)) return cao_fail(CAO_E_TOO_LARGE, "V >= 2^32");
+    s->meta.V = (uint32_t)V; s->d_scratch = d_scratch; s->counted = true; s->filled = false;
+    *h_V = V;
+    const uint64_t rowB = s->meta.rowB;
+    uint64_t off = 0;
+    s->off_rows = off; off = align256(off + std::max<uint64_t>(1, V) * rowB);
+    s->off_Ltab = off; off = align256(off + std::max<uint64_t>(1, V) * 8);
+    s->off_dir = off; off = align256(off + (s->nd + 1) * 4);
+    s->table_bytes = off;
+    return CAO_OK;
+}
+
+int cao_space_table_bytes(const cao_space* s, uint64_t* bytes) {
+    if (!s || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_table_bytes: NULL argument");
+    if (!s->counted) return cao_fail(CAO_E_STATE, "cao_space_table_bytes: call cao_space_build_count first");
+    *bytes = s->table_bytes;
+    return CAO_OK;
+}
+
+int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_build_fill: NULL space");
+    if (!s->counted) return cao_fail(CAO_E_STATE, "cao_space_build_fill: call cao_space_build_count first");
+    if (!d_table || ((uintptr_t)d_table & 255)) return cao_fail(CAO_E_WORKSPACE, "cao_space_build_fill: table must be non-NULL and 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    uint8_t* tb = (uint8_t*)d_table;
+    uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
+    const uint32_t* cnt = (const uint32_t*)((uint8_t*)s->d_scratch + s->off_cnt);
+    uint64_t threads = s->nd * 16;
+    unsigned grid = (unsigned)((threads + 255) / 256);
+    if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+    else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+    CAO_LAUNCHED("k_fill");
+    s->meta.rows = rows; s->meta.Ltab = Ltab; s->meta.dir = dir;
+    s->filled = true;
+    return CAO_OK;
+}
+
+int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_sizes: NULL space");
+    if (!s->planned) return cao_fail(CAO_E_STATE, "cao_space_sizes: space not planned yet");
+    if (N) *N = s->meta.N;
+    if (V) *V = s->counted ? s->meta.V : 0;
+    if (n) *n = s->meta.n;
+    if (row_bytes) *row_bytes = s->meta.rowB;
+    return CAO_OK;
+}
+
+int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t** d_rows, const uint64_t** d_Ltab,
+                    const uint32_t** d_rank_dir) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_views: NULL space");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_views: space not built");
+    if (d_bitmap) *d_bitmap = s->meta.bitmap;
+    if (d_rows) *d_rows = s->meta.rows;
+    if (d_Ltab) *d_Ltab = s->meta.Ltab;
+    if (d_rank_dir) *d_rank_dir = s->meta.dir;
+    return CAO_OK;
+}
+
+int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint8_t* d_out, void* stream) {
+    if (!s || (count && (!d_idx_rows || !d_out))) return cao_fail(CAO_E_INVALID_ARG, "cao_space_is_valid: NULL argument");
+    if (!s->counted) return cao_fail(CAO_E_STATE, "cao_space_is_valid: space not built");
+    if (count == 0) return CAO_OK;
+    if ((uintptr_t)d_idx_rows & 15) return cao_fail(CAO_E_WORKSPACE, "cao_space_is_valid: rows must be 16-byte aligned");
+    unsigned grid = (unsigned)((count + 255) / 256);
+    if (s->meta.rowB == 16) k_is_valid<4><<<grid, 256, 0, (cudaStream_t)stream>>>(s->meta, d_idx_rows, count, d_out);
+    else k_is_valid<8><<<grid, 256, 0, (cudaStream_t)stream>>>(s->meta, d_idx_rows, count, d_out);
+    CAO_LAUNCHED("k_is_valid");
+    return CAO_OK;
+}
+
+int cao_space_set_objective(cao_space* s, const float* d_obj) {
+    if (!s || !d_obj) return cao_fail(CAO_E_INVALID_ARG, "cao_space_set_objective: NULL argument");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_set_objective: space not built");
+    s->meta.obj = d_obj;
+    return CAO_OK;
+}
+
+}  // extern "C"
