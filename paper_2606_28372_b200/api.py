@@ -1,0 +1,357 @@
+"""ctypes binding of include/cao.h: same names, argument marshalling only.
+
+PyTorch is used for device memory (``torch.empty(..., device='cuda')``) and the current stream.
+The product path never imports ``oracle`` and has no CPU fallback.
+"""
+from __future__ import annotations
+import ctypes as C
+import os
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcao.so")
+ALGOS = {"de": 0, "pso": 1, "firefly": 2, "ga": 3}
+
+CAO_ERRORS = {-1: "CAO_E_INVALID_ARG", -2: "CAO_E_STATE", -3: "CAO_E_TOO_LARGE", -4: "CAO_E_EMPTY_SPACE",
+              -5: "CAO_E_POP_GT_VALID", -6: "CAO_E_WORKSPACE", -7: "CAO_E_CUDA"}
+
+
+class CaoError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{CAO_ERRORS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class HParams(C.Structure):
+    """cao_hparams; defaults from Table IV, ga_beta_b per reading A18."""
+    _fields_ = [("de_F", C.c_float), ("de_CR", C.c_float),
+                ("pso_w", C.c_float), ("pso_c1", C.c_float), ("pso_c2", C.c_float),
+                ("ff_B0", C.c_float), ("ff_gamma", C.c_float), ("ff_alpha", C.c_float),
+                ("ga_mutation_chance", C.c_int32), ("ga_beta_b", C.c_int32)]
+
+    @classmethod
+    def default(cls):
+        return cls(0.7, 0.6, 0.5, 3.0, 0.5, 1.0, 1.0, 0.2, 5, 3)
+
+
+vp, u64, u32, i32 = C.c_void_p, C.c_uint64, C.c_uint32, C.c_int32
+pu64, pi32, pvp = C.POINTER(C.c_uint64), C.POINTER(C.c_int32), C.POINTER(C.c_void_p)
+
+# name -> (restype, argtypes): every symbol include/cao.h declares
+SIGNATURES = {
+    "cao_space_create": (C.c_int, [pvp]),
+    "cao_space_destroy": (None, [vp]),
+    "cao_space_add_param": (C.c_int, [vp, C.c_char_p, C.POINTER(C.c_int64), i32]),
+    "cao_space_add_constraint": (C.c_int, [vp, pi32, i32]),
+    "cao_space_set_build_mode": (C.c_int, [vp, i32]),
+    "cao_space_build_workspace_bytes": (C.c_int, [vp, pu64, pu64]),
+    "cao_space_build_count": (C.c_int, [vp, vp, vp, vp, pu64]),
+    "cao_space_table_bytes": (C.c_int, [vp, pu64]),
+    "cao_space_build_fill": (C.c_int, [vp, vp, vp]),
+    "cao_space_sizes": (C.c_int, [vp, pu64, pu64, pi32, pi32]),
+    "cao_space_views": (C.c_int, [vp, pvp, pvp, pvp, pvp]),
+    "cao_space_is_valid": (C.c_int, [vp, vp, u64, vp, vp]),
+    "cao_space_repair_scratch_bytes": (C.c_int, [vp, u64, pu64]),
+    "cao_space_repair": (C.c_int, [vp, vp, u64, vp, vp, i32, vp, vp]),
+    "cao_space_set_objective": (C.c_int, [vp, vp]),
+    "cao_runs_workspace_bytes": (C.c_int, [vp, i32, i32, u32, u32, pu64]),
+    "cao_runs_create": (C.c_int, [vp, i32, C.POINTER(HParams), u32, u32, i32, u32, u32, u64, vp, vp, pvp]),
+    "cao_runs_destroy": (None, [vp]),
+    "cao_runs_step": (C.c_int, [vp, u32, vp]),
+    "cao_runs_best": (C.c_int, [vp, vp, vp, vp, vp, vp]),
+    "cao_runs_trajectory": (C.c_int, [vp, pvp, C.POINTER(u32)]),
+    "cao_runs_debug_last": (C.c_int, [vp, pvp, pvp, pvp, pvp, pvp, pvp, pvp]),
+    "cao_runs_debug_state": (C.c_int, [vp, i32, pvp, pu64]),
+    "cao_runs_counters": (C.c_int, [vp, vp, pu64, pu64, pu64]),
+    "cao_launch_count": (u64, []),
+    "cao_test_philox": (C.c_int, [vp, vp, u64, vp]),
+    "cao_test_exp_neg": (C.c_int, [vp, vp, u64, vp]),
+    "cao_last_error": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def lib():
+    """Loads libcao.so (built by paper_2606_28372_b200/build.py); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_28372_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise CaoError(rc, (lib().cao_last_error() or b"").decode())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev_bytes(nbytes, device):
+    # torch's caching allocator returns >= 512-byte aligned blocks
+    t = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device=device)
+    assert t.data_ptr() % 256 == 0
+    return t
+
+
+def launch_count() -> int:
+    return int(lib().cao_launch_count())
+
+
+def _view(base: torch.Tensor, ptr: int, nbytes: int, dtype, shape):
+    off = ptr - base.data_ptr()
+    assert 0 <= off and off + nbytes <= base.numel(), "borrowed view outside its buffer"
+    return base[off:off + nbytes].view(dtype).view(*shape)
+
+
+class Space:
+    """P = (X, D, C), resolved on the GPU before tuning (L137)."""
+
+    def __init__(self, domains, programs, names=None, build_mode=0, device="cuda"):
+        L = lib()
+        self.device = torch.device(device)
+        h = C.c_void_p()
+        _check(L.cao_space_create(C.byref(h)))
+        self._h = h
+        self.m = [len(d) for d in domains]
+        for k, d in enumerate(domains):
+            a = np.ascontiguousarray(d, dtype=np.int64)
+            nm = (names[k] if names else f"p{k}").encode()
+            _check(L.cao_space_add_param(h, nm, a.ctypes.data_as(C.POINTER(C.c_int64)), a.size))
+        for prog in programs:
+            a = np.ascontiguousarray(prog, dtype=np.int32)
+            _check(L.cao_space_add_constraint(h, a.ctypes.data_as(pi32), a.size))
+        _check(L.cao_space_set_build_mode(h, build_mode))
+        self.built = False
+        self._bitmap = self._scratch = self._table = self._obj = None
+
+    @classmethod
+    def from_space(cls, sp, **kw):
+        return cls(sp.domains, sp.rpn, names=sp.param_names, **kw)
+
+    # -- S1
+    def alloc_build(self):
+        bb, sb = u64(), u64()
+        _check(lib().cao_space_build_workspace_bytes(self._h, C.byref(bb), C.byref(sb)))
+        self._bitmap = _dev_bytes(bb.value, self.device)
+        self._scratch = _dev_bytes(sb.value, self.device)
+
+    def build_count(self) -> int:
+        V = u64()
+        _check(lib().cao_space_build_count(self._h, self._bitmap.data_ptr(), self._scratch.data_ptr(), _stream(), C.byref(V)))
+        return V.value
+
+    def alloc_table(self):
+        tb = u64()
+        _check(lib().cao_space_table_bytes(self._h, C.byref(tb)))
+        if self._table is None or self._table.numel() < tb.value:
+            self._table = _dev_bytes(tb.value, self.device)
+
+    def build_fill(self):
+        _check(lib().cao_space_build_fill(self._h, self._table.data_ptr(), _stream()))
+        self.built = True
+
+    def build(self):
+        """cao_space_build_count + cao_space_build_fill with freshly allocated buffers; returns self."""
+        if self._bitmap is None:
+            self.alloc_build()
+        self.build_count()
+        self.alloc_table()
+        self.build_fill()
+        return self
+
+    def sizes(self):
+        N, V, n, rb = u64(), u64(), i32(), i32()
+        _check(lib().cao_space_sizes(self._h, C.byref(N), C.byref(V), C.byref(n), C.byref(rb)))
+        return N.value, V.value, n.value, rb.value
+
+    @property
+    def N(self): return self.sizes()[0]
+    @property
+    def V(self): return self.sizes()[1]
+    @property
+    def n(self): return len(self.m)
+    @property
+    def row_bytes(self): return 16 if self.n <= 16 else 32
+
+    def _views(self):
+        p = [C.c_void_p() for _ in range(4)]
+        _check(lib().cao_space_views(self._h, *[C.byref(x) for x in p]))
+        return [x.value for x in p]
+
+    def bitmap(self) -> torch.Tensor:
+        """ceil(N/64) int64 words (bit L&63 of word L>>6)."""
+        nw = (self.N + 63) // 64
+        return self._bitmap[:nw * 8].view(torch.int64)
+
+    def rows(self) -> torch.Tensor:
+        """(V, row_bytes) uint8, ascending L, padding zero."""
+        N, V, n, rb = self.sizes()
+        return _view(self._table, self._views()[1], V * rb, torch.uint8, (V, rb))
+
+    def Ltab(self) -> torch.Tensor:
+        N, V, n, rb = self.sizes()
+        return _view(self._table, self._views()[2], V * 8, torch.int64, (V,))
+
+    def rank_dir(self) -> torch.Tensor:
+        N, V, n, rb = self.sizes()
+        nd = (N + 511) // 512 + 1
+        return _view(self._table, self._views()[3], nd * 4, torch.int32, (nd,))
+
+    # -- queries (L139)
+    def pack_rows(self, rows) -> torch.Tensor:
+        """(count, n) host/device integer rows -> (count, row_bytes) uint8 device rows, padding zero."""
+        t = torch.as_tensor(np.ascontiguousarray(rows)) if not isinstance(rows, torch.Tensor) else rows
+        t = t.to(self.device).to(torch.uint8).reshape(-1, t.shape[-1])
+        if t.shape[1] == self.row_bytes:
+            return t.contiguous()
+        out = torch.zeros((t.shape[0], self.row_bytes), dtype=torch.uint8, device=self.device)
+        out[:, :t.shape[1]] = t
+        return out
+
+    def is_valid(self, rows) -> torch.Tensor:
+        r = self.pack_rows(rows)
+        out = torch.empty(r.shape[0], dtype=torch.uint8, device=self.device)
+        _check(lib().cao_space_is_valid(self._h, r.data_ptr(), r.shape[0], out.data_ptr(), _stream()))
+        return out
+
+    def repair(self, rows, use_probe=True):
+        """-> (rank int32-as-uint32 tensor, key int64 tensor: ham << 45 | sad << 32 | rank)."""
+        r = self.pack_rows(rows)
+        c = r.shape[0]
+        sb = u64()
+        _check(lib().cao_space_repair_scratch_bytes(self._h, c, C.byref(sb)))
+        scratch = _dev_bytes(sb.value, self.device)
+        rank = torch.empty(c, dtype=torch.int32, device=self.device)
+        key = torch.empty(c, dtype=torch.int64, device=self.device)
+        _check(lib().cao_space_repair(self._h, r.data_ptr(), c, rank.data_ptr(), key.data_ptr(), 1 if use_probe else 0,
+                                      scratch.data_ptr(), _stream()))
+        self._last_scratch = scratch
+        return rank, key
+
+    def set_objective(self, obj):
+        t = obj if isinstance(obj, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(obj, dtype=np.float32))
+        t = t.to(self.device, dtype=torch.float32).contiguous()
+        assert t.numel() == self.V
+        _check(lib().cao_space_set_objective(self._h, t.data_ptr()))
+        self._obj = t
+
+    def __del__(self):
+        try:
+            lib().cao_space_destroy(self._h)
+        except Exception:
+            pass
+
+
+class Runs:
+    """n_runs independent simulated tuning runs of one algorithm; creation executes generation 0 (S2)."""
+
+    def __init__(self, space: Space, algo, n_runs, pop, budget=0, max_gens=100, seed=0, first_run=0, hparams=None):
+        self.space, self.R, self.P, self.n = space, int(n_runs), int(pop), space.n
+        self.algo = ALGOS[algo] if isinstance(algo, str) else int(algo)
+        self.hp = hparams or HParams.default()
+        self.max_gens = int(max_gens)
+        wb = u64()
+        _check(lib().cao_runs_workspace_bytes(space._h, self.algo, self.P, self.R, self.max_gens, C.byref(wb)))
+        self.workspace_bytes = wb.value
+        self._ws = _dev_bytes(wb.value, space.device)
+        h = C.c_void_p()
+        _check(lib().cao_runs_create(space._h, self.algo, C.byref(self.hp), self.R, int(first_run), self.P, int(budget),
+                                     self.max_gens, int(seed), self._ws.data_ptr(), _stream(), C.byref(h)))
+        self._h = h
+
+    def step(self, k=1):
+        _check(lib().cao_runs_step(self._h, int(k), _stream()))
+
+    def best_into(self, best_f, best_rank, uniq, gens_done):
+        _check(lib().cao_runs_best(self._h, best_f.data_ptr(), best_rank.data_ptr(), uniq.data_ptr(), gens_done.data_ptr(),
+                                   _stream()))
+
+    def best(self):
+        dev = self.space.device
+        bf = torch.empty(self.R, dtype=torch.float32, device=dev)
+        br, uq, gd = (torch.empty(self.R, dtype=torch.int32, device=dev) for _ in range(3))
+        self.best_into(bf, br, uq, gd)
+        return dict(best_f=bf, best_rank=br, uniq=uq, gens_done=gd)
+
+    @property
+    def gen(self):
+        p, g = C.c_void_p(), u32()
+        _check(lib().cao_runs_trajectory(self._h, C.byref(p), C.byref(g)))
+        return g.value
+
+    def trajectory(self) -> torch.Tensor:
+        """(gen+1, R, 3) int32: {best_f bits, best_rank, uniq}."""
+        p, g = C.c_void_p(), u32()
+        _check(lib().cao_runs_trajectory(self._h, C.byref(p), C.byref(g)))
+        G = g.value + 1
+        return _view(self._ws, p.value, G * self.R * 12, torch.int32, (G, self.R, 3))
+
+    def taps(self):
+        p = [C.c_void_p() for _ in range(7)]
+        _check(lib().cao_runs_debug_last(self._h, *[C.byref(x) for x in p]))
+        R, P, rb = self.R, self.P, self.space.row_bytes
+        v = lambda k, nb, dt, shape: _view(self._ws, p[k].value, nb, dt, shape)
+        return dict(cand=v(0, R * P * rb, torch.uint8, (R, P, rb)), valid=v(1, R * P, torch.uint8, (R, P)),
+                    rep_rank=v(2, R * P * 4, torch.int32, (R, P)), eval_rank=v(3, R * P * 4, torch.int32, (R, P)),
+                    f=v(4, R * P * 4, torch.float32, (R, P)), accept=v(5, R * P, torch.uint8, (R, P)),
+                    active=v(6, R, torch.uint8, (R,)))
+
+    def _state(self, which, dtype, shape):
+        p, b = C.c_void_p(), u64()
+        _check(lib().cao_runs_debug_state(self._h, which, C.byref(p), C.byref(b)))
+        return _view(self._ws, p.value, b.value, dtype, shape)
+
+    def state(self):
+        """Population state; x / v / pbest are returned as (R, P, n) (stored dimension-major [run][dim][ind])."""
+        R, P, n, rb = self.R, self.P, self.n, self.space.row_bytes
+        out = dict(rank=self._state(1, torch.int32, (R, P)), f=self._state(2, torch.float32, (R, P)))
+        if self.algo in (0, 3):
+            out["idx"] = self._state(0, torch.uint8, (R, P, rb))[:, :, :n]
+        else:
+            out["x"] = self._state(3, torch.float32, (R, n, P)).permute(0, 2, 1)
+        if self.algo == 1:
+            out["v"] = self._state(4, torch.float32, (R, n, P)).permute(0, 2, 1)
+            out["pbest"] = self._state(5, torch.float32, (R, n, P)).permute(0, 2, 1)
+            out["pbest_f"] = self._state(6, torch.float32, (R, P))
+        return out
+
+    def counters(self):
+        a, b, c = u64(), u64(), u64()
+        _check(lib().cao_runs_counters(self._h, _stream(), C.byref(a), C.byref(b), C.byref(c)))
+        return dict(n_repaired=a.value, n_scanned=b.value, n_evaluated=c.value)
+
+    def __del__(self):
+        try:
+            lib().cao_runs_destroy(self._h)
+        except Exception:
+            pass
+
+
+def test_philox(ctr_key: torch.Tensor) -> torch.Tensor:
+    """(count, 6) int32 {c0,c1,c2,c3,k0,k1} -> (count, 4) int32 Philox4x32-10 outputs (device self-test, O3)."""
+    t = ctr_key.contiguous()
+    out = torch.empty((t.shape[0], 4), dtype=torch.int32, device=t.device)
+    _check(lib().cao_test_philox(t.data_ptr(), out.data_ptr(), t.shape[0], _stream()))
+    return out
+
+
+def test_exp_neg(z: torch.Tensor) -> torch.Tensor:
+    t = z.contiguous()
+    out = torch.empty_like(t)
+    _check(lib().cao_test_exp_neg(t.data_ptr(), out.data_ptr(), t.numel(), _stream()))
+    return out
+
+
+test_philox.__test__ = False
+test_exp_neg.__test__ = False

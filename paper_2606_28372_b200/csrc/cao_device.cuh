@@ -146,7 +146,7 @@ __device__ __forceinline__ int64_t sat_mul(int64_t a, int64_t b) {
 }
 
 // O1: postfix interpreter over the VALUES x[d]; returns 1/0; a zero divisor makes the constraint false.
-__device__ __noinline__ int eval_program(const int32_t* __restrict__ w, int nw, const int64_t* __restrict__ x) {
+static __device__ __noinline__ int eval_program(const int32_t* __restrict__ w, int nw, const int64_t* __restrict__ x) {
     int64_t st[CAO_MAX_STACK];
     int sp = 0;
     for (int pc = 0; pc < nw; ++pc) {
@@ -177,3 +177,46 @@ __device__ __noinline__ int eval_program(const int32_t* __restrict__ w, int nw, 
     }
     return st[0] != 0;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Packed index rows: ROWW uint32 words (ROWW = 4 for n <= 16, 8 for n <= 32), 16-byte aligned.
+template <int ROWW>
+__device__ __forceinline__ void load_row(const uint8_t* __restrict__ p, uint32_t (&w)[ROWW]) {
+    const uint4* q = (const uint4*)p;
+    uint4 a = __ldg(&q[0]); w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
+    if (ROWW == 8) { uint4 b = __ldg(&q[1]); w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w; }
+}
+template <int ROWW>
+__device__ __forceinline__ void load_row_rw(const uint8_t* p, uint32_t (&w)[ROWW]) {     // state written by earlier kernels
+    const uint4* q = (const uint4*)p;
+    uint4 a = q[0]; w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
+    if (ROWW == 8) { uint4 b = q[1]; w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w; }
+}
+template <int ROWW>
+__device__ __forceinline__ void store_row(uint8_t* p, const uint32_t (&w)[ROWW]) {
+    uint4* q = (uint4*)p;
+    q[0] = make_uint4(w[0], w[1], w[2], w[3]);
+    if (ROWW == 8) q[1] = make_uint4(w[4], w[5], w[6], w[7]);
+}
+template <int ROWW>
+__device__ __forceinline__ uint64_t row_lin(const SpaceMeta& sm, const uint32_t (&w)[ROWW]) {
+    uint64_t L = 0;
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d)
+        if (d < sm.n) L += (uint64_t)((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) * sm.stride[d];
+    return L;
+}
+
+// Sum of absolute byte differences with accumulate: one VABSDIFF4.U8.ACC.
+__device__ __forceinline__ uint32_t sad4_acc(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("vabsdiff4.u32.u32.u32.add %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+
+// Repair key (O9): ham << 45 | sad << 32 | rank; rank is monotone in L, so the order equals (ham, sad, L).
+#define CAO_KEY_NONE 0xFFFFFFFFFFFFFFFFull
+__device__ __forceinline__ uint64_t make_key(uint32_t ham, uint32_t sad, uint32_t rank) {
+    return ((uint64_t)ham << 45) | ((uint64_t)sad << 32) | rank;
+}
+__device__ __forceinline__ uint32_t fbits(float f) { return __float_as_uint(f); }

@@ -21,16 +21,6 @@ __device__ __forceinline__ void decode_row(const SpaceMeta& sm, uint64_t L, uint
     }
 }
 
-// L of a packed row.
-template <int ROWW>
-__device__ __forceinline__ uint64_t row_lin(const SpaceMeta& sm, const uint32_t (&w)[ROWW]) {
-    uint64_t L = 0;
-#pragma unroll
-    for (int d = 0; d < ROWW * 4; ++d)
-        if (d < sm.n) L += (uint64_t)((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) * sm.stride[d];
-    return L;
-}
-
 // One thread per 32-bit half word of the bitmap; the 16 lanes of a 512-config group share a directory
 // entry and find their row offsets with a 16-lane shuffle scan.  Rows are written in ascending L.
 template <int ROWW>

@@ -1,0 +1,136 @@
+// cao_repair_kernels.cuh -- S5: repair to the nearest valid configuration (O9).
+//
+// repair(c) = c if valid, else argmin over the valid table of (Hamming, sum |didx|, L).  Two exact routes:
+//   probe : the Hamming-1 neighbours of c are tested in the bitmap by increasing |delta|; the first level
+//           with a valid neighbour gives the minimum (1, |delta|, L') directly.
+//   scan  : candidates without a valid Hamming-1 neighbour are compacted into a worklist; each CTA takes a
+//           tile of 128 candidates (one per thread, row in registers) and a chunk of the valid table, staged
+//           through shared memory in 512-row tiles and read back as broadcast LDS.128; per (candidate,row):
+//           one VABSDIFF4.ACC per word for sum|didx|, a carry trick + one POPC per row for the Hamming count.
+//           Chunks of the same candidate are merged with a 64-bit atomicMin on the packed key (order-free).
+#pragma once
+#include "cao_host.h"
+
+// Hamming-1 probe of an INVALID, in-domain row with linear index L.  Returns the key or CAO_KEY_NONE.
+template <int ROWW>
+__device__ __forceinline__ uint64_t probe_h1(const SpaceMeta& sm, const uint32_t (&w)[ROWW], uint64_t L) {
+    for (int delta = 1; delta < sm.M; ++delta) {
+        uint64_t bestL = ~0ull;
+#pragma unroll
+        for (int d = 0; d < ROWW * 4; ++d) {
+            if (d < sm.n) {
+                int c = (int)((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu);
+                uint64_t step = (uint64_t)delta * sm.stride[d];
+                if (c >= delta) { uint64_t L2 = L - step; if (L2 < bestL && bit_test(sm.bitmap, L2)) bestL = L2; }
+                if (c + delta < (int)sm.m[d]) { uint64_t L2 = L + step; if (L2 < bestL && bit_test(sm.bitmap, L2)) bestL = L2; }
+            }
+        }
+        if (bestL != ~0ull) return make_key(1u, (uint32_t)delta, rank_of(sm, bestL));
+    }
+    return CAO_KEY_NONE;
+}
+
+// Validity + probe of one row; in_domain = every index byte is < m_d.
+template <int ROWW>
+__device__ __forceinline__ uint64_t validate_probe(const SpaceMeta& sm, const uint32_t (&w)[ROWW], bool use_probe, bool& valid) {
+    bool in_dom = true;
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d)
+        if (d < sm.n && ((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) >= sm.m[d]) in_dom = false;
+    valid = false;
+    if (!in_dom) return CAO_KEY_NONE;
+    uint64_t L = row_lin<ROWW>(sm, w);
+    if (bit_test(sm.bitmap, L)) { valid = true; return make_key(0, 0, rank_of(sm, L)); }
+    return use_probe ? probe_h1<ROWW>(sm, w, L) : CAO_KEY_NONE;
+}
+
+// Appends `slot` to the worklist (warp-aggregated by the compiler's REDUX path or plain atomics; order-free).
+__device__ __forceinline__ void worklist_push(uint32_t* wl, uint32_t* wl_count, uint32_t slot) {
+    uint32_t pos = atomicAdd(wl_count, 1u);
+    wl[pos] = slot;
+}
+
+#define SCAN_TC 128          // candidates per tile = threads per CTA
+#define SCAN_TR 512          // valid rows per shared-memory tile
+
+// WU = words of a row that carry indices (ceil(n/4)); row stride in HBM = 4 or 8 words.
+// SMALL: every index < 128, so a byte of c^v is non-zero iff adding 0x7f carries into its bit 7.
+template <int WU, bool SMALL>
+__global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
+                                                  const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
+                                                  unsigned long long* key) {
+    constexpr int ROWW = WU <= 4 ? 4 : 8;
+    __shared__ uint4 tile[SCAN_TR * (ROWW / 4)];
+    const uint32_t count = *wl_count;
+    if (count == 0 || sm.V == 0) return;
+    const uint32_t tid = threadIdx.x;
+    const uint32_t ntiles = (count + SCAN_TC - 1) / SCAN_TC;
+    const uint32_t nrt = (sm.V + SCAN_TR - 1) / SCAN_TR;                 // row tiles in the table
+    uint32_t nchunks = gridDim.x / ntiles; if (nchunks < 1) nchunks = 1; if (nchunks > nrt) nchunks = nrt;
+    const uint32_t tpc = (nrt + nchunks - 1) / nchunks;                  // row tiles per chunk
+    nchunks = (nrt + tpc - 1) / tpc;
+    const uint64_t items = (uint64_t)ntiles * nchunks;
+    for (uint64_t item = blockIdx.x; item < items; item += gridDim.x) {
+        const uint32_t ct = (uint32_t)(item / nchunks), rc = (uint32_t)(item - (uint64_t)ct * nchunks);
+        const uint32_t ci = ct * SCAN_TC + tid;
+        const bool has = ci < count;
+        const uint32_t slot = has ? wl[ci] : 0;
+        uint32_t c[ROWW];
+        if (has) load_row_rw<ROWW>(cand_rows + (uint64_t)slot * (ROWW * 4), c);
+        else { for (int k = 0; k < ROWW; ++k) c[k] = 0; }
+        uint32_t bestk = 0xFFFFFFFFu, bestr = 0xFFFFFFFFu;
+        uint32_t rt1 = (rc + 1) * tpc; if (rt1 > nrt) rt1 = nrt;
+        for (uint32_t rt = rc * tpc; rt < rt1; ++rt) {
+            const uint32_t r0 = rt * SCAN_TR;
+            const uint32_t nr = min((uint32_t)SCAN_TR, sm.V - r0);
+            __syncthreads();
+            const uint4* src = (const uint4*)(sm.rows + (uint64_t)r0 * (ROWW * 4));
+            for (uint32_t q = tid; q < nr * (ROWW / 4); q += SCAN_TC) tile[q] = __ldg(&src[q]);
+            __syncthreads();
+#pragma unroll 4
+            for (uint32_t r = 0; r < nr; ++r) {
+                uint32_t v[ROWW];
+                { uint4 a = tile[r * (ROWW / 4)]; v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; }
+                if (ROWW == 8) { uint4 b = tile[r * 2 + 1]; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w; }
+                uint32_t sad = 0, hb = 0, ham = 0;
+#pragma unroll
+                for (int k = 0; k < WU; ++k) {
+                    sad = sad4_acc(c[k], v[k], sad);
+                    uint32_t x = c[k] ^ v[k];
+                    uint32_t t = SMALL ? (x + 0x7f7f7f7fu) : (((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x);
+                    if ((k & 3) == 0 && k) { ham += __popc(hb); hb = 0; }
+                    hb |= (t & 0x80808080u) >> (k & 3);
+                }
+                ham += __popc(hb);
+                uint32_t k32 = (ham << 13) + sad;
+                if (k32 < bestk) { bestk = k32; bestr = r0 + r; }         // ascending rank: ties keep the smallest L
+            }
+        }
+        if (has && bestr != 0xFFFFFFFFu) atomicMin(&key[slot], ((unsigned long long)bestk << 32) | bestr);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Standalone batched repair (cao_space_repair): probe kernel, k_scan, finish kernel.
+template <int ROWW>
+__global__ void __launch_bounds__(256) k_repair_probe(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ rows_in,
+                                                      uint64_t count, int use_probe, unsigned long long* key,
+                                                      uint32_t* wl, uint32_t* wl_count) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    uint32_t w[ROWW];
+    load_row<ROWW>(rows_in + i * (ROWW * 4), w);
+    bool valid;
+    uint64_t k = validate_probe<ROWW>(sm, w, use_probe != 0, valid);
+    key[i] = k;
+    if (k == CAO_KEY_NONE) worklist_push(wl, wl_count, (uint32_t)i);
+}
+
+__global__ void __launch_bounds__(256) k_repair_finish(const unsigned long long* __restrict__ key, uint64_t count,
+                                                       uint32_t* rank_out, uint64_t* key_out) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    unsigned long long k = key[i];
+    if (rank_out) rank_out[i] = (uint32_t)k;
+    if (key_out) key_out[i] = k;
+}

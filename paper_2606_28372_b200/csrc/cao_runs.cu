@@ -1,0 +1,312 @@
+// cao_runs.cu -- host side of the repair query and of the runs half of include/cao.h (S2-S7).
+#include <algorithm>
+#include <cstring>
+#include "cao_runs_kernels.cuh"
+
+#define SCAN_GRID (148 * 8)
+
+struct cao_runs {
+    const cao_space* s = nullptr;
+    SpaceMeta sm{};
+    RunsMeta rm{};
+    uint32_t gen = 0;
+    unsigned block = 32;
+    size_t smem_init = 0, smem_op = 0, smem_fin = 0;
+    // raw state views for cao_runs_debug_state
+    uint64_t bytes_idx = 0, bytes_pi = 0, bytes_pn = 0;
+};
+
+// ---------------------------------------------------------------------------------------------
+template <int WU>
+static void launch_scan_wu(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
+                           unsigned long long* key, cudaStream_t st) {
+    if (sm.M <= 128) k_scan<WU, true><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
+    else k_scan<WU, false><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
+}
+static int launch_scan(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
+                       unsigned long long* key, cudaStream_t st) {
+    switch ((sm.n + 3) / 4) {
+        case 1: launch_scan_wu<1>(sm, cand, wl, wl_count, key, st); break;
+        case 2: launch_scan_wu<2>(sm, cand, wl, wl_count, key, st); break;
+        case 3: launch_scan_wu<3>(sm, cand, wl, wl_count, key, st); break;
+        case 4: launch_scan_wu<4>(sm, cand, wl, wl_count, key, st); break;
+        case 5: launch_scan_wu<5>(sm, cand, wl, wl_count, key, st); break;
+        case 6: launch_scan_wu<6>(sm, cand, wl, wl_count, key, st); break;
+        case 7: launch_scan_wu<7>(sm, cand, wl, wl_count, key, st); break;
+        default: launch_scan_wu<8>(sm, cand, wl, wl_count, key, st); break;
+    }
+    CAO_LAUNCHED("k_scan");
+    return CAO_OK;
+}
+
+// Dispatch over (algorithm, row words).
+#define DISPATCH_ALGO_ROWW(algo, roww, CALL)                                         \
+    do {                                                                             \
+        if ((roww) == 4) {                                                           \
+            switch (algo) {                                                          \
+                case CAO_DE: { CALL(CAO_DE, 4); } break;                             \
+                case CAO_PSO: { CALL(CAO_PSO, 4); } break;                           \
+                case CAO_FIREFLY: { CALL(CAO_FIREFLY, 4); } break;                   \
+                default: { CALL(CAO_GA, 4); } break;                                 \
+            }                                                                        \
+        } else {                                                                     \
+            switch (algo) {                                                          \
+                case CAO_DE: { CALL(CAO_DE, 8); } break;                             \
+                case CAO_PSO: { CALL(CAO_PSO, 8); } break;                           \
+                case CAO_FIREFLY: { CALL(CAO_FIREFLY, 8); } break;                   \
+                default: { CALL(CAO_GA, 8); } break;                                 \
+            }                                                                        \
+        }                                                                            \
+    } while (0)
+
+extern "C" {
+
+// ---------------------------------------------------------------------------------------------
+int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes) {
+    if (!s || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_scratch_bytes: NULL argument");
+    *bytes = align256(std::max<uint64_t>(1, count) * 8) + align256(std::max<uint64_t>(1, count) * 4) + 256;
+    return CAO_OK;
+}
+
+int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
+                     uint64_t* d_key_out, int32_t use_probe, void* d_scratch, void* stream) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair: NULL space");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_repair: space not built");
+    if (count == 0) return CAO_OK;
+    if (!d_idx_rows || (!d_rank_out && !d_key_out)) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair: NULL argument");
+    if (count >= (1ull << 32)) return cao_fail(CAO_E_TOO_LARGE, "cao_space_repair: count >= 2^32");
+    if (s->meta.V == 0) return cao_fail(CAO_E_EMPTY_SPACE, "cao_space_repair: the space has no valid configuration");
+    if (!d_scratch || ((uintptr_t)d_scratch & 255) || ((uintptr_t)d_idx_rows & 15))
+        return cao_fail(CAO_E_WORKSPACE, "cao_space_repair: scratch must be 256-byte aligned, rows 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    uint8_t* sc = (uint8_t*)d_scratch;
+    unsigned long long* key = (unsigned long long*)sc;
+    uint32_t* wl = (uint32_t*)(sc + align256(count * 8));
+    uint32_t* wl_count = (uint32_t*)(sc + align256(count * 8) + align256(count * 4));
+    CAO_CUDA(cudaMemsetAsync(wl_count, 0, 4, st));
+    unsigned grid = (unsigned)((count + 255) / 256);
+    if (s->meta.rowB == 16) k_repair_probe<4><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, use_probe, key, wl, wl_count);
+    else k_repair_probe<8><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, use_probe, key, wl, wl_count);
+    CAO_LAUNCHED("k_repair_probe");
+    int rc = launch_scan(s->meta, d_idx_rows, wl, wl_count, key, st);
+    if (rc) return rc;
+    k_repair_finish<<<grid, 256, 0, st>>>(key, count, d_rank_out, d_key_out);
+    CAO_LAUNCHED("k_repair_finish");
+    return CAO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+struct RunsLayout {
+    uint64_t cand, key, valid, rep_rank, eval_rank, tap_f, accept, active, idx, rank, f, x, v, pb, pbf, dedup,
+        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl_count, counters, total;
+    uint64_t zero_from, zero_bytes;       // region that must start as zero: dedup .. stagn
+    uint32_t dedup_words;
+};
+
+static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_t R, uint64_t max_gens) {
+    RunsLayout L{};
+    const uint64_t RP = R * P, rowB = sm.rowB, n = sm.n;
+    uint64_t off = 0;
+    auto take = [&](uint64_t bytes) { uint64_t o = off; off = align256(off + std::max<uint64_t>(1, bytes)); return o; };
+    L.cand = take(RP * rowB); L.key = take(RP * 8); L.valid = take(RP); L.rep_rank = take(RP * 4);
+    L.eval_rank = take(RP * 4); L.tap_f = take(RP * 4); L.accept = take(RP); L.active = take(R);
+    const bool cont = algo == CAO_PSO || algo == CAO_FIREFLY;
+    L.idx = take(cont ? 0 : RP * rowB); L.rank = take(RP * 4); L.f = take(RP * 4);
+    L.x = take(cont ? RP * n * 4 : 0);
+    L.v = take(algo == CAO_PSO ? RP * n * 4 : 0); L.pb = take(algo == CAO_PSO ? RP * n * 4 : 0);
+    L.pbf = take(algo == CAO_PSO ? RP * 4 : 0);
+    L.dedup_words = (uint32_t)(((uint64_t)sm.V + 31) / 32);
+    L.zero_from = off;
+    L.dedup = take(R * L.dedup_words * 4);
+    L.uniq = take(R * 4); L.gens_done = take(R * 4); L.stagn = take(R * 4);
+    L.wl_count = take(4); L.counters = take(3 * 8);
+    L.zero_bytes = off - L.zero_from;
+    L.best_rank = take(R * 4); L.best_f = take(R * 4);
+    L.traj = take((max_gens + 1) * R * 12);
+    L.wl = take(RP * 4);
+    L.total = off;
+    return L;
+}
+
+static int check_runs_args(const cao_space* s, int32_t algo, int32_t pop, uint32_t n_runs, uint32_t max_gens) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "runs: NULL space");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "runs: space not built");
+    if (algo < 0 || algo > 3) return cao_fail(CAO_E_INVALID_ARG, "runs: unknown algorithm");
+    if (pop < 1 || n_runs < 1) return cao_fail(CAO_E_INVALID_ARG, "runs: pop and n_runs must be >= 1");
+    if (pop > 1024) return cao_fail(CAO_E_TOO_LARGE, "runs: pop > 1024");
+    if (s->meta.V == 0) return cao_fail(CAO_E_EMPTY_SPACE, "runs: the space has no valid configuration");
+    if ((uint64_t)pop > s->meta.V) return cao_fail(CAO_E_POP_GT_VALID, "runs: population larger than the number of valid configurations");
+    if (algo == CAO_DE && pop < 3) return cao_fail(CAO_E_INVALID_ARG, "runs: DE needs pop >= 3");
+    if (algo == CAO_GA && pop < 2) return cao_fail(CAO_E_INVALID_ARG, "runs: GA needs pop >= 2");
+    if ((uint64_t)pop * n_runs >= (1ull << 32)) return cao_fail(CAO_E_TOO_LARGE, "runs: pop * n_runs >= 2^32");
+    if (max_gens >= (1u << 24)) return cao_fail(CAO_E_TOO_LARGE, "runs: max_gens >= 2^24");
+    return CAO_OK;
+}
+
+int cao_runs_workspace_bytes(const cao_space* s, int32_t algo, int32_t pop, uint32_t n_runs, uint32_t max_gens, uint64_t* bytes) {
+    if (!bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_workspace_bytes: NULL argument");
+    int rc = check_runs_args(s, algo, pop, n_runs, max_gens);
+    if (rc) return rc;
+    *bytes = runs_layout(s->meta, algo, (uint64_t)pop, n_runs, max_gens).total;
+    return CAO_OK;
+}
+
+int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uint32_t n_runs, uint32_t first_run, int32_t pop,
+                    uint32_t budget_unique, uint32_t max_gens, uint64_t seed, void* d_workspace, void* stream, cao_runs** out) {
+    if (!out || !hp) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_create: NULL argument");
+    int rc = check_runs_args(s, algo, pop, n_runs, max_gens);
+    if (rc) return rc;
+    if (!s->meta.obj) return cao_fail(CAO_E_STATE, "cao_runs_create: call cao_space_set_objective first");
+    if (algo == CAO_GA && (hp->ga_beta_b < 1 || hp->ga_beta_b > 16 || hp->ga_mutation_chance < 1))
+        return cao_fail(CAO_E_INVALID_ARG, "cao_runs_create: ga_beta_b must be 1..16 and ga_mutation_chance >= 1");
+    if (!d_workspace || ((uintptr_t)d_workspace & 255)) return cao_fail(CAO_E_WORKSPACE, "cao_runs_create: workspace must be non-NULL and 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const RunsLayout L = runs_layout(s->meta, algo, (uint64_t)pop, n_runs, max_gens);
+    uint8_t* w = (uint8_t*)d_workspace;
+    cao_runs* r = new cao_runs();
+    r->s = s; r->sm = s->meta;
+    RunsMeta& m = r->rm;
+    m.R = n_runs; m.first_run = first_run; m.P = (uint32_t)pop; m.budget = budget_unique; m.max_gens = max_gens;
+    m.dedup_words = L.dedup_words; m.algo = algo; m.seed = seed; m.hp = *hp;
+    m.cand = w + L.cand; m.key = (unsigned long long*)(w + L.key); m.valid = w + L.valid;
+    m.rep_rank = (uint32_t*)(w + L.rep_rank); m.eval_rank = (uint32_t*)(w + L.eval_rank); m.tap_f = (float*)(w + L.tap_f);
+    m.accept = w + L.accept; m.active = w + L.active;
+    m.idx = w + L.idx; m.rank = (uint32_t*)(w + L.rank); m.f = (float*)(w + L.f);
+    m.x = (float*)(w + L.x); m.v = (float*)(w + L.v); m.pb = (float*)(w + L.pb); m.pbf = (float*)(w + L.pbf);
+    m.dedup = (uint32_t*)(w + L.dedup); m.uniq = (uint32_t*)(w + L.uniq); m.gens_done = (uint32_t*)(w + L.gens_done);
+    m.stagn = (uint32_t*)(w + L.stagn); m.best_rank = (uint32_t*)(w + L.best_rank); m.best_f = (float*)(w + L.best_f);
+    m.traj = (uint32_t*)(w + L.traj); m.wl = (uint32_t*)(w + L.wl); m.wl_count = (uint32_t*)(w + L.wl_count);
+    m.counters = (unsigned long long*)(w + L.counters);
+    const uint64_t RP = (uint64_t)n_runs * pop;
+    r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
+    r->block = (unsigned)((pop + 31) / 32 * 32);
+    const size_t P = (size_t)pop, n = (size_t)s->meta.n;
+    r->smem_init = P * 4;
+    r->smem_op = algo == CAO_GA ? P * 12 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
+    r->smem_fin = algo == CAO_DE ? P * 8 : 0;
+    int rc2 = CAO_OK;
+    do {
+        if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.zero_from, 0, L.zero_bytes, st), "memset state"))) break;
+        if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.best_rank, 0xFF, (uint64_t)n_runs * 4, st), "memset best_rank"))) break;
+        if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.cand, 0, L.idx - L.cand, st), "memset taps"))) break;
+#define CALL_INIT(A, W) \
+        if (r->smem_op > 48 * 1024) cudaFuncSetAttribute(k_op<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
+        k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
+        DISPATCH_ALGO_ROWW(algo, s->meta.rowB / 4, CALL_INIT);
+        ++g_cao_launches;
+        rc2 = cao_cuda_check(cudaGetLastError(), "k_init");
+    } while (0);
+    if (rc2) { delete r; return rc2; }
+    *out = r;
+    return CAO_OK;
+}
+
+void cao_runs_destroy(cao_runs* r) { delete r; }
+
+int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
+    if (!r) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_step: NULL runs");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int algo = r->rm.algo, roww = r->sm.rowB / 4;
+    for (uint32_t it = 0; it < n_generations; ++it) {
+        if (r->gen >= r->rm.max_gens) break;                            // g <= max_gens (O10)
+        const uint32_t g = r->gen + 1;
+#define CALL_OP(A, W) k_op<A, W><<<r->rm.R, r->block, r->smem_op, st>>>(r->sm, r->rm, g)
+        DISPATCH_ALGO_ROWW(algo, roww, CALL_OP);
+        CAO_LAUNCHED("k_op");
+        int rc = launch_scan(r->sm, r->rm.cand, r->rm.wl, r->rm.wl_count, r->rm.key, st);
+        if (rc) return rc;
+#define CALL_FIN(A, W) k_finish<A, W><<<r->rm.R, r->block, r->smem_fin, st>>>(r->sm, r->rm, g)
+        DISPATCH_ALGO_ROWW(algo, roww, CALL_FIN);
+        CAO_LAUNCHED("k_finish");
+        r->gen = g;
+    }
+    return CAO_OK;
+}
+
+int cao_runs_best(const cao_runs* r, float* d_best_f, uint32_t* d_best_rank, uint32_t* d_uniq, uint32_t* d_gens_done, void* stream) {
+    if (!r) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_best: NULL runs");
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t b = (uint64_t)r->rm.R * 4;
+    if (d_best_f) CAO_CUDA(cudaMemcpyAsync(d_best_f, r->rm.best_f, b, cudaMemcpyDeviceToDevice, st));
+    if (d_best_rank) CAO_CUDA(cudaMemcpyAsync(d_best_rank, r->rm.best_rank, b, cudaMemcpyDeviceToDevice, st));
+    if (d_uniq) CAO_CUDA(cudaMemcpyAsync(d_uniq, r->rm.uniq, b, cudaMemcpyDeviceToDevice, st));
+    if (d_gens_done) CAO_CUDA(cudaMemcpyAsync(d_gens_done, r->rm.gens_done, b, cudaMemcpyDeviceToDevice, st));
+    return CAO_OK;
+}
+
+int cao_runs_trajectory(const cao_runs* r, const void** d_traj, uint32_t* gens_recorded) {
+    if (!r) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_trajectory: NULL runs");
+    if (d_traj) *d_traj = r->rm.traj;
+    if (gens_recorded) *gens_recorded = r->gen;
+    return CAO_OK;
+}
+
+int cao_runs_debug_last(const cao_runs* r, const uint8_t** d_postsnap_rows, const uint8_t** d_valid, const uint32_t** d_repaired_rank,
+                        const uint32_t** d_eval_rank, const float** d_f, const uint8_t** d_accept, const uint8_t** d_active) {
+    if (!r) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_debug_last: NULL runs");
+    if (d_postsnap_rows) *d_postsnap_rows = r->rm.cand;
+    if (d_valid) *d_valid = r->rm.valid;
+    if (d_repaired_rank) *d_repaired_rank = r->rm.rep_rank;
+    if (d_eval_rank) *d_eval_rank = r->rm.eval_rank;
+    if (d_f) *d_f = r->rm.tap_f;
+    if (d_accept) *d_accept = r->rm.accept;
+    if (d_active) *d_active = r->rm.active;
+    return CAO_OK;
+}
+
+int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, uint64_t* bytes) {
+    if (!r || !d_ptr || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_debug_state: NULL argument");
+    const int a = r->rm.algo;
+    const bool cont = a == CAO_PSO || a == CAO_FIREFLY;
+    switch (which) {
+        case 0: if (cont) break; *d_ptr = r->rm.idx; *bytes = r->bytes_idx; return CAO_OK;
+        case 1: *d_ptr = r->rm.rank; *bytes = r->bytes_pi; return CAO_OK;
+        case 2: *d_ptr = r->rm.f; *bytes = r->bytes_pi; return CAO_OK;
+        case 3: if (!cont) break; *d_ptr = r->rm.x; *bytes = r->bytes_pn; return CAO_OK;
+        case 4: if (a != CAO_PSO) break; *d_ptr = r->rm.v; *bytes = r->bytes_pn; return CAO_OK;
+        case 5: if (a != CAO_PSO) break; *d_ptr = r->rm.pb; *bytes = r->bytes_pn; return CAO_OK;
+        case 6: if (a != CAO_PSO) break; *d_ptr = r->rm.pbf; *bytes = r->bytes_pi; return CAO_OK;
+        default: break;
+    }
+    return cao_fail(CAO_E_INVALID_ARG, "cao_runs_debug_state: this algorithm has no such state array");
+}
+
+int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uint64_t* n_scanned, uint64_t* n_evaluated) {
+    if (!r) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_counters: NULL runs");
+    unsigned long long h[3] = {0, 0, 0};
+    CAO_CUDA(cudaMemcpyAsync(h, r->rm.counters, 24, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CAO_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    if (n_repaired) *n_repaired = h[0];
+    if (n_scanned) *n_scanned = h[1];
+    if (n_evaluated) *n_evaluated = h[2];
+    return CAO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+__global__ void k_test_philox(const uint32_t* __restrict__ in, uint32_t* out, uint64_t count) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const uint32_t* p = in + i * 6;
+    uint4 r = philox4x32_10(make_uint4(p[0], p[1], p[2], p[3]), p[4], p[5]);
+    ((uint4*)out)[i] = r;
+}
+__global__ void k_test_exp_neg(const float* __restrict__ z, float* out, uint64_t count) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) out[i] = exp_neg_spec(z[i]);
+}
+int cao_test_philox(const uint32_t* d_ctr_key, uint32_t* d_out, uint64_t count, void* stream) {
+    if (count == 0) return CAO_OK;
+    if (!d_ctr_key || !d_out) return cao_fail(CAO_E_INVALID_ARG, "cao_test_philox: NULL argument");
+    k_test_philox<<<(unsigned)((count + 255) / 256), 256, 0, (cudaStream_t)stream>>>(d_ctr_key, d_out, count);
+    CAO_LAUNCHED("k_test_philox");
+    return CAO_OK;
+}
+int cao_test_exp_neg(const float* d_z, float* d_out, uint64_t count, void* stream) {
+    if (count == 0) return CAO_OK;
+    if (!d_z || !d_out) return cao_fail(CAO_E_INVALID_ARG, "cao_test_exp_neg: NULL argument");
+    k_test_exp_neg<<<(unsigned)((count + 255) / 256), 256, 0, (cudaStream_t)stream>>>(d_z, d_out, count);
+    CAO_LAUNCHED("k_test_exp_neg");
+    return CAO_OK;
+}
+
+}  // extern "C"
