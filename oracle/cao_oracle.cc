@@ -192,6 +192,8 @@ void enumerate(Space& s) {
     // idx holds the mixed-radix digits of L, idx_d = (L / stride_d) mod m_d; it is advanced like an odometer
     // (last digit fastest) instead of re-dividing every L.  orc_space_count_range() below does the literal
     // division decode and the tests check the two against each other.
+    // The odometer counts in unsigned (a 256-value digit must reach 256 to carry); idx is its byte copy.
+    unsigned odo[32] = { 0 };
     uint8_t idx[32] = { 0 };
     for (uint64_t L = 0; L < s.N; ++L) {
         if (s.valid_idx(idx)) {
@@ -200,8 +202,8 @@ void enumerate(Space& s) {
             s.Ltab.push_back(L);
         }
         for (int d = s.n - 1; d >= 0; --d) {
-            if (++idx[d] < s.dom[d].size()) break;
-            idx[d] = 0;
+            if (++odo[d] < s.dom[d].size()) { idx[d] = (uint8_t)odo[d]; break; }
+            odo[d] = 0; idx[d] = 0;
         }
     }
     s.V = s.Ltab.size();

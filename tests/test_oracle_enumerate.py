@@ -177,3 +177,16 @@ def test_repair_identity_on_every_valid_config_cfg1_sample():
     pick = np.random.default_rng(0).integers(0, s.V, 40)
     got = s.repair(rows[pick])
     assert (got["rank"] == pick).all() and (got["ham"] == 0).all() and (got["sad"] == 0).all()
+
+
+def test_256_value_digit_carries():
+    """O1: idx_d = (L / stride_d) mod m_d also for m_d = 256, the largest domain the boundary allows (a byte
+    odometer would wrap without carrying).  Closed form: #{(a, b) in [0,200) x [0,256): (a + b) % 7 == 3}."""
+    from workloads import P
+    doms = [list(range(200)), list(range(256))]
+    s = O.OracleSpace(doms, [((P(0) + P(1)) % 7).eq(3).program()]).build()
+    want = sum(1 for a in range(200) for b in range(256) if (a + b) % 7 == 3)
+    assert s.V == want == s.count_range(0, 200 * 256)
+    rows = s.rows()
+    assert ((rows[:, 0].astype(int) + rows[:, 1].astype(int)) % 7 == 3).all()
+    assert np.array_equal(s.Ltab(), rows[:, 0].astype(np.uint64) * 256 + rows[:, 1].astype(np.uint64))
