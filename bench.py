@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- whole-hot-path throughput of the batched constraint-aware generation step on B200.
+
+One "step" = one pass of every S-row of the hot path over one batch of synthetic input:
+  S1  build the search space on the GPU (bitmap, valid table, rank directory)
+  S2  create R runs of each algorithm (generation 0)
+  S3-S7  step every run until its budget of unique evaluations / the generation cap
+  read best-so-far.
+Workload at N=1: BASELINE.json configs[1] (GEMM-like space, DE+PSO+Firefly+GA, pop 32, budget 1000 unique
+evaluations, cap 200 generations, 1000 runs each).  N>1: every rank processes its own 1000 runs per algorithm
+(run indices rank*1000..), no data-path collective (weak scaling).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+ALGO_GENS_CAP = {1: 200, 0: 50, 2: 150, 3: 100, 4: 200}
+ISSUE_LANES_PER_SM_CLK = 128          # 4 SMSP x 32 lanes: one warp instruction per SMSP per clock (B300_MICROARCH.md)
+N_SM = 148
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def workload(cfg: int, runs: int | None):
+    import workloads as W
+    w = W.WORKLOADS[cfg]
+    return dict(cfg=cfg, space=w.space(), algos=list(w.algos), pop=w.pop, gens=w.gens, runs=runs or w.runs,
+                budget=w.budget, seed=w.seed)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.sm_max = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {getattr(nv, k): k for k in dir(nv) if k.startswith("nvmlClocksEventReason") or k.startswith("nvmlClocksThrottleReason")}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if isinstance(bit, int) and bit and (r & bit) == bit and bin(bit).count("1") == 1:
+                        self.reasons.add(nm.replace("nvmlClocksEventReason", "").replace("nvmlClocksThrottleReason", ""))
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def summary(self):
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["unavailable"]}
+        drop = {"None", "GpuIdle", "ApplicationsClocksSetting"}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": float(self.sm_max),
+                "reasons": sorted(x for x in self.reasons if x not in drop)}
+
+
+# ----------------------------------------------------------------------------------------------------------
+def oracle_sample_step(wl, R_o):
+    """One bounded pass of the hot path on the CPU oracle: returns (candidates evaluated, seconds)."""
+    import oracle as O
+    import workloads as W
+    sp = wl["space"]
+    t0 = time.perf_counter()
+    s = O.OracleSpace.from_space(sp).build()
+    s.set_objective(W.objective_table(s.rows(), sp.m, 0))
+    cands = 0
+    for algo in wl["algos"]:
+        r = O.OracleRuns(s, algo, n_runs=R_o, pop=wl["pop"], budget=wl["budget"], max_gens=wl["gens"], seed=wl["seed"])
+        r.step(wl["gens"])
+        cands += r.n_evaluated
+    return cands, time.perf_counter() - t0
+
+
+def oracle_sample_text(wl, R_o):
+    sp = wl["space"]
+    return (f"full space build (N={sp.N}) + first {R_o} runs of each of {len(wl['algos'])} algorithms "
+            f"(pop {wl['pop']}, budget {wl['budget']}, cap {wl['gens']} generations), single thread")
+
+
+def reference_arm(args):
+    """The CPU oracle as it stands, on the host cores, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = workload(args.config, None)
+    sp = wl["space"]
+    sample = oracle_sample_text(wl, args.ref_runs)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample_step(wl, args.ref_runs)
+    tot_c, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        c, t = oracle_sample_step(wl, args.ref_runs)
+        tot_c += c; tot_t += t
+    val = tot_c / tot_t
+    line = {"impl": "reference", "metric": "candidates_repaired_evaluated_per_s", "value": val, "unit": "candidates/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/u64 integer + f32 (no FMA)",
+            "data": "synthetic", "config": {"workload": f"BASELINE configs[{args.config}] ({sp.name}), bounded sample: {sample}"},
+            "cpu_baseline": {"value": val, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "candidates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------------------
+def scan_ops_per_pair(n):
+    """Integer instructions per (candidate, valid row) of k_scan: per index word
+    VABSDIFF4.ACC + XOR + ADD + AND/OR-merge (+ shift), per row POPC + key pack + compare/select x2 + LDS."""
+    wu = (n + 3) // 4
+    return 5 * wu + 6
+
+
+def enum_bytes(N, V, row_bytes):
+    """Algorithmic bytes of S1: bitmap + rank directory + rows + Ltab."""
+    return N / 8 + N / 128 + V * (row_bytes + 8)
+
+
+def gpu_arm(args):
+    import torch
+    import torch.distributed as dist
+    import workloads as W
+    import paper_2606_28372_b200 as cao
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    pk = peaks()
+    wl = workload(args.config, args.runs)
+    sp, R, P, G = wl["space"], wl["runs"], wl["pop"], wl["gens"]
+    first_run = rank * R
+
+    # inputs resident in HBM before the timed region: the objective table (indexed by valid rank, so it is
+    # derived once from a first build of the same space) on the device and in pinned host memory
+    g0 = cao.Space.from_space(sp).build()
+    N, V, n, rb = g0.sizes()
+    obj = W.objective_table(g0.rows().cpu().numpy(), sp.m, 0)
+    obj_d = torch.from_numpy(obj).to(dev)
+    obj_h = torch.from_numpy(obj).pin_memory()
+    host_out = [torch.empty(4 * R, dtype=torch.int32).pin_memory() for _ in wl["algos"]]
+    del g0
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
+
+    def one_step(e2e):
+        space = cao.Space.from_space(sp).build()                          # S1
+        space.set_objective(obj_h.to(dev, non_blocking=True) if e2e else obj_d)
+        runs = []
+        for a, algo in enumerate(wl["algos"]):
+            r = cao.Runs(space, algo, n_runs=R, pop=P, budget=wl["budget"], max_gens=G, seed=wl["seed"],
+                         first_run=first_run)                             # S2
+            r.step(G)                                                     # S3-S7
+            b = r.best()
+            if e2e:
+                packed = torch.cat([b["best_f"].view(torch.int32), b["best_rank"], b["uniq"], b["gens_done"]])
+                host_out[a].copy_(packed, non_blocking=True)
+            runs.append(r)
+        return space, runs
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(K, e2e, profile):
+        evs = []
+        kept = None
+        if profile:
+            cao.profile_enable(True)
+        l0 = cao.launch_count()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(K):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            kept = one_step(e2e)
+            e1.record()
+            evs.append((e0, e1))
+            if e2e:
+                e1.synchronize()                                          # the user reads the result every step
+        barrier()
+        wall = time.perf_counter() - t0
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+        prof = cao.profile_read() if profile else None
+        if profile:
+            cao.profile_enable(False)
+        launches = cao.launch_count() - l0
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, wall, prof, launches, kept
+
+    for _ in range(args.warmup):
+        one_step(False)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local); sampler.start()
+    ms, wall, prof, launches, kept = timed(args.steps, False, True)
+    sampler.stop_flag = True; sampler.join(timeout=2)
+    space, runs = kept
+    counters = [r.counters() for r in runs]
+    cands_step = sum(c["n_evaluated"] for c in counters)
+    scanned_step = sum(c["n_scanned"] for c in counters)
+    repaired_step = sum(c["n_repaired"] for c in counters)
+    gens_done = [int(r.best()["gens_done"].sum().item()) for r in runs]
+    value = world * cands_step * args.steps / (ms / 1e3)
+
+    one_step(True); torch.cuda.synchronize()
+    ms_e, wall_e, _, _, _ = timed(args.steps, True, False)
+    value_e = world * cands_step * args.steps / (ms_e / 1e3)
+    h2d = obj.nbytes + sum(len(d) * 8 for d in sp.domains) + sum(len(p) * 4 for p in sp.rpn)
+    d2h = len(wl["algos"]) * 16 * R + 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (device time per kernel class, CUDA events inside the library on the
+    # launching stream, over the timed region)
+    clocks = sampler.summary()
+    kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps} for k, v in prof.items() if v[1]}
+    top = max(kern, key=lambda k: kern[k]["ms_per_step"])
+    top_ms, top_n = kern[top]["ms_per_step"], kern[top]["launches_per_step"]
+    dur_s = top_ms / 1e3 / top_n                                          # average launch duration
+    sm_max = clocks.get("sm_max_mhz") or pk["sm_max_mhz"]
+    alu_peak = N_SM * ISSUE_LANES_PER_SM_CLK * sm_max * 1e6 / 1e12        # T int-instr/s at the issue limit
+    if top == "k_scan":
+        ops = scanned_step * V * scan_ops_per_pair(n) / top_n             # per launch
+        roof = {"kernel": top, "bound": "alu", "achieved": ops / dur_s / 1e12, "peak": alu_peak, "unit": "Tiop/s",
+                "peak_source": f"148 SM x 128 lanes/clk x {sm_max:.0f} MHz (issue limit; DESIGN.md section 6)",
+                "traffic": None}
+    elif top == "k_enum_pass1":
+        by = N / 8
+        roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "peak_source": pk["source"], "traffic": None}
+    else:
+        # k_op / k_finish / k_init: sector-granular bytes per candidate: state + bitmap + dir + obj + dedup
+        per = {"k_op": 2 * rb + 8 + 32 + 32, "k_finish": 8 + 32 + 64 + rb + 24, "k_init": 32 + 64 + rb + 8}.get(top, 64)
+        by = per * cands_step / max(top_n, 1)
+        roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "peak_source": pk["source"], "traffic": None}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["avg_launch_us"] = dur_s * 1e6
+    roof["share_of_step"] = top_ms / (ms / args.steps)
+
+    # ---- S1 alone (BASELINE metric "enumeration Gcfg/s"): configs[3] (sparse, 5.7e8) and configs[2], resident buffers
+    enum = {}
+    for cfg in ([1, 2, 3] if not args.no_enum else []):
+        spx = W.WORKLOADS[cfg].space()
+        gx = cao.Space.from_space(spx)
+        gx.alloc_build(); gx.build_count(); gx.alloc_table(); gx.build_fill()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(7):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); gx.build_count(); gx.build_fill(); e1.record(); e1.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        Nx, Vx, nx, rbx = gx.sizes()
+        t = float(np.median(ts)) / 1e3
+        enum[f"cfg{cfg}"] = {"N": Nx, "V": Vx, "ms": t * 1e3, "gcfg_s": Nx / t / 1e9,
+                             "hbm_gbs": enum_bytes(Nx, Vx, rbx) / t / 1e9,
+                             "hbm_frac": enum_bytes(Nx, Vx, rbx) / t / 1e9 / pk["hbm_gbs"]}
+        del gx
+
+    # ---- CPU oracle on a bounded sample of the same workload (rank 0, N=1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        c, t = oracle_sample_step(wl, args.ref_runs)
+        cpu = {"value": c / t, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": oracle_sample_text(wl, args.ref_runs),
+               "seconds": t}
+
+    line = {
+        "metric": "candidates_repaired_evaluated_per_s", "value": value, "unit": "candidates/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u8/u64 integer + f32 (no FMA)", "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[{args.config}] ({sp.name}): N={N} V={V} n={n}; " +
+                               "+".join(wl["algos"]) + f", pop {P}, budget {wl['budget']} unique, cap {G} generations, "
+                               f"{R} runs per algorithm per GPU; step = S1 build + S2 init + S3-S7 to budget + read best",
+                   "runs_per_gpu": R, "pop": P, "l2": "flushed between steps (512 MiB write outside the per-step events)",
+                   "timing": "CUDA events per step on the launching stream, max over ranks"},
+        "clocks": clocks,
+        "e2e": {"value": value_e, "unit": "candidates/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "ms_per_step": ms_e / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "cpu_baseline": cpu,
+        "extra": {"candidates_per_step": int(cands_step), "invalid_post_snap_per_step": int(repaired_step),
+                  "scanned_per_step": int(scanned_step), "generations_done_sum": gens_done,
+                  "kernels": kern, "enumeration": enum, "wall_s_timed_region": wall, "peaks": pk},
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--runs", type=int, default=None, help="runs per algorithm per GPU (default: the config's)")
+    ap.add_argument("--ref-runs", type=int, default=1, help="runs per algorithm of the CPU-oracle sample")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-enum", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        reference_arm(args)
+    else:
+        gpu_arm(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -145,6 +145,14 @@ int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uin
 /* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
 uint64_t cao_launch_count(void);
 
+/* Optional device timing per kernel class (bench.py's roofline): while enabled, every launch is bracketed by
+ * CUDA events on its stream.  enable(1) clears the totals.  read() synchronises the recorded events and
+ * returns the summed milliseconds and the launch count of class `cls`: 0 k_build_table, 1 k_enum_pass1,
+ * 2 count scan, 3 k_fill, 4 k_init, 5 k_op, 6 k_scan, 7 k_finish, 8 queries; name() gives the kernel names. */
+int cao_profile_enable(int32_t on);
+int cao_profile_read(int32_t cls, double* h_ms_total, uint64_t* h_launches);
+const char* cao_profile_name(int32_t cls);
+
 /* Device self-tests for the parity of the arithmetic primitives (O3, O5-O7): out[i] from in[i]. */
 int cao_test_philox(const uint32_t* d_ctr_key /* count x 6 */, uint32_t* d_out /* count x 4 */,
                     uint64_t count, void* stream);

@@ -65,6 +65,9 @@ SIGNATURES = {
     "cao_runs_debug_state": (C.c_int, [vp, i32, pvp, pu64]),
     "cao_runs_counters": (C.c_int, [vp, vp, pu64, pu64, pu64]),
     "cao_launch_count": (u64, []),
+    "cao_profile_enable": (C.c_int, [i32]),
+    "cao_profile_read": (C.c_int, [i32, C.POINTER(C.c_double), pu64]),
+    "cao_profile_name": (C.c_char_p, [i32]),
     "cao_test_philox": (C.c_int, [vp, vp, u64, vp]),
     "cao_test_exp_neg": (C.c_int, [vp, vp, u64, vp]),
     "cao_last_error": (C.c_char_p, []),
@@ -106,6 +109,20 @@ def _dev_bytes(nbytes, device):
 
 def launch_count() -> int:
     return int(lib().cao_launch_count())
+
+
+def profile_enable(on=True):
+    _check(lib().cao_profile_enable(1 if on else 0))
+
+
+def profile_read():
+    """{kernel class name: (total ms, launches)} since profile_enable(True)."""
+    out = {}
+    for cls in range(9):
+        ms, n = C.c_double(), u64()
+        _check(lib().cao_profile_read(cls, C.byref(ms), C.byref(n)))
+        out[lib().cao_profile_name(cls).decode()] = (ms.value, n.value)
+    return out
 
 
 def _view(base: torch.Tensor, ptr: int, nbytes: int, dtype, shape):

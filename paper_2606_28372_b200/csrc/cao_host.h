@@ -15,6 +15,16 @@ int cao_cuda_check(cudaError_t e, const char* what);
 #define CAO_CUDA(x) do { int rc_ = cao_cuda_check((x), #x); if (rc_) return rc_; } while (0)
 #define CAO_LAUNCHED(what) do { ++g_cao_launches; int rc_ = cao_cuda_check(cudaGetLastError(), what); if (rc_) return rc_; } while (0)
 
+// Optional per-kernel-class device timing (cao_profile_*): CUDA events on the launching stream around each launch.
+enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_N };
+extern std::atomic<int> g_cao_prof_on;
+void cao_prof_mark(int cls, bool end, cudaStream_t st);
+struct ProfScope {
+    int cls; cudaStream_t st; bool on;
+    ProfScope(int c, cudaStream_t s) : cls(c), st(s), on(g_cao_prof_on.load(std::memory_order_relaxed) != 0) { if (on) cao_prof_mark(cls, false, st); }
+    ~ProfScope() { if (on) cao_prof_mark(cls, true, st); }
+};
+
 static inline uint64_t align256(uint64_t x) { return (x + 255) & ~255ull; }
 
 // One constraint in the enumeration plan.

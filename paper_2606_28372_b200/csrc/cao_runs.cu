@@ -25,6 +25,7 @@ static void launch_scan_wu(const SpaceMeta& sm, const uint8_t* cand, const uint3
 }
 static int launch_scan(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
                        unsigned long long* key, cudaStream_t st) {
+    ProfScope ps(PK_SCAN, st);
     switch ((sm.n + 3) / 4) {
         case 1: launch_scan_wu<1>(sm, cand, wl, wl_count, key, st); break;
         case 2: launch_scan_wu<2>(sm, cand, wl, wl_count, key, st); break;
@@ -192,7 +193,7 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
 #define CALL_INIT(A, W) \
         if (r->smem_op > 48 * 1024) cudaFuncSetAttribute(k_op<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
         k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
-        DISPATCH_ALGO_ROWW(algo, s->meta.rowB / 4, CALL_INIT);
+        { ProfScope ps(PK_INIT, st); DISPATCH_ALGO_ROWW(algo, s->meta.rowB / 4, CALL_INIT); }
         ++g_cao_launches;
         rc2 = cao_cuda_check(cudaGetLastError(), "k_init");
     } while (0);
@@ -211,12 +212,12 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
         if (r->gen >= r->rm.max_gens) break;                            // g <= max_gens (O10)
         const uint32_t g = r->gen + 1;
 #define CALL_OP(A, W) k_op<A, W><<<r->rm.R, r->block, r->smem_op, st>>>(r->sm, r->rm, g)
-        DISPATCH_ALGO_ROWW(algo, roww, CALL_OP);
+        { ProfScope ps(PK_OP, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_OP); }
         CAO_LAUNCHED("k_op");
         int rc = launch_scan(r->sm, r->rm.cand, r->rm.wl, r->rm.wl_count, r->rm.key, st);
         if (rc) return rc;
 #define CALL_FIN(A, W) k_finish<A, W><<<r->rm.R, r->block, r->smem_fin, st>>>(r->sm, r->rm, g)
-        DISPATCH_ALGO_ROWW(algo, roww, CALL_FIN);
+        { ProfScope ps(PK_FINISH, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_FIN); }
         CAO_LAUNCHED("k_finish");
         r->gen = g;
     }

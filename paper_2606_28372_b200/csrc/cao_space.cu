@@ -12,6 +12,47 @@ int cao_cuda_check(cudaError_t e, const char* what) {
     return cao_fail(CAO_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 
+// ---------------------------------------------------------------------------------------------
+// Profiling: event pairs per launch, summed per kernel class when read.
+#include <mutex>
+std::atomic<int> g_cao_prof_on{0};
+namespace {
+struct ProfRec { int cls; cudaEvent_t e0, e1; };
+std::mutex g_prof_mu;
+std::vector<ProfRec> g_prof_pending;
+std::vector<cudaEvent_t> g_prof_pool;
+double g_prof_ms[PK_N];
+uint64_t g_prof_n[PK_N];
+cudaEvent_t prof_event() {
+    if (!g_prof_pool.empty()) { cudaEvent_t e = g_prof_pool.back(); g_prof_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr; cudaEventCreate(&e); return e;
+}
+void prof_drain() {
+    for (auto& r : g_prof_pending) {
+        if (!r.e0 || !r.e1) continue;
+        float ms = 0.0f;
+        if (cudaEventSynchronize(r.e1) == cudaSuccess && cudaEventElapsedTime(&ms, r.e0, r.e1) == cudaSuccess) {
+            g_prof_ms[r.cls] += ms; g_prof_n[r.cls] += 1;
+        }
+        g_prof_pool.push_back(r.e0); g_prof_pool.push_back(r.e1);
+    }
+    g_prof_pending.clear();
+}
+}  // namespace
+void cao_prof_mark(int cls, bool end, cudaStream_t st) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    if (!end) {
+        ProfRec r{cls, prof_event(), nullptr};
+        if (r.e0) cudaEventRecord(r.e0, st);
+        g_prof_pending.push_back(r);
+    } else {
+        for (size_t k = g_prof_pending.size(); k-- > 0;) {
+            ProfRec& r = g_prof_pending[k];
+            if (r.cls == cls && !r.e1) { r.e1 = prof_event(); if (r.e1) cudaEventRecord(r.e1, st); break; }
+        }
+    }
+}
+
 static bool program_ok(const int32_t* w, int nw, int n_params) {
     int sp = 0;
     for (int pc = 0; pc < nw; ++pc) {
@@ -30,6 +71,26 @@ extern "C" {
 
 const char* cao_last_error(void) { return g_cao_err.c_str(); }
 uint64_t cao_launch_count(void) { return g_cao_launches.load(); }
+
+int cao_profile_enable(int32_t on) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    if (on) { prof_drain(); for (int c = 0; c < PK_N; ++c) { g_prof_ms[c] = 0.0; g_prof_n[c] = 0; } }
+    g_cao_prof_on.store(on ? 1 : 0);
+    return CAO_OK;
+}
+int cao_profile_read(int32_t cls, double* ms_total, uint64_t* launches) {
+    if (cls < 0 || cls >= PK_N) return cao_fail(CAO_E_INVALID_ARG, "cao_profile_read: unknown kernel class");
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    prof_drain();
+    if (ms_total) *ms_total = g_prof_ms[cls];
+    if (launches) *launches = g_prof_n[cls];
+    return CAO_OK;
+}
+const char* cao_profile_name(int32_t cls) {
+    static const char* names[PK_N] = {"k_build_table", "k_enum_pass1", "k_scan_reduce+partials+apply", "k_fill", "k_init",
+                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish"};
+    return cls >= 0 && cls < PK_N ? names[cls] : "";
+}
 
 int cao_space_create(cao_space** out) {
     if (!out) return cao_fail(CAO_E_INVALID_ARG, "cao_space_create: out is NULL");
@@ -184,7 +245,7 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
         a.n_outer = (int32_t)p.outer.size();
         for (size_t e = 0; e < p.outer.size(); ++e) { a.dig[e] = (uint8_t)p.outer[e]; a.cstride[e] = p.cstride[e]; }
         uint64_t threads = p.rows * s->Wb;
-        k_build_table<<<(unsigned)((threads + 127) / 128), 128, 0, st>>>(s->meta, a);
+        { ProfScope ps(PK_TABLE, st); k_build_table<<<(unsigned)((threads + 127) / 128), 128, 0, st>>>(s->meta, a); }
         CAO_LAUNCHED("k_build_table");
     }
     EnumArgs ea{};
@@ -195,17 +256,20 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
     size_t smem = (size_t)(s->nb + 1) * s->Wb * 8 + (size_t)CAO_MAX_DIMS * 256;
     if (smem > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_enum_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     uint64_t grid = (s->n_blocks + s->nb - 1) / s->nb;
-    k_enum_pass1<<<(unsigned)grid, 256, smem, st>>>(s->meta, ea);
+    { ProfScope ps(PK_ENUM, st); k_enum_pass1<<<(unsigned)grid, 256, smem, st>>>(s->meta, ea); }
     CAO_LAUNCHED("k_enum_pass1");
     uint32_t* d_cnt = (uint32_t*)(sc + s->off_cnt);
     uint32_t* d_part = (uint32_t*)(sc + s->off_part);
     uint64_t* d_V = (uint64_t*)(sc + s->off_V);
-    k_scan_reduce<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
-    CAO_LAUNCHED("k_scan_reduce");
-    k_scan_partials<<<1, 1024, 0, st>>>(d_part, s->n_part, d_V);
-    CAO_LAUNCHED("k_scan_partials");
-    k_scan_apply<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
-    CAO_LAUNCHED("k_scan_apply");
+    {
+        ProfScope ps(PK_CSCAN, st);
+        k_scan_reduce<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
+        CAO_LAUNCHED("k_scan_reduce");
+        k_scan_partials<<<1, 1024, 0, st>>>(d_part, s->n_part, d_V);
+        CAO_LAUNCHED("k_scan_partials");
+        k_scan_apply<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
+        CAO_LAUNCHED("k_scan_apply");
+    }
     uint64_t V = 0;
     CAO_CUDA(cudaMemcpyAsync(&V, d_V, 8, cudaMemcpyDeviceToHost, st));
     CAO_CUDA(cudaStreamSynchronize(st));
@@ -238,8 +302,11 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
     const uint32_t* cnt = (const uint32_t*)((uint8_t*)s->d_scratch + s->off_cnt);
     uint64_t threads = s->nd * 16;
     unsigned grid = (unsigned)((threads + 255) / 256);
-    if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
-    else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+    {
+        ProfScope ps(PK_FILL, st);
+        if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+        else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+    }
     CAO_LAUNCHED("k_fill");
     s->meta.rows = rows; s->meta.Ltab = Ltab; s->meta.dir = dir;
     s->filled = true;
