@@ -87,6 +87,11 @@ int cao_space_add_constraint(cao_space* s, const int32_t* h_rpn, int32_t n_words
  * give identical results.  Set before build_workspace_bytes. */
 int cao_space_set_build_mode(cao_space* s, int32_t mode);
 int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64_t* scratch_bytes);
+/* Highest Hamming level the generation step probes in the bitmap before it falls back to the table scan:
+ * -1 (default) = cost model (level h is probed while (number of rows at distance h) * 60 <= V * scan cost),
+ * 0..3 = fixed.  Call before build_count; probe_levels() reports the level in use after build_count. */
+int cao_space_set_probe_levels(cao_space* s, int32_t levels);
+int cao_space_probe_levels(const cao_space* s, int32_t* levels);
 /* Pass 1: validity bitmap + per-512-config counts, then the exclusive scan of the counts.
  * Synchronises `stream` once to return V in *h_V.  d_scratch may be released after build_fill. */
 int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V);
@@ -104,11 +109,14 @@ int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t c
                        void* stream);
 /* S5 standalone: d_rank_out[i] = rank of argmin (Hamming, sum |didx|, L) over the valid table; the
  * identity for valid rows (L143, L215, L270; O9).  d_key_out (optional, may be NULL) receives
- * ham << 45 | sad << 32 | rank.  use_probe: 1 = bitmap probes of the Hamming-1 neighbours first,
- * 0 = table scan only.  d_scratch: cao_space_repair_scratch_bytes(count) bytes. */
+ * ham << 45 | sad << 32 | rank.  probe_levels: 0 = table scan only; 1, 2, 3 = first test the neighbours
+ * at Hamming distance <= that level in the bitmap (exact: Hamming is the primary key); any other value
+ * (e.g. -1) = the level the library's cost model chose for this space.  All settings give identical
+ * results.  Rows with an index outside its domain are legal inputs (they are invalid and go to the scan).
+ * d_scratch: cao_space_repair_scratch_bytes(count) bytes. */
 int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
 int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
-                     uint64_t* d_key_out, int32_t use_probe, void* d_scratch, void* stream);
+                     uint64_t* d_key_out, int32_t probe_levels, void* d_scratch, void* stream);
 /* Objective table by rank: V floats, > 0 and finite (borrowed; L268: the evaluation is a lookup). */
 int cao_space_set_objective(cao_space* s, const float* d_obj);
 

@@ -46,6 +46,8 @@ SIGNATURES = {
     "cao_space_add_constraint": (C.c_int, [vp, pi32, i32]),
     "cao_space_set_build_mode": (C.c_int, [vp, i32]),
     "cao_space_build_workspace_bytes": (C.c_int, [vp, pu64, pu64]),
+    "cao_space_set_probe_levels": (C.c_int, [vp, i32]),
+    "cao_space_probe_levels": (C.c_int, [vp, pi32]),
     "cao_space_build_count": (C.c_int, [vp, vp, vp, vp, pu64]),
     "cao_space_table_bytes": (C.c_int, [vp, pu64]),
     "cao_space_build_fill": (C.c_int, [vp, vp, vp]),
@@ -134,7 +136,7 @@ def _view(base: torch.Tensor, ptr: int, nbytes: int, dtype, shape):
 class Space:
     """P = (X, D, C), resolved on the GPU before tuning (L137)."""
 
-    def __init__(self, domains, programs, names=None, build_mode=0, device="cuda"):
+    def __init__(self, domains, programs, names=None, build_mode=0, device="cuda", probe_levels=-1):
         L = lib()
         self.device = torch.device(device)
         h = C.c_void_p()
@@ -149,6 +151,7 @@ class Space:
             a = np.ascontiguousarray(prog, dtype=np.int32)
             _check(L.cao_space_add_constraint(h, a.ctypes.data_as(pi32), a.size))
         _check(L.cao_space_set_build_mode(h, build_mode))
+        _check(L.cao_space_set_probe_levels(h, probe_levels))
         self.built = False
         self._bitmap = self._scratch = self._table = self._obj = None
 
@@ -242,8 +245,16 @@ class Space:
         _check(lib().cao_space_is_valid(self._h, r.data_ptr(), r.shape[0], out.data_ptr(), _stream()))
         return out
 
+    @property
+    def probe_levels(self):
+        v = i32()
+        _check(lib().cao_space_probe_levels(self._h, C.byref(v)))
+        return v.value
+
     def repair(self, rows, use_probe=True):
-        """-> (rank int32-as-uint32 tensor, key int64 tensor: ham << 45 | sad << 32 | rank)."""
+        """-> (rank int32-as-uint32 tensor, key int64 tensor: ham << 45 | sad << 32 | rank).
+        use_probe: True = the library's probe level, False = scan only, or an explicit level 0..3."""
+        use_probe = -1 if use_probe is True else 0 if use_probe is False else int(use_probe)
         r = self.pack_rows(rows)
         c = r.shape[0]
         sb = u64()
@@ -251,7 +262,7 @@ class Space:
         scratch = _dev_bytes(sb.value, self.device)
         rank = torch.empty(c, dtype=torch.int32, device=self.device)
         key = torch.empty(c, dtype=torch.int64, device=self.device)
-        _check(lib().cao_space_repair(self._h, r.data_ptr(), c, rank.data_ptr(), key.data_ptr(), 1 if use_probe else 0,
+        _check(lib().cao_space_repair(self._h, r.data_ptr(), c, rank.data_ptr(), key.data_ptr(), use_probe,
                                       scratch.data_ptr(), _stream()))
         self._last_scratch = scratch
         return rank, key

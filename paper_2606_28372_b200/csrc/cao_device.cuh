@@ -26,6 +26,14 @@ struct SpaceMeta {
     uint16_t m[CAO_MAX_DIMS];
 };
 
+// Targets of the Hamming-2/3 probes: every (dimension, value index) pair, sorted by dimension then value.
+struct ProbeMeta {
+    const uint16_t* tgt;                // T entries: d << 8 | v
+    uint32_t T;
+    int32_t levels;                     // highest Hamming level probed in the bitmap before the table scan (1..3)
+    uint16_t dim_first[CAO_MAX_DIMS + 1];   // first target of dimension d; dim_first[n] = T
+};
+
 // ---------------------------------------------------------------------------------------------
 // O3: Philox4x32-10 (Salmon et al., SC'11).
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1) {

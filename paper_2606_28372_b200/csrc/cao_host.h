@@ -16,7 +16,7 @@ int cao_cuda_check(cudaError_t e, const char* what);
 #define CAO_LAUNCHED(what) do { ++g_cao_launches; int rc_ = cao_cuda_check(cudaGetLastError(), what); if (rc_) return rc_; } while (0)
 
 // Optional per-kernel-class device timing (cao_profile_*): CUDA events on the launching stream around each launch.
-enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_N };
+enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_N };
 extern std::atomic<int> g_cao_prof_on;
 void cao_prof_mark(int cls, bool end, cudaStream_t st);
 struct ProfScope {
@@ -56,7 +56,11 @@ struct cao_space {
     uint64_t bitmap_bytes = 0;
     void* d_scratch = nullptr;
     // table layout
-    uint64_t off_rows = 0, off_Ltab = 0, off_dir = 0, table_bytes = 0;
+    uint64_t off_rows = 0, off_Ltab = 0, off_dir = 0, off_tgt = 0, table_bytes = 0;
+    // Hamming-level probes (S5)
+    ProbeMeta probe{};
+    std::vector<uint16_t> h_tgt;
+    int probe_levels_req = -1;         // -1 = cost model
 };
 
 // Arguments of the pass-1 kernel, passed by value.

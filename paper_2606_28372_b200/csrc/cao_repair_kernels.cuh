@@ -50,6 +50,88 @@ __device__ __forceinline__ void worklist_push(uint32_t* wl, uint32_t* wl_count, 
     wl[pos] = slot;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Hamming-2 / Hamming-3 probe of the worklist: one warp per candidate.  All index rows at Hamming distance
+// exactly h are enumerated as h targets (dimension, value) of strictly increasing dimension; the outer
+// targets are walked by the whole warp, the innermost one is spread over the lanes.  Each probe is one bit
+// test at L + sum (v - c) * stride; the level minimum of (sum |v - c|, L') is exact because Hamming is the
+// primary key.  Candidates without a valid neighbour up to `levels` go on to the table scan (wl_out).
+__device__ __forceinline__ uint64_t warp_min_u64(uint64_t v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) { uint64_t t = __shfl_xor_sync(0xFFFFFFFFu, v, o); v = t < v ? t : v; }
+    return v;
+}
+
+template <int ROWW>
+__global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
+                                                 const uint8_t* __restrict__ cand_rows, const uint32_t* __restrict__ wl,
+                                                 const uint32_t* __restrict__ wl_count, unsigned long long* key,
+                                                 uint32_t* wl_out, uint32_t* wl_out_count, unsigned long long* n_scanned) {
+    __shared__ uint8_t s_c[8][ROWW * 4];
+    const uint32_t count = *wl_count;
+    const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
+    const uint32_t T = pm.T;
+    for (uint32_t ci = blockIdx.x * (blockDim.x >> 5) + wib; ci < count; ci += nwarps) {
+        const uint32_t slot = wl[ci];
+        __syncwarp();
+        if (lane < ROWW) ((uint32_t*)s_c[wib])[lane] = ((const uint32_t*)(cand_rows + (uint64_t)slot * (ROWW * 4)))[lane];
+        __syncwarp();
+        const uint8_t* c = s_c[wib];
+        uint64_t L = 0;
+        for (int d = 0; d < sm.n; ++d) L += (uint64_t)c[d] * sm.stride[d];
+        uint64_t best = ~0ull;
+        int found = 0;
+        if (pm.levels >= 2) {
+            for (uint32_t t1 = 0; t1 < T; ++t1) {
+                const uint32_t e1 = __ldg(&pm.tgt[t1]), d1 = e1 >> 8;
+                const int dv1 = (int)(e1 & 255) - (int)c[d1];
+                if (dv1 == 0) continue;
+                const uint64_t L1 = L + (int64_t)dv1 * (int64_t)sm.stride[d1];
+                const uint32_t s1 = (uint32_t)abs(dv1);
+                for (uint32_t t2 = pm.dim_first[d1 + 1] + lane; t2 < T; t2 += 32) {
+                    const uint32_t e2 = __ldg(&pm.tgt[t2]), d2 = e2 >> 8;
+                    const int dv2 = (int)(e2 & 255) - (int)c[d2];
+                    if (dv2 == 0) continue;
+                    const uint64_t L2 = L1 + (int64_t)dv2 * (int64_t)sm.stride[d2];
+                    if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)(s1 + (uint32_t)abs(dv2)) << 40) | L2; best = k < best ? k : best; }
+                }
+            }
+            best = warp_min_u64(best);
+            if (best != ~0ull) found = 2;
+        }
+        if (!found && pm.levels >= 3) {
+            for (uint32_t t1 = 0; t1 < T; ++t1) {
+                const uint32_t e1 = __ldg(&pm.tgt[t1]), d1 = e1 >> 8;
+                const int dv1 = (int)(e1 & 255) - (int)c[d1];
+                if (dv1 == 0) continue;
+                const uint64_t L1 = L + (int64_t)dv1 * (int64_t)sm.stride[d1];
+                const uint32_t s1 = (uint32_t)abs(dv1);
+                for (uint32_t t2 = pm.dim_first[d1 + 1]; t2 < T; ++t2) {
+                    const uint32_t e2 = __ldg(&pm.tgt[t2]), d2 = e2 >> 8;
+                    const int dv2 = (int)(e2 & 255) - (int)c[d2];
+                    if (dv2 == 0) continue;
+                    const uint64_t L2 = L1 + (int64_t)dv2 * (int64_t)sm.stride[d2];
+                    const uint32_t s2 = s1 + (uint32_t)abs(dv2);
+                    for (uint32_t t3 = pm.dim_first[d2 + 1] + lane; t3 < T; t3 += 32) {
+                        const uint32_t e3 = __ldg(&pm.tgt[t3]), d3 = e3 >> 8;
+                        const int dv3 = (int)(e3 & 255) - (int)c[d3];
+                        if (dv3 == 0) continue;
+                        const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
+                        if (bit_test(sm.bitmap, L3)) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
+                    }
+                }
+            }
+            best = warp_min_u64(best);
+            if (best != ~0ull) found = 3;
+        }
+        if (lane == 0) {
+            if (found) key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
+            else { wl_out[atomicAdd(wl_out_count, 1u)] = slot; if (n_scanned) atomicAdd(n_scanned, 1ull); }
+        }
+    }
+}
+
 #define SCAN_TC 128          // candidates per tile = threads per CTA
 #define SCAN_TR 512          // valid rows per shared-memory tile
 
@@ -115,15 +197,20 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
 template <int ROWW>
 __global__ void __launch_bounds__(256) k_repair_probe(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ rows_in,
                                                       uint64_t count, int use_probe, unsigned long long* key,
-                                                      uint32_t* wl, uint32_t* wl_count) {
+                                                      uint32_t* wl, uint32_t* wl_count, uint32_t* wl2, uint32_t* wl2_count) {
     uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
     uint32_t w[ROWW];
     load_row<ROWW>(rows_in + i * (ROWW * 4), w);
     bool valid;
+    bool in_dom = true;
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d)
+        if (d < sm.n && ((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) >= sm.m[d]) in_dom = false;
     uint64_t k = validate_probe<ROWW>(sm, w, use_probe != 0, valid);
     key[i] = k;
-    if (k == CAO_KEY_NONE) worklist_push(wl, wl_count, (uint32_t)i);
+    // rows with an index outside its domain skip the neighbour probes and go straight to the scan (wl2)
+    if (k == CAO_KEY_NONE) { if (in_dom && wl2 != wl) worklist_push(wl, wl_count, (uint32_t)i); else worklist_push(wl2, wl2_count, (uint32_t)i); }
 }
 
 __global__ void __launch_bounds__(256) k_repair_finish(const unsigned long long* __restrict__ key, uint64_t count,

@@ -40,6 +40,19 @@ static int launch_scan(const SpaceMeta& sm, const uint8_t* cand, const uint32_t*
     return CAO_OK;
 }
 
+// Hamming-2/3 probe of worklist wl; survivors go to wl2 (the scan's input).
+static int launch_probe23(const cao_space* s, const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
+                          unsigned long long* key, uint32_t* wl2, uint32_t* wl2_count, unsigned long long* n_scanned,
+                          int levels, cudaStream_t st) {
+    ProbeMeta pm = s->probe;
+    pm.levels = levels;
+    ProfScope ps(PK_PROBE, st);
+    if (sm.rowB == 16) k_probe23<4><<<148 * 4, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
+    else k_probe23<8><<<148 * 4, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
+    CAO_LAUNCHED("k_probe23");
+    return CAO_OK;
+}
+
 // Dispatch over (algorithm, row words).
 #define DISPATCH_ALGO_ROWW(algo, roww, CALL)                                         \
     do {                                                                             \
@@ -65,7 +78,7 @@ extern "C" {
 // ---------------------------------------------------------------------------------------------
 int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes) {
     if (!s || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_scratch_bytes: NULL argument");
-    *bytes = align256(std::max<uint64_t>(1, count) * 8) + align256(std::max<uint64_t>(1, count) * 4) + 256;
+    *bytes = align256(std::max<uint64_t>(1, count) * 8) + 2 * align256(std::max<uint64_t>(1, count) * 4) + 256;
     return CAO_OK;
 }
 
@@ -83,13 +96,23 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
     uint8_t* sc = (uint8_t*)d_scratch;
     unsigned long long* key = (unsigned long long*)sc;
     uint32_t* wl = (uint32_t*)(sc + align256(count * 8));
-    uint32_t* wl_count = (uint32_t*)(sc + align256(count * 8) + align256(count * 4));
-    CAO_CUDA(cudaMemsetAsync(wl_count, 0, 4, st));
+    uint32_t* wl2 = (uint32_t*)(sc + align256(count * 8) + align256(count * 4));
+    uint32_t* wl_count = (uint32_t*)(sc + align256(count * 8) + 2 * align256(count * 4));
+    uint32_t* wl2_count = wl_count + 1;
+    CAO_CUDA(cudaMemsetAsync(wl_count, 0, 8, st));
+    const int levels = use_probe < 0 || use_probe > 3 ? s->probe.levels : use_probe;
+    const bool two = levels >= 2;
     unsigned grid = (unsigned)((count + 255) / 256);
-    if (s->meta.rowB == 16) k_repair_probe<4><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, use_probe, key, wl, wl_count);
-    else k_repair_probe<8><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, use_probe, key, wl, wl_count);
+    {   // without Hamming-2/3 probes everything unresolved goes to the scan list directly
+        ProfScope ps(PK_QUERY, st);
+        uint32_t* a = two ? wl : wl2; uint32_t* ac = two ? wl_count : wl2_count;
+        if (s->meta.rowB == 16) k_repair_probe<4><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, levels >= 1, key, a, ac, wl2, wl2_count);
+        else k_repair_probe<8><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, levels >= 1, key, a, ac, wl2, wl2_count);
+    }
     CAO_LAUNCHED("k_repair_probe");
-    int rc = launch_scan(s->meta, d_idx_rows, wl, wl_count, key, st);
+    int rc = CAO_OK;
+    if (two) { rc = launch_probe23(s, s->meta, d_idx_rows, wl, wl_count, key, wl2, wl2_count, nullptr, levels, st); if (rc) return rc; }
+    rc = launch_scan(s->meta, d_idx_rows, wl2, wl2_count, key, st);
     if (rc) return rc;
     k_repair_finish<<<grid, 256, 0, st>>>(key, count, d_rank_out, d_key_out);
     CAO_LAUNCHED("k_repair_finish");
@@ -99,7 +122,7 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
 // ---------------------------------------------------------------------------------------------
 struct RunsLayout {
     uint64_t cand, key, valid, rep_rank, eval_rank, tap_f, accept, active, idx, rank, f, x, v, pb, pbf, dedup,
-        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl_count, counters, total;
+        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl2, wl_count, counters, total;
     uint64_t zero_from, zero_bytes;       // region that must start as zero: dedup .. stagn
     uint32_t dedup_words;
 };
@@ -120,11 +143,12 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
     L.zero_from = off;
     L.dedup = take(R * L.dedup_words * 4);
     L.uniq = take(R * 4); L.gens_done = take(R * 4); L.stagn = take(R * 4);
-    L.wl_count = take(4); L.counters = take(3 * 8);
+    L.wl_count = take(8); L.counters = take(4 * 8);
     L.zero_bytes = off - L.zero_from;
     L.best_rank = take(R * 4); L.best_f = take(R * 4);
     L.traj = take((max_gens + 1) * R * 12);
     L.wl = take(RP * 4);
+    L.wl2 = take(RP * 4);
     L.total = off;
     return L;
 }
@@ -168,7 +192,7 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     r->s = s; r->sm = s->meta;
     RunsMeta& m = r->rm;
     m.R = n_runs; m.first_run = first_run; m.P = (uint32_t)pop; m.budget = budget_unique; m.max_gens = max_gens;
-    m.dedup_words = L.dedup_words; m.algo = algo; m.seed = seed; m.hp = *hp;
+    m.dedup_words = L.dedup_words; m.algo = algo; m.probe_levels = s->probe.levels; m.seed = seed; m.hp = *hp;
     m.cand = w + L.cand; m.key = (unsigned long long*)(w + L.key); m.valid = w + L.valid;
     m.rep_rank = (uint32_t*)(w + L.rep_rank); m.eval_rank = (uint32_t*)(w + L.eval_rank); m.tap_f = (float*)(w + L.tap_f);
     m.accept = w + L.accept; m.active = w + L.active;
@@ -177,6 +201,7 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     m.dedup = (uint32_t*)(w + L.dedup); m.uniq = (uint32_t*)(w + L.uniq); m.gens_done = (uint32_t*)(w + L.gens_done);
     m.stagn = (uint32_t*)(w + L.stagn); m.best_rank = (uint32_t*)(w + L.best_rank); m.best_f = (float*)(w + L.best_f);
     m.traj = (uint32_t*)(w + L.traj); m.wl = (uint32_t*)(w + L.wl); m.wl_count = (uint32_t*)(w + L.wl_count);
+    m.wl2 = (uint32_t*)(w + L.wl2); m.wl2_count = m.wl_count + 1;
     m.counters = (unsigned long long*)(w + L.counters);
     const uint64_t RP = (uint64_t)n_runs * pop;
     r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
@@ -214,7 +239,14 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
 #define CALL_OP(A, W) k_op<A, W><<<r->rm.R, r->block, r->smem_op, st>>>(r->sm, r->rm, g)
         { ProfScope ps(PK_OP, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_OP); }
         CAO_LAUNCHED("k_op");
-        int rc = launch_scan(r->sm, r->rm.cand, r->rm.wl, r->rm.wl_count, r->rm.key, st);
+        int rc = CAO_OK;
+        const int levels = r->s->probe.levels;
+        if (levels >= 2) {
+            rc = launch_probe23(r->s, r->sm, r->rm.cand, r->rm.wl, r->rm.wl_count, r->rm.key, r->rm.wl2, r->rm.wl2_count,
+                                &r->rm.counters[1], levels, st);
+            if (rc) return rc;
+        }
+        rc = launch_scan(r->sm, r->rm.cand, levels >= 2 ? r->rm.wl2 : r->rm.wl, levels >= 2 ? r->rm.wl2_count : r->rm.wl_count, r->rm.key, st);
         if (rc) return rc;
 #define CALL_FIN(A, W) k_finish<A, W><<<r->rm.R, r->block, r->smem_fin, st>>>(r->sm, r->rm, g)
         { ProfScope ps(PK_FINISH, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_FIN); }

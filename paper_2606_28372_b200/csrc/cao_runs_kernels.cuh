@@ -13,7 +13,7 @@
 
 struct RunsMeta {
     uint32_t R, first_run, P, budget, max_gens, dedup_words;
-    int32_t algo;
+    int32_t algo, probe_levels;
     uint64_t seed;
     cao_hparams hp;
     // taps of the last generation, [run][ind]
@@ -24,7 +24,8 @@ struct RunsMeta {
     uint32_t* dedup;                                   // [run][dedup_words]
     uint32_t* uniq; uint32_t* gens_done; uint32_t* stagn; uint32_t* best_rank; float* best_f;
     uint32_t* traj;                                    // [gen][run]{f32 bits, rank, uniq}
-    uint32_t* wl; uint32_t* wl_count;
+    uint32_t* wl; uint32_t* wl_count;                  // candidates without a valid Hamming-1 neighbour
+    uint32_t* wl2; uint32_t* wl2_count;                // ... and none up to the probed level: table scan
     unsigned long long* counters;                      // n_repaired, n_scanned, n_evaluated
 };
 
@@ -136,11 +137,14 @@ template <int ROWW>
 __device__ __forceinline__ void candidate_tail(const SpaceMeta& sm, const RunsMeta& rm, uint64_t slot, const uint32_t (&w)[ROWW]) {
     store_row<ROWW>(rm.cand + slot * (ROWW * 4), w);
     bool valid;
-    uint64_t key = validate_probe<ROWW>(sm, w, true, valid);
+    uint64_t key = validate_probe<ROWW>(sm, w, rm.probe_levels >= 1, valid);
     rm.valid[slot] = valid ? 1 : 0;
     rm.key[slot] = key;
     if (!valid) atomicAdd(&rm.counters[0], 1ull);
-    if (key == CAO_KEY_NONE) { atomicAdd(&rm.counters[1], 1ull); worklist_push(rm.wl, rm.wl_count, (uint32_t)slot); }
+    if (key == CAO_KEY_NONE) {
+        worklist_push(rm.wl, rm.wl_count, (uint32_t)slot);
+        if (rm.probe_levels < 2) atomicAdd(&rm.counters[1], 1ull);       // straight to the scan
+    }
 }
 
 #define ROW_BYTE(w, d) (((w)[(d) >> 2] >> (((d) & 3) * 8)) & 0xFFu)
@@ -293,7 +297,7 @@ __global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMe
     __shared__ RunShared sh;
     const uint32_t k = blockIdx.x, i = threadIdx.x, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
-    if (k == 0 && i == 0) *rm.wl_count = 0;                             // the scan of this generation is done
+    if (k == 0 && i == 0) { *rm.wl_count = 0; *rm.wl2_count = 0; }                             // the scan of this generation is done
     if (!rm.active[k]) {                                                // frozen run: its trajectory row repeats (O10)
         if (i == 0) {
             uint32_t* t = rm.traj + ((uint64_t)g * rm.R + k) * 3;

@@ -88,7 +88,7 @@ int cao_profile_read(int32_t cls, double* ms_total, uint64_t* launches) {
 }
 const char* cao_profile_name(int32_t cls) {
     static const char* names[PK_N] = {"k_build_table", "k_enum_pass1", "k_scan_reduce+partials+apply", "k_fill", "k_init",
-                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish"};
+                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish", "k_probe23"};
     return cls >= 0 && cls < PK_N ? names[cls] : "";
 }
 
@@ -120,6 +120,19 @@ int cao_space_set_build_mode(cao_space* s, int32_t mode) {
     if (!s || (mode != 0 && mode != 1)) return cao_fail(CAO_E_INVALID_ARG, "cao_space_set_build_mode: mode must be 0 or 1");
     if (s->planned) return cao_fail(CAO_E_STATE, "cao_space_set_build_mode: after build_workspace_bytes");
     s->mode = mode;
+    return CAO_OK;
+}
+
+int cao_space_set_probe_levels(cao_space* s, int32_t levels) {
+    if (!s || levels < -1 || levels > 3) return cao_fail(CAO_E_INVALID_ARG, "cao_space_set_probe_levels: levels must be -1 (auto) or 0..3");
+    if (s->counted) return cao_fail(CAO_E_STATE, "cao_space_set_probe_levels: call before cao_space_build_count");
+    s->probe_levels_req = levels;
+    return CAO_OK;
+}
+int cao_space_probe_levels(const cao_space* s, int32_t* levels) {
+    if (!s || !levels) return cao_fail(CAO_E_INVALID_ARG, "cao_space_probe_levels: NULL argument");
+    if (!s->counted) return cao_fail(CAO_E_STATE, "cao_space_probe_levels: space not built");
+    *levels = s->probe.levels;
     return CAO_OK;
 }
 
@@ -281,6 +294,26 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
     s->off_rows = off; off = align256(off + std::max<uint64_t>(1, V) * rowB);
     s->off_Ltab = off; off = align256(off + std::max<uint64_t>(1, V) * 8);
     s->off_dir = off; off = align256(off + (s->nd + 1) * 4);
+    // probe targets and the cost model that decides how many Hamming levels are probed before the scan:
+    // C_h = number of index rows at Hamming distance exactly h from a point (upper bound, e_h of the m_d)
+    {
+        const int n = s->meta.n;
+        s->h_tgt.clear();
+        for (int d = 0; d < n; ++d) {
+            s->probe.dim_first[d] = (uint16_t)s->h_tgt.size();
+            for (int v = 0; v < (int)s->meta.m[d]; ++v) s->h_tgt.push_back((uint16_t)(d << 8 | v));
+        }
+        for (int d = n; d <= CAO_MAX_DIMS; ++d) s->probe.dim_first[d] = (uint16_t)s->h_tgt.size();
+        s->probe.T = (uint32_t)s->h_tgt.size();
+        double e[4] = {1, 0, 0, 0};
+        for (int d = 0; d < n; ++d) for (int h = 3; h >= 1; --h) e[h] += e[h - 1] * (double)s->meta.m[d];
+        const double scan_cost = (double)V * (5.0 * ((n + 3) / 4) + 6.0);
+        int lv = 1;
+        if (e[2] * 60.0 <= scan_cost) { lv = 2; if (e[3] * 60.0 <= scan_cost) lv = 3; }
+        if (s->probe_levels_req >= 0) lv = std::min(3, std::max(0, s->probe_levels_req));
+        s->probe.levels = lv;
+    }
+    s->off_tgt = off; off = align256(off + std::max<uint64_t>(1, s->h_tgt.size()) * 2);
     s->table_bytes = off;
     return CAO_OK;
 }
@@ -308,6 +341,8 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
         else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
     }
     CAO_LAUNCHED("k_fill");
+    CAO_CUDA(cudaMemcpyAsync(tb + s->off_tgt, s->h_tgt.data(), s->h_tgt.size() * 2, cudaMemcpyHostToDevice, st));
+    s->probe.tgt = (const uint16_t*)(tb + s->off_tgt);
     s->meta.rows = rows; s->meta.Ltab = Ltab; s->meta.dir = dir;
     s->filled = true;
     return CAO_OK;

@@ -161,3 +161,27 @@ def test_small_populations_and_tiny_spaces():
             for _ in range(8):
                 gr.step(1); orr.step(1)
                 compare(gr, orr, sp.n)
+
+
+@pytest.mark.parametrize("levels", [0, 1, 2, 3])
+def test_forced_probe_levels_give_identical_runs(levels):
+    """The Hamming-level probes are an exact shortcut of the scan: every setting reproduces the oracle."""
+    import paper_2606_28372_b200 as cao
+    sp, os_ = oracle_space(0)
+    g = cao.Space.from_space(sp, probe_levels=levels).build()
+    assert g.probe_levels == levels
+    g.set_objective(os_._obj)
+    for algo in ["de", "pso", "firefly", "ga"]:
+        kw = dict(n_runs=30, pop=20, budget=0, max_gens=12, seed=3)
+        orr = O.OracleRuns(os_, algo, **kw); gr = cao.Runs(g, algo, **kw)
+        for _ in range(4):
+            gr.step(3); orr.step(3)
+            compare(gr, orr, sp.n)
+
+
+def test_auto_probe_levels():
+    import paper_2606_28372_b200 as cao
+    sp, os_ = oracle_space(1)
+    assert gpu_space(1, os_, sp).probe_levels == 3
+    sp0, os0 = oracle_space(0)
+    assert gpu_space(0, os0, sp0).probe_levels == 1

@@ -94,7 +94,7 @@ def test_is_valid_and_repair_cfg0_all_configs():
     assert np.array_equal(gs.is_valid(rows).cpu().numpy(), want_valid)
     want = os_.repair(rows)
     wkey = (want["ham"].astype(np.uint64) << np.uint64(45)) | (want["sad"].astype(np.uint64) << np.uint64(32)) | want["rank"].astype(np.uint64)
-    for probe in (True, False):
+    for probe in (True, False, 1, 2, 3):
         rank, key = gs.repair(rows, use_probe=probe)
         assert np.array_equal(rank.cpu().numpy().view(np.uint32), want["rank"])
         assert np.array_equal(_u64(key), wkey)
@@ -110,7 +110,7 @@ def test_repair_random_rows(cfg, count):
     want = os_.repair(rows)
     wkey = (want["ham"].astype(np.uint64) << np.uint64(45)) | (want["sad"].astype(np.uint64) << np.uint64(32)) | want["rank"].astype(np.uint64)
     assert (want["ham"][:5] == 0).all()
-    for probe in (True, False):
+    for probe in (True, False, 1, 2, 3):
         rank, key = gs.repair(rows, use_probe=probe)
         assert np.array_equal(_u64(key), wkey)
         assert np.array_equal(rank.cpu().numpy().view(np.uint32), want["rank"])
@@ -129,7 +129,7 @@ def test_repair_tiny_spaces_and_ragged_counts():
         count = int(rng.integers(1, 700))
         rows = np.stack([rng.integers(0, m, size=count) for m in sp.m], axis=1).astype(np.uint8)
         want = os_.repair(rows)
-        for probe in (True, False):
+        for probe in (True, False, 1, 2, 3):
             rank, key = g.repair(rows, use_probe=probe)
             assert np.array_equal(rank.cpu().numpy().view(np.uint32), want["rank"]), seed
             k = _u64(key)
