@@ -120,7 +120,7 @@ def profile_enable(on=True):
 def profile_read():
     """{kernel class name: (total ms, launches)} since profile_enable(True)."""
     out = {}
-    for cls in range(9):
+    for cls in range(10):
         ms, n = C.c_double(), u64()
         _check(lib().cao_profile_read(cls, C.byref(ms), C.byref(n)))
         out[lib().cao_profile_name(cls).decode()] = (ms.value, n.value)

@@ -29,7 +29,8 @@ struct SpaceMeta {
 // Targets of the Hamming-2/3 probes: every (dimension, value index) pair, sorted by dimension then value.
 struct ProbeMeta {
     const uint16_t* tgt;                // T entries: d << 8 | v
-    uint32_t T;
+    const uint32_t* pairs;              // C2 entries: t1 | t2 << 16, dimension(t1) < dimension(t2)
+    uint32_t T, C2;
     int32_t levels;                     // highest Hamming level probed in the bitmap before the table scan (1..3)
     uint16_t dim_first[CAO_MAX_DIMS + 1];   // first target of dimension d; dim_first[n] = T
 };

@@ -8,39 +8,37 @@
 #pragma once
 #include "cao_host.h"
 
-struct TableBuildArgs {
-    const int64_t* dom; const int32_t* prog; uint64_t* out;
-    uint64_t rows, B;
-    uint32_t Wb; int32_t nw, t, n_outer;
-    uint8_t dig[CAO_MAX_DIMS]; uint32_t cstride[CAO_MAX_DIMS];
-};
-
-// One thread per (row, 64-bit word of the row): evaluates the program for up to 64 inner patterns.
-__global__ void __launch_bounds__(128) k_build_table(const __grid_constant__ SpaceMeta sm,
-                                                     const __grid_constant__ TableBuildArgs a) {
-    uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= a.rows * a.Wb) return;
-    uint64_t row = gid / a.Wb; uint32_t j = (uint32_t)(gid - row * a.Wb);
-    int64_t x[CAO_MAX_DIMS];
-    for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
-    for (int k = 0; k < a.n_outer; ++k) {
-        int d = a.dig[k];
-        uint32_t idx = (uint32_t)((row / a.cstride[k]) % sm.m[d]);
-        x[d] = a.dom[d * 256 + idx];
-    }
-    uint64_t word = 0;
-    for (int b = 0; b < 64; ++b) {
-        uint64_t p = (uint64_t)j * 64 + b;
-        if (p >= a.B) break;
-        uint64_t q = p;
-        for (int d = sm.n - 1; d >= a.t; --d) {
-            uint32_t m = sm.m[d];
-            uint32_t idx = (uint32_t)(q % m); q /= m;
-            x[d] = a.dom[d * 256 + idx];
+// All constraint tables in one launch: blockIdx.y = tabled constraint, one thread per (row, inner pattern);
+// a warp ballot assembles 32 patterns into one half word of the row.
+// Tabled descriptor: {toff_lo, toff_hi, n_outer, (digit, cstride) x n_outer, prog_off, prog_len, rows}.
+__global__ void __launch_bounds__(256) k_build_tables(const __grid_constant__ SpaceMeta sm, const int64_t* __restrict__ dom,
+                                                      const int32_t* __restrict__ desc, uint64_t* tables, uint64_t B,
+                                                      uint32_t Wb, int32_t t) {
+    const int32_t* ds = desc + desc[blockIdx.y];
+    const uint64_t toff = (uint32_t)ds[0] | ((uint64_t)(uint32_t)ds[1] << 32);
+    const int no = ds[2];
+    const int32_t* prog = desc + ds[3 + 2 * no];
+    const int nw = ds[4 + 2 * no];
+    const uint64_t rows = (uint32_t)ds[5 + 2 * no];
+    const uint64_t per_row = (uint64_t)Wb * 64, total = rows * per_row;
+    uint32_t* out32 = (uint32_t*)(tables + toff);
+    for (uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; gid < total; gid += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t row = gid / per_row, p = gid - row * per_row;          // per_row is a multiple of 64: a warp stays in one row
+        int ok = 0;
+        if (p < B) {
+            int64_t x[CAO_MAX_DIMS];
+            for (int d = 0; d < sm.n; ++d) x[d] = dom[d * 256];
+            for (int k = 0; k < no; ++k) {
+                const int d = ds[3 + 2 * k];
+                x[d] = dom[d * 256 + (uint32_t)((row / (uint32_t)ds[4 + 2 * k]) % sm.m[d])];
+            }
+            uint64_t q = p;
+            for (int d = sm.n - 1; d >= t; --d) { const uint32_t m = sm.m[d]; x[d] = dom[d * 256 + (uint32_t)(q % m)]; q /= m; }
+            ok = eval_program(prog, nw, x);
         }
-        if (eval_program(a.prog, a.nw, x)) word |= 1ull << b;
+        const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
+        if ((threadIdx.x & 31) == 0) out32[gid >> 5] = word;
     }
-    a.out[gid] = word;
 }
 
 __device__ __forceinline__ uint64_t get64(const uint64_t* mk, uint32_t r, uint32_t Wb) {

@@ -52,7 +52,7 @@ struct cao_space {
     int n_tab = 0, n_res = 0;
     // scratch layout (byte offsets)
     uint64_t off_dom = 0, off_desc = 0, off_tables = 0, off_cnt = 0, off_part = 0, off_V = 0, scratch_bytes = 0;
-    uint64_t tables_words = 0, n_part = 0;
+    uint64_t tables_words = 0, n_part = 0, max_table_threads = 0;
     uint64_t bitmap_bytes = 0;
     void* d_scratch = nullptr;
     // table layout
@@ -60,6 +60,8 @@ struct cao_space {
     // Hamming-level probes (S5)
     ProbeMeta probe{};
     std::vector<uint16_t> h_tgt;
+    std::vector<uint32_t> h_pairs;
+    uint64_t off_pairs = 0;
     int probe_levels_req = -1;         // -1 = cost model
 };
 

@@ -51,7 +51,7 @@ __device__ __forceinline__ void worklist_push(uint32_t* wl, uint32_t* wl_count, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Hamming-2 / Hamming-3 probe of the worklist: one warp per candidate.  All index rows at Hamming distance
+// Hamming-2 / Hamming-3 probe of the worklist: one CTA per candidate.  All index rows at Hamming distance
 // exactly h are enumerated as h targets (dimension, value) of strictly increasing dimension; the outer
 // targets are walked by the whole warp, the innermost one is spread over the lanes.  Each probe is one bit
 // test at L + sum (v - c) * stride; the level minimum of (sum |v - c|, L') is exact because Hamming is the
@@ -67,65 +67,50 @@ __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMe
                                                  const uint8_t* __restrict__ cand_rows, const uint32_t* __restrict__ wl,
                                                  const uint32_t* __restrict__ wl_count, unsigned long long* key,
                                                  uint32_t* wl_out, uint32_t* wl_out_count, unsigned long long* n_scanned) {
-    __shared__ uint8_t s_c[8][ROWW * 4];
-    const uint32_t count = *wl_count;
-    const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
-    const uint32_t T = pm.T;
-    for (uint32_t ci = blockIdx.x * (blockDim.x >> 5) + wib; ci < count; ci += nwarps) {
+    // One CTA per worklist candidate.  Threads walk the flattened list of target pairs (t1 < t2, different
+    // dimensions); level 3 adds a serial walk over the targets of the dimensions after t2's.
+    __shared__ uint32_t s_cw[ROWW];
+    __shared__ unsigned long long s_best;
+    const uint8_t* c = (const uint8_t*)s_cw;
+    const uint32_t count = *wl_count, tid = threadIdx.x, T = pm.T, C2 = pm.C2;
+    for (uint32_t ci = blockIdx.x; ci < count; ci += gridDim.x) {
         const uint32_t slot = wl[ci];
-        __syncwarp();
-        if (lane < ROWW) ((uint32_t*)s_c[wib])[lane] = ((const uint32_t*)(cand_rows + (uint64_t)slot * (ROWW * 4)))[lane];
-        __syncwarp();
-        const uint8_t* c = s_c[wib];
+        __syncthreads();
+        if (tid < ROWW) s_cw[tid] = ((const uint32_t*)(cand_rows + (uint64_t)slot * (ROWW * 4)))[tid];
+        if (tid == 0) s_best = ~0ull;
+        __syncthreads();
         uint64_t L = 0;
         for (int d = 0; d < sm.n; ++d) L += (uint64_t)c[d] * sm.stride[d];
-        uint64_t best = ~0ull;
         int found = 0;
-        if (pm.levels >= 2) {
-            for (uint32_t t1 = 0; t1 < T; ++t1) {
-                const uint32_t e1 = __ldg(&pm.tgt[t1]), d1 = e1 >> 8;
-                const int dv1 = (int)(e1 & 255) - (int)c[d1];
-                if (dv1 == 0) continue;
-                const uint64_t L1 = L + (int64_t)dv1 * (int64_t)sm.stride[d1];
-                const uint32_t s1 = (uint32_t)abs(dv1);
-                for (uint32_t t2 = pm.dim_first[d1 + 1] + lane; t2 < T; t2 += 32) {
-                    const uint32_t e2 = __ldg(&pm.tgt[t2]), d2 = e2 >> 8;
-                    const int dv2 = (int)(e2 & 255) - (int)c[d2];
-                    if (dv2 == 0) continue;
-                    const uint64_t L2 = L1 + (int64_t)dv2 * (int64_t)sm.stride[d2];
-                    if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)(s1 + (uint32_t)abs(dv2)) << 40) | L2; best = k < best ? k : best; }
-                }
-            }
-            best = warp_min_u64(best);
-            if (best != ~0ull) found = 2;
-        }
-        if (!found && pm.levels >= 3) {
-            for (uint32_t t1 = 0; t1 < T; ++t1) {
-                const uint32_t e1 = __ldg(&pm.tgt[t1]), d1 = e1 >> 8;
-                const int dv1 = (int)(e1 & 255) - (int)c[d1];
-                if (dv1 == 0) continue;
-                const uint64_t L1 = L + (int64_t)dv1 * (int64_t)sm.stride[d1];
-                const uint32_t s1 = (uint32_t)abs(dv1);
-                for (uint32_t t2 = pm.dim_first[d1 + 1]; t2 < T; ++t2) {
-                    const uint32_t e2 = __ldg(&pm.tgt[t2]), d2 = e2 >> 8;
-                    const int dv2 = (int)(e2 & 255) - (int)c[d2];
-                    if (dv2 == 0) continue;
-                    const uint64_t L2 = L1 + (int64_t)dv2 * (int64_t)sm.stride[d2];
-                    const uint32_t s2 = s1 + (uint32_t)abs(dv2);
-                    for (uint32_t t3 = pm.dim_first[d2 + 1] + lane; t3 < T; t3 += 32) {
+        for (int level = 2; level <= pm.levels && !found; ++level) {
+            uint64_t best = ~0ull;
+            for (uint32_t q = tid; q < C2; q += blockDim.x) {
+                const uint32_t pr = __ldg(&pm.pairs[q]);
+                const uint32_t e1 = __ldg(&pm.tgt[pr & 0xFFFFu]), e2 = __ldg(&pm.tgt[pr >> 16]);
+                const uint32_t d1 = e1 >> 8, d2 = e2 >> 8;
+                const int dv1 = (int)(e1 & 255) - (int)c[d1], dv2 = (int)(e2 & 255) - (int)c[d2];
+                if (dv1 == 0 || dv2 == 0) continue;
+                const uint64_t L2 = L + (int64_t)dv1 * (int64_t)sm.stride[d1] + (int64_t)dv2 * (int64_t)sm.stride[d2];
+                const uint32_t s2 = (uint32_t)(abs(dv1) + abs(dv2));
+                if (level == 2) {
+                    if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)s2 << 40) | L2; best = k < best ? k : best; }
+                } else {
+#pragma unroll 4
+                    for (uint32_t t3 = pm.dim_first[d2 + 1]; t3 < T; ++t3) {
                         const uint32_t e3 = __ldg(&pm.tgt[t3]), d3 = e3 >> 8;
                         const int dv3 = (int)(e3 & 255) - (int)c[d3];
-                        if (dv3 == 0) continue;
                         const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
-                        if (bit_test(sm.bitmap, L3)) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
+                        if (dv3 != 0 && bit_test(sm.bitmap, L3)) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
                     }
                 }
             }
             best = warp_min_u64(best);
-            if (best != ~0ull) found = 3;
+            if ((tid & 31) == 0 && best != ~0ull) atomicMin(&s_best, best);
+            __syncthreads();
+            if (s_best != ~0ull) found = level;
         }
-        if (lane == 0) {
+        if (tid == 0) {
+            const uint64_t best = s_best;
             if (found) key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
             else { wl_out[atomicAdd(wl_out_count, 1u)] = slot; if (n_scanned) atomicAdd(n_scanned, 1ull); }
         }

@@ -193,21 +193,27 @@ static int plan_space(cao_space* s) {
     s->n_tab = (int)tab.size(); s->n_res = (int)res.size();
     std::vector<int32_t>& D = s->desc;
     D.assign(tab.size() + res.size() + s->cons.size(), 0);       // [tab offs][res offs][program offs of every constraint]
+    // programs first, so that the tabled descriptors can point at them
+    std::vector<int32_t> prog_off(s->cons.size());
+    for (size_t c = 0; c < s->cons.size(); ++c) {
+        prog_off[c] = (int32_t)D.size();
+        D[tab.size() + res.size() + c] = (int32_t)D.size();
+        D.insert(D.end(), s->cons[c].begin(), s->cons[c].end());
+    }
+    s->max_table_threads = 0;
     for (size_t k = 0; k < tab.size(); ++k) {
         const ConsPlan& p = s->plan[tab[k]];
         D[k] = (int32_t)D.size();
         D.push_back((int32_t)(uint32_t)p.table_off); D.push_back((int32_t)(uint32_t)(p.table_off >> 32));
         D.push_back((int32_t)p.outer.size());
         for (size_t e = 0; e < p.outer.size(); ++e) { D.push_back(p.outer[e]); D.push_back((int32_t)p.cstride[e]); }
+        D.push_back(prog_off[tab[k]]); D.push_back((int32_t)s->cons[tab[k]].size()); D.push_back((int32_t)p.rows);
+        s->max_table_threads = std::max<uint64_t>(s->max_table_threads, p.rows * s->Wb * 64);
     }
     for (size_t k = 0; k < res.size(); ++k) {
         D[tab.size() + k] = (int32_t)D.size();
         D.push_back((int32_t)s->cons[res[k]].size());
         D.insert(D.end(), s->cons[res[k]].begin(), s->cons[res[k]].end());
-    }
-    for (size_t c = 0; c < s->cons.size(); ++c) {
-        D[tab.size() + res.size() + c] = (int32_t)D.size();
-        D.insert(D.end(), s->cons[c].begin(), s->cons[c].end());
     }
     // scratch layout
     uint64_t off = 0;
@@ -248,18 +254,11 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
     const int64_t* d_dom = (const int64_t*)(sc + s->off_dom);
     const int32_t* d_desc = (const int32_t*)(sc + s->off_desc);
     uint64_t* d_tables = (uint64_t*)(sc + s->off_tables);
-    const size_t prog_base = (size_t)s->n_tab + s->n_res;
-    for (size_t c = 0; c < s->cons.size(); ++c) {
-        const ConsPlan& p = s->plan[c];
-        if (!p.tabled) continue;
-        TableBuildArgs a{};
-        a.dom = d_dom; a.prog = d_desc + s->desc[prog_base + c]; a.out = d_tables + p.table_off;
-        a.rows = p.rows; a.B = s->B; a.Wb = s->Wb; a.nw = (int32_t)s->cons[c].size(); a.t = s->t;
-        a.n_outer = (int32_t)p.outer.size();
-        for (size_t e = 0; e < p.outer.size(); ++e) { a.dig[e] = (uint8_t)p.outer[e]; a.cstride[e] = p.cstride[e]; }
-        uint64_t threads = p.rows * s->Wb;
-        { ProfScope ps(PK_TABLE, st); k_build_table<<<(unsigned)((threads + 127) / 128), 128, 0, st>>>(s->meta, a); }
-        CAO_LAUNCHED("k_build_table");
+    if (s->n_tab) {
+        ProfScope ps(PK_TABLE, st);
+        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 255) / 256, 148 * 16), (unsigned)s->n_tab);
+        k_build_tables<<<grid, 256, 0, st>>>(s->meta, d_dom, d_desc, d_tables, s->B, s->Wb, s->t);
+        CAO_LAUNCHED("k_build_tables");
     }
     EnumArgs ea{};
     ea.B = s->B; ea.magicB = s->B > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + s->B - 1) / s->B) : 0;
@@ -311,9 +310,17 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
         int lv = 1;
         if (e[2] * 60.0 <= scan_cost) { lv = 2; if (e[3] * 60.0 <= scan_cost) lv = 3; }
         if (s->probe_levels_req >= 0) lv = std::min(3, std::max(0, s->probe_levels_req));
+        if (e[2] > 65536.0) lv = std::min(lv, 1);                      // the pair list would not fit its budget
+        s->h_pairs.clear();
+        if (lv >= 2)
+            for (uint32_t t1 = 0; t1 < s->probe.T; ++t1)
+                for (uint32_t t2 = s->probe.dim_first[(s->h_tgt[t1] >> 8) + 1]; t2 < s->probe.T; ++t2)
+                    s->h_pairs.push_back(t1 | (t2 << 16));
+        s->probe.C2 = (uint32_t)s->h_pairs.size();
         s->probe.levels = lv;
     }
     s->off_tgt = off; off = align256(off + std::max<uint64_t>(1, s->h_tgt.size()) * 2);
+    s->off_pairs = off; off = align256(off + std::max<uint64_t>(1, s->h_pairs.size()) * 4);
     s->table_bytes = off;
     return CAO_OK;
 }
@@ -343,6 +350,9 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
     CAO_LAUNCHED("k_fill");
     CAO_CUDA(cudaMemcpyAsync(tb + s->off_tgt, s->h_tgt.data(), s->h_tgt.size() * 2, cudaMemcpyHostToDevice, st));
     s->probe.tgt = (const uint16_t*)(tb + s->off_tgt);
+    if (!s->h_pairs.empty())
+        CAO_CUDA(cudaMemcpyAsync(tb + s->off_pairs, s->h_pairs.data(), s->h_pairs.size() * 4, cudaMemcpyHostToDevice, st));
+    s->probe.pairs = (const uint32_t*)(tb + s->off_pairs);
     s->meta.rows = rows; s->meta.Ltab = Ltab; s->meta.dir = dir;
     s->filled = true;
     return CAO_OK;
