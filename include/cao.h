@@ -98,6 +98,10 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
 int cao_space_table_bytes(const cao_space* s, uint64_t* bytes);
 /* Pass 2: valid rows (V x row_bytes), Ltab (V x u64) and the rank directory, into d_table. */
 int cao_space_build_fill(cao_space* s, void* d_table, void* stream);
+/* Re-runs the whole of S1 (tables, bitmap, counts, scan, rows, Ltab, directory) into the buffers of the last
+ * build, asynchronously and without any host round trip: the definition is unchanged, so V and the layout are
+ * the ones build_count returned.  Needs a completed build_count + build_fill; d_scratch must still be alive. */
+int cao_space_rebuild(cao_space* s, void* stream);
 int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes);
 /* Borrowed device views into the caller's buffers; rank_dir[i] = number of valid L < 512*i. */
 int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t** d_rows,

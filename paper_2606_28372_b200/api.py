@@ -51,6 +51,7 @@ SIGNATURES = {
     "cao_space_build_count": (C.c_int, [vp, vp, vp, vp, pu64]),
     "cao_space_table_bytes": (C.c_int, [vp, pu64]),
     "cao_space_build_fill": (C.c_int, [vp, vp, vp]),
+    "cao_space_rebuild": (C.c_int, [vp, vp]),
     "cao_space_sizes": (C.c_int, [vp, pu64, pu64, pi32, pi32]),
     "cao_space_views": (C.c_int, [vp, pvp, pvp, pvp, pvp]),
     "cao_space_is_valid": (C.c_int, [vp, vp, u64, vp, vp]),
@@ -189,6 +190,10 @@ class Space:
         self.alloc_table()
         self.build_fill()
         return self
+
+    def rebuild(self):
+        """All of S1 again into the same buffers, asynchronously (no host round trip)."""
+        _check(lib().cao_space_rebuild(self._h, _stream()))
 
     def sizes(self):
         N, V, n, rb = u64(), u64(), i32(), i32()

@@ -154,13 +154,18 @@ __device__ __forceinline__ int64_t sat_mul(int64_t a, int64_t b) {
     return sat64(lo);
 }
 
-// O1: postfix interpreter over the VALUES x[d]; returns 1/0; a zero divisor makes the constraint false.
-static __device__ __noinline__ int eval_program(const int32_t* __restrict__ w, int nw, const int64_t* __restrict__ x) {
-    int64_t st[CAO_MAX_STACK];
-    int sp = 0;
-    for (int pc = 0; pc < nw; ++pc) {
+// O1: postfix interpreter over the VALUES x[d].  Runs from token pc with the stack st[0..sp).  Returns 1/0 at
+// the end of the program (a zero divisor makes the constraint false: 0).  If stop_t >= 0 it stops BEFORE the
+// first PUSH_PARAM d with d >= stop_t and returns 2 with the resume point in *pc_out / *sp_out: the prefix of
+// a program that reads only outer digits is executed once per block of configs, not once per config.
+static __device__ __noinline__ int eval_core(const int32_t* __restrict__ w, int nw, const int64_t* __restrict__ x, int pc,
+                                             int64_t* st, int sp, int stop_t, int* pc_out, int* sp_out) {
+    for (; pc < nw; ++pc) {
         int op = w[pc];
-        if (op == 1) { st[sp++] = sat64(x[w[++pc]]); continue; }
+        if (op == 1) {
+            if (stop_t >= 0 && w[pc + 1] >= stop_t) { *pc_out = pc; *sp_out = sp; return 2; }
+            st[sp++] = sat64(x[w[++pc]]); continue;
+        }
         if (op == 2) {
             uint64_t lo = (uint32_t)w[pc + 1], hi = (uint32_t)w[pc + 2]; pc += 2;
             st[sp++] = sat64((int64_t)(lo | (hi << 32))); continue;
@@ -186,7 +191,16 @@ static __device__ __noinline__ int eval_program(const int32_t* __restrict__ w, i
     }
     return st[0] != 0;
 }
-
+static __device__ __forceinline__ int eval_program(const int32_t* __restrict__ w, int nw, const int64_t* __restrict__ x) {
+    int64_t st[CAO_MAX_STACK];
+    int a, b;
+    return eval_core(w, nw, x, 0, st, 0, -1, &a, &b);
+}
+// k-th (0-based) set bit of a 64-bit word that has more than k bits set.
+__device__ __forceinline__ int kth_set_bit64(uint64_t word, uint32_t k) {
+    const uint32_t lo = (uint32_t)word, hi = (uint32_t)(word >> 32), cl = __popc(lo);
+    return k < cl ? (int)__fns(lo, 0, (int)k + 1) : 32 + (int)__fns(hi, 0, (int)(k - cl) + 1);
+}
 // ---------------------------------------------------------------------------------------------
 // Packed index rows: ROWW uint32 words (ROWW = 4 for n <= 16, 8 for n <= 32), 16-byte aligned.
 template <int ROWW>

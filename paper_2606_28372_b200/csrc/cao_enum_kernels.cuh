@@ -83,27 +83,60 @@ __global__ void __launch_bounds__(256) k_enum_pass1(const __grid_constant__ Spac
             any = 0;
             for (uint32_t j = 0; j < a.Wb; ++j) { uint64_t v = mk[j] & __ldg(&tab[j]); mk[j] = v; any |= v; }
         }
-        if (a.n_res && any) {
+    }
+    // Phase 1b: residual constraints (too wide for a table, or plain mode).  One warp per block of configs: the
+    // program prefix that reads only outer digits runs once per block, the lanes then share the surviving bits
+    // of each mask word (warp-level compaction by k-th-set-bit selection) and clear the ones that fail.
+    if (a.n_res) {
+        __syncthreads();
+        const uint32_t lane = tid & 31, warp = tid >> 5, nwarp = bd >> 5;
+        for (uint32_t i = warp; i <= a.nb; i += nwarp) {
+            const uint64_t o = o0 + i;
+            if (o >= a.n_blocks) continue;
+            uint64_t* mk = masks + (size_t)i * a.Wb;
+            uint64_t anyb = 0;
+            for (uint32_t j = lane; j < a.Wb; j += 32) anyb |= mk[j];
+            if (!__any_sync(0xFFFFFFFFu, anyb != 0)) continue;
             int64_t x[CAO_MAX_DIMS];
-            for (int d = 0; d < a.t; ++d) x[d] = a.dom[d * 256 + od[d * bd + tid]];
-            for (uint32_t j = 0; j < a.Wb; ++j) {
-                uint64_t v = mk[j], keep = v;
-                while (v) {
-                    int b = __ffsll((long long)v) - 1; v &= v - 1;
-                    uint64_t p = (uint64_t)j * 64 + b;
-                    for (int d = sm.n - 1; d >= a.t; --d) {
-                        uint32_t m = sm.m[d]; uint32_t idx = 0;
-                        if (m > 1) { uint64_t p2 = div_magic(p, sm.magic[d]); idx = (uint32_t)(p - p2 * m); p = p2; }
-                        x[d] = a.dom[d * 256 + idx];
-                    }
-                    bool ok = true;
-                    for (int r = 0; r < a.n_res && ok; ++r) {
-                        const int32_t* ds = a.desc + __ldg(&a.desc[a.n_tab + r]);
-                        ok = eval_program(ds + 1, __ldg(&ds[0]), x);
-                    }
-                    if (!ok) keep &= ~(1ull << b);
+            {
+                uint64_t q = o;
+                for (int d = a.t - 1; d >= 0; --d) {
+                    const uint32_t m = sm.m[d]; uint32_t idx = 0;
+                    if (m > 1) { const uint64_t q2 = div_magic(q, sm.magic[d]); idx = (uint32_t)(q - q2 * m); q = q2; }
+                    x[d] = a.dom[d * 256 + idx];
                 }
-                mk[j] = keep;
+            }
+            for (int r = 0; r < a.n_res; ++r) {
+                const int32_t* ds = a.desc + __ldg(&a.desc[a.n_tab + r]);
+                const int nw = __ldg(&ds[0]);
+                int64_t st0[CAO_MAX_STACK];
+                int pc0 = 0, sp0 = 0;
+                const int pre = eval_core(ds + 1, nw, x, 0, st0, 0, a.t, &pc0, &sp0);       // block-uniform
+                if (pre == 1) continue;                                                    // holds for the whole block
+                if (pre == 0) { for (uint32_t j = lane; j < a.Wb; j += 32) mk[j] = 0; __syncwarp(); break; }
+                for (uint32_t j = 0; j < a.Wb; ++j) {
+                    const uint64_t word = mk[j];
+                    const uint32_t c = __popcll(word);
+                    uint64_t kill = 0;
+                    for (uint32_t k = lane; k < c; k += 32) {
+                        const int bit = kth_set_bit64(word, k);
+                        uint64_t p = (uint64_t)j * 64 + bit;
+                        for (int d = sm.n - 1; d >= a.t; --d) {
+                            const uint32_t m = sm.m[d]; uint32_t idx = 0;
+                            if (m > 1) { const uint64_t p2 = div_magic(p, sm.magic[d]); idx = (uint32_t)(p - p2 * m); p = p2; }
+                            x[d] = a.dom[d * 256 + idx];
+                        }
+                        int64_t st[CAO_MAX_STACK];
+                        for (int z = 0; z < sp0; ++z) st[z] = st0[z];
+                        int u0, u1;
+                        if (!eval_core(ds + 1, nw, x, pc0, st, sp0, -1, &u0, &u1)) kill |= 1ull << bit;
+                    }
+                    const uint32_t klo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)kill);
+                    const uint32_t khi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(kill >> 32));
+                    __syncwarp();
+                    if (lane == 0 && (klo | khi)) mk[j] = word & ~(((uint64_t)khi << 32) | klo);
+                    __syncwarp();
+                }
             }
         }
     }

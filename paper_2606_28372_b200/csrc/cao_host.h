@@ -55,6 +55,7 @@ struct cao_space {
     uint64_t tables_words = 0, n_part = 0, max_table_threads = 0;
     uint64_t bitmap_bytes = 0;
     void* d_scratch = nullptr;
+    void* d_table = nullptr;
     // table layout
     uint64_t off_rows = 0, off_Ltab = 0, off_dir = 0, off_tgt = 0, table_bytes = 0;
     // Hamming-level probes (S5)

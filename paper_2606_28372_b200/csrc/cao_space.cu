@@ -237,18 +237,8 @@ int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64
     return CAO_OK;
 }
 
-int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V) {
-    if (!s || !h_V) return cao_fail(CAO_E_INVALID_ARG, "cao_space_build_count: NULL argument");
-    if (!s->planned) return cao_fail(CAO_E_STATE, "cao_space_build_count: call cao_space_build_workspace_bytes first");
-    if (!d_bitmap || !d_scratch || ((uintptr_t)d_bitmap & 255) || ((uintptr_t)d_scratch & 255))
-        return cao_fail(CAO_E_WORKSPACE, "cao_space_build_count: bitmap/scratch must be non-NULL and 256-byte aligned");
-    cudaStream_t st = (cudaStream_t)stream;
-    const int n = s->meta.n;
-    uint8_t* sc = (uint8_t*)d_scratch;
-    std::vector<int64_t> hdom((size_t)n * 256, 0);
-    for (int d = 0; d < n; ++d) std::copy(s->dom[d].begin(), s->dom[d].end(), hdom.begin() + (size_t)d * 256);
-    CAO_CUDA(cudaMemcpyAsync(sc + s->off_dom, hdom.data(), hdom.size() * 8, cudaMemcpyHostToDevice, st));
-    CAO_CUDA(cudaMemcpyAsync(sc + s->off_desc, s->desc.data(), s->desc.size() * 4, cudaMemcpyHostToDevice, st));
+// S1 pass 1 on `st`: constraint tables, block masks -> bitmap + per-512 counts, exclusive scan of the counts.
+static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t st) {
     CAO_CUDA(cudaMemsetAsync(sc + s->off_cnt, 0, (s->nd + 1) * 4, st));
     s->meta.bitmap = (const uint64_t*)d_bitmap;
     const int64_t* d_dom = (const int64_t*)(sc + s->off_dom);
@@ -282,6 +272,38 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
         k_scan_apply<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
         CAO_LAUNCHED("k_scan_apply");
     }
+    return CAO_OK;
+}
+
+// S1 pass 2 on `st`: rows, Ltab, rank directory.
+static int launch_fill(cao_space* s, uint8_t* tb, cudaStream_t st) {
+    uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
+    const uint32_t* cnt = (const uint32_t*)((uint8_t*)s->d_scratch + s->off_cnt);
+    uint64_t threads = s->nd * 16;
+    unsigned grid = (unsigned)((threads + 255) / 256);
+    {
+        ProfScope ps(PK_FILL, st);
+        if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+        else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+    }
+    CAO_LAUNCHED("k_fill");
+    return CAO_OK;
+}
+
+int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V) {
+    if (!s || !h_V) return cao_fail(CAO_E_INVALID_ARG, "cao_space_build_count: NULL argument");
+    if (!s->planned) return cao_fail(CAO_E_STATE, "cao_space_build_count: call cao_space_build_workspace_bytes first");
+    if (!d_bitmap || !d_scratch || ((uintptr_t)d_bitmap & 255) || ((uintptr_t)d_scratch & 255))
+        return cao_fail(CAO_E_WORKSPACE, "cao_space_build_count: bitmap/scratch must be non-NULL and 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n = s->meta.n;
+    uint8_t* sc = (uint8_t*)d_scratch;
+    std::vector<int64_t> hdom((size_t)n * 256, 0);
+    for (int d = 0; d < n; ++d) std::copy(s->dom[d].begin(), s->dom[d].end(), hdom.begin() + (size_t)d * 256);
+    CAO_CUDA(cudaMemcpyAsync(sc + s->off_dom, hdom.data(), hdom.size() * 8, cudaMemcpyHostToDevice, st));
+    CAO_CUDA(cudaMemcpyAsync(sc + s->off_desc, s->desc.data(), s->desc.size() * 4, cudaMemcpyHostToDevice, st));
+    { int rc = launch_pass1(s, d_bitmap, sc, st); if (rc) return rc; }
+    uint64_t* d_V = (uint64_t*)(sc + s->off_V);
     uint64_t V = 0;
     CAO_CUDA(cudaMemcpyAsync(&V, d_V, 8, cudaMemcpyDeviceToHost, st));
     CAO_CUDA(cudaStreamSynchronize(st));
@@ -339,23 +361,25 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     uint8_t* tb = (uint8_t*)d_table;
     uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
-    const uint32_t* cnt = (const uint32_t*)((uint8_t*)s->d_scratch + s->off_cnt);
-    uint64_t threads = s->nd * 16;
-    unsigned grid = (unsigned)((threads + 255) / 256);
-    {
-        ProfScope ps(PK_FILL, st);
-        if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
-        else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
-    }
-    CAO_LAUNCHED("k_fill");
+    { int rc = launch_fill(s, tb, st); if (rc) return rc; }
     CAO_CUDA(cudaMemcpyAsync(tb + s->off_tgt, s->h_tgt.data(), s->h_tgt.size() * 2, cudaMemcpyHostToDevice, st));
     s->probe.tgt = (const uint16_t*)(tb + s->off_tgt);
     if (!s->h_pairs.empty())
         CAO_CUDA(cudaMemcpyAsync(tb + s->off_pairs, s->h_pairs.data(), s->h_pairs.size() * 4, cudaMemcpyHostToDevice, st));
     s->probe.pairs = (const uint32_t*)(tb + s->off_pairs);
     s->meta.rows = rows; s->meta.Ltab = Ltab; s->meta.dir = dir;
+    s->d_table = d_table;
     s->filled = true;
     return CAO_OK;
+}
+
+int cao_space_rebuild(cao_space* s, void* stream) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_rebuild: NULL space");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_rebuild: the space must have been built once");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st);
+    if (rc) return rc;
+    return launch_fill(s, (uint8_t*)s->d_table, st);
 }
 
 int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes) {

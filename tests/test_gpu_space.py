@@ -184,3 +184,18 @@ def test_exp_neg_spec_bit_exact():
     zb = (np.arange(1 << 22, dtype=np.uint32) + np.float32(1.0).view(np.uint32)).view(np.float32)
     got = cao.test_exp_neg(torch.from_numpy(zb).cuda()).cpu().numpy()
     assert np.array_equal(got.view(np.uint32), O.exp_neg_spec_many(zb).view(np.uint32))
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_rebuild_reproduces_the_space(cfg):
+    """cao_space_rebuild: all of S1 again, asynchronously, into the same (wiped) buffers."""
+    sp, os_ = oracle_space(cfg, with_objective=False)
+    gs = _gpu_space(sp)
+    gs._bitmap.zero_(); gs._table.zero_()
+    gs.rebuild()
+    torch.cuda.synchronize()
+    _check_space(sp, os_, gs)
+    rows = np.stack([np.random.default_rng(1).integers(0, m, size=64) for m in sp.m], axis=1).astype(np.uint8)
+    want = os_.repair(rows)
+    rank, key = gs.repair(rows)                                         # probe tables survive the rebuild
+    assert np.array_equal(rank.cpu().numpy().view(np.uint32), want["rank"])
