@@ -135,6 +135,10 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
                     uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens,
                     uint64_t seed, void* d_workspace, void* stream, cao_runs** out);
 void cao_runs_destroy(cao_runs* r);
+/* How cao_runs_step executes: 1 (default) = one fused persistent kernel, one CTA per run for all the requested
+ * generations; 0 = phased, per generation k_op -> k_probe23 -> k_scan -> k_finish over all runs (better when
+ * most candidates need the table scan).  Identical results. */
+int cao_runs_set_mode(cao_runs* r, int32_t mode);
 /* S3-S7, n_generations times (stops recording at max_gens).  Asynchronous. */
 int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream);
 /* Copies per-run results to DEVICE arrays of n_runs elements each (any may be NULL). */

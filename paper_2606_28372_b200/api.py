@@ -61,6 +61,7 @@ SIGNATURES = {
     "cao_runs_workspace_bytes": (C.c_int, [vp, i32, i32, u32, u32, pu64]),
     "cao_runs_create": (C.c_int, [vp, i32, C.POINTER(HParams), u32, u32, i32, u32, u32, u64, vp, vp, pvp]),
     "cao_runs_destroy": (None, [vp]),
+    "cao_runs_set_mode": (C.c_int, [vp, i32]),
     "cao_runs_step": (C.c_int, [vp, u32, vp]),
     "cao_runs_best": (C.c_int, [vp, vp, vp, vp, vp, vp]),
     "cao_runs_trajectory": (C.c_int, [vp, pvp, C.POINTER(u32)]),
@@ -121,7 +122,7 @@ def profile_enable(on=True):
 def profile_read():
     """{kernel class name: (total ms, launches)} since profile_enable(True)."""
     out = {}
-    for cls in range(10):
+    for cls in range(11):
         ms, n = C.c_double(), u64()
         _check(lib().cao_profile_read(cls, C.byref(ms), C.byref(n)))
         out[lib().cao_profile_name(cls).decode()] = (ms.value, n.value)
@@ -289,7 +290,8 @@ class Space:
 class Runs:
     """n_runs independent simulated tuning runs of one algorithm; creation executes generation 0 (S2)."""
 
-    def __init__(self, space: Space, algo, n_runs, pop, budget=0, max_gens=100, seed=0, first_run=0, hparams=None):
+    def __init__(self, space: Space, algo, n_runs, pop, budget=0, max_gens=100, seed=0, first_run=0, hparams=None,
+                 mode=None):
         self.space, self.R, self.P, self.n = space, int(n_runs), int(pop), space.n
         self.algo = ALGOS[algo] if isinstance(algo, str) else int(algo)
         self.hp = hparams or HParams.default()
@@ -302,6 +304,13 @@ class Runs:
         _check(lib().cao_runs_create(space._h, self.algo, C.byref(self.hp), self.R, int(first_run), self.P, int(budget),
                                      self.max_gens, int(seed), self._ws.data_ptr(), _stream(), C.byref(h)))
         self._h = h
+        if mode is not None:
+            self.set_mode(mode)
+
+    def set_mode(self, mode):
+        """'fused' / 1 = one persistent kernel per step call; 'phased' / 0 = per-generation kernels."""
+        m = {"fused": 1, "phased": 0}.get(mode, mode)
+        _check(lib().cao_runs_set_mode(self._h, int(m)))
 
     def step(self, k=1):
         _check(lib().cao_runs_step(self._h, int(k), _stream()))

@@ -196,10 +196,19 @@ static __device__ __forceinline__ int eval_program(const int32_t* __restrict__ w
     int a, b;
     return eval_core(w, nw, x, 0, st, 0, -1, &a, &b);
 }
-// k-th (0-based) set bit of a 64-bit word that has more than k bits set.
+// k-th (0-based) set bit of a word that has more than k bits set: binary search on popcounts of the low part.
+__device__ __forceinline__ int kth_set_bit32(uint32_t w, uint32_t k) {
+    int pos = 0; uint32_t c;
+    c = __popc(w & 0xFFFFu); if (k >= c) { pos += 16; k -= c; w >>= 16; }
+    c = __popc(w & 0xFFu);   if (k >= c) { pos += 8;  k -= c; w >>= 8; }
+    c = __popc(w & 0xFu);    if (k >= c) { pos += 4;  k -= c; w >>= 4; }
+    c = __popc(w & 0x3u);    if (k >= c) { pos += 2;  k -= c; w >>= 2; }
+    c = w & 1u;              if (k >= c) { pos += 1; }
+    return pos;
+}
 __device__ __forceinline__ int kth_set_bit64(uint64_t word, uint32_t k) {
     const uint32_t lo = (uint32_t)word, hi = (uint32_t)(word >> 32), cl = __popc(lo);
-    return k < cl ? (int)__fns(lo, 0, (int)k + 1) : 32 + (int)__fns(hi, 0, (int)(k - cl) + 1);
+    return k < cl ? kth_set_bit32(lo, k) : 32 + kth_set_bit32(hi, k - cl);
 }
 // ---------------------------------------------------------------------------------------------
 // Packed index rows: ROWW uint32 words (ROWW = 4 for n <= 16, 8 for n <= 32), 16-byte aligned.

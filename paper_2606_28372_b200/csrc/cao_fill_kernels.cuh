@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) k_fill(const __grid_constant__ SpaceMeta 
         uint32_t t = 0;                                                  // last lane with off <= j
 #pragma unroll
         for (int step = 16; step; step >>= 1) { const uint32_t c = t + step; if (c < 32 && s_off[wib][c] <= j) t = c; }
-        const uint32_t b = __fns(s_bits[wib][t], 0, (int)(j - s_off[wib][t]) + 1);
+        const uint32_t b = (uint32_t)kth_set_bit32(s_bits[wib][t], j - s_off[wib][t]);
         const uint64_t L = (hw0 + t) * 32 + b;
         uint32_t w[ROWW];
         decode_row<ROWW>(sm, L, w);

@@ -16,7 +16,7 @@ int cao_cuda_check(cudaError_t e, const char* what);
 #define CAO_LAUNCHED(what) do { ++g_cao_launches; int rc_ = cao_cuda_check(cudaGetLastError(), what); if (rc_) return rc_; } while (0)
 
 // Optional per-kernel-class device timing (cao_profile_*): CUDA events on the launching stream around each launch.
-enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_N };
+enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_GEN, PK_N };
 extern std::atomic<int> g_cao_prof_on;
 void cao_prof_mark(int cls, bool end, cudaStream_t st);
 struct ProfScope {
@@ -46,7 +46,7 @@ struct cao_space {
     // enumeration plan
     int t = 0;                         // first inner digit: digits t..n-1 form one bitmap block of B configs
     uint64_t B = 0, n_blocks = 0, nd = 0, n_words = 0;
-    uint32_t Wb = 0, nb = 0;           // u64 words per block mask; blocks per CTA
+    uint32_t Wb = 0, nb = 0, nb_tabled = 0;           // u64 words per block mask; blocks per CTA
     std::vector<ConsPlan> plan;
     std::vector<int32_t> desc;         // descriptor words uploaded to the device
     int n_tab = 0, n_res = 0;

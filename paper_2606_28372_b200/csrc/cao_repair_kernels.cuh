@@ -62,53 +62,101 @@ __device__ __forceinline__ uint64_t warp_min_u64(uint64_t v) {
     return v;
 }
 
+// Block-cooperative probe of ONE candidate whose row sits in shared memory (s_cw, ROWW words).  *s_best must be
+// ~0 and visible to the block on entry.  Threads walk the flattened list of target pairs (t1 < t2, different
+// dimensions); level 3 adds a serial walk over the targets of the dimensions after t2's.  Returns the level
+// that found a valid neighbour (0 = none) -- block-uniform -- and leaves (sad << 40 | L') in *s_best.
+template <int ROWW>
+__device__ __forceinline__ int probe23_cta(const SpaceMeta& sm, const ProbeMeta& pm, const uint32_t* s_cw,
+                                           unsigned long long* s_best) {
+    const uint8_t* c = (const uint8_t*)s_cw;
+    const uint32_t tid = threadIdx.x, T = pm.T, C2 = pm.C2;
+    uint64_t L = 0;
+    for (int d = 0; d < sm.n; ++d) L += (uint64_t)c[d] * sm.stride[d];
+    int found = 0;
+    for (int level = 2; level <= pm.levels && !found; ++level) {
+        uint64_t best = ~0ull;
+        for (uint32_t q = tid; q < C2; q += blockDim.x) {
+            const uint32_t pr = __ldg(&pm.pairs[q]);
+            const uint32_t e1 = __ldg(&pm.tgt[pr & 0xFFFFu]), e2 = __ldg(&pm.tgt[pr >> 16]);
+            const uint32_t d1 = e1 >> 8, d2 = e2 >> 8;
+            const int dv1 = (int)(e1 & 255) - (int)c[d1], dv2 = (int)(e2 & 255) - (int)c[d2];
+            if (dv1 == 0 || dv2 == 0) continue;
+            const uint64_t L2 = L + (int64_t)dv1 * (int64_t)sm.stride[d1] + (int64_t)dv2 * (int64_t)sm.stride[d2];
+            const uint32_t s2 = (uint32_t)(abs(dv1) + abs(dv2));
+            if (level == 2) {
+                if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)s2 << 40) | L2; best = k < best ? k : best; }
+            } else {
+#pragma unroll 4
+                for (uint32_t t3 = pm.dim_first[d2 + 1]; t3 < T; ++t3) {
+                    const uint32_t e3 = __ldg(&pm.tgt[t3]), d3 = e3 >> 8;
+                    const int dv3 = (int)(e3 & 255) - (int)c[d3];
+                    const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
+                    if (dv3 != 0 && bit_test(sm.bitmap, L3)) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
+                }
+            }
+        }
+        best = warp_min_u64(best);
+        if ((tid & 31) == 0 && best != ~0ull) atomicMin(s_best, best);
+        __syncthreads();
+        if (*s_best != ~0ull) found = level;
+    }
+    return found;
+}
+
+// Block-cooperative brute-force scan of the whole valid table for up to NB candidates at once (rows in shared
+// memory, s_cw[b * ROWW ..]); the rows are read straight from L2, coalesced, every thread keeps NB running minima.
+// s_key[b] must be ~0 on entry; on exit it holds ham << 45 | sad << 32 | rank.  Ends with a barrier.
+template <int ROWW, int NB>
+__device__ __forceinline__ void scan_cta(const SpaceMeta& sm, const uint32_t* s_cw, int nb, unsigned long long* s_key) {
+    uint32_t c[NB][ROWW];
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int k = 0; k < ROWW; ++k) c[b][k] = b < nb ? s_cw[b * ROWW + k] : 0;
+    uint64_t best[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) best[b] = ~0ull;
+    for (uint32_t r = threadIdx.x; r < sm.V; r += blockDim.x) {
+        uint32_t v[ROWW];
+        load_row<ROWW>(sm.rows + (uint64_t)r * (ROWW * 4), v);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            uint32_t sad = 0, ham = 0;
+#pragma unroll
+            for (int k = 0; k < ROWW; ++k) {
+                sad = sad4_acc(c[b][k], v[k], sad);
+                const uint32_t x = c[b][k] ^ v[k];
+                ham += __popc((((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x) & 0x80808080u);
+            }
+            const uint64_t key = ((uint64_t)((ham << 13) + sad) << 32) | r;
+            best[b] = key < best[b] ? key : best[b];
+        }
+    }
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const uint64_t m = warp_min_u64(best[b]);
+        if ((threadIdx.x & 31) == 0 && b < nb) atomicMin(&s_key[b], m);
+    }
+    __syncthreads();
+}
+
 template <int ROWW>
 __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
                                                  const uint8_t* __restrict__ cand_rows, const uint32_t* __restrict__ wl,
                                                  const uint32_t* __restrict__ wl_count, unsigned long long* key,
                                                  uint32_t* wl_out, uint32_t* wl_out_count, unsigned long long* n_scanned) {
-    // One CTA per worklist candidate.  Threads walk the flattened list of target pairs (t1 < t2, different
-    // dimensions); level 3 adds a serial walk over the targets of the dimensions after t2's.
+    // One CTA per worklist candidate.
     __shared__ uint32_t s_cw[ROWW];
     __shared__ unsigned long long s_best;
-    const uint8_t* c = (const uint8_t*)s_cw;
-    const uint32_t count = *wl_count, tid = threadIdx.x, T = pm.T, C2 = pm.C2;
+    const uint32_t count = *wl_count, tid = threadIdx.x;
     for (uint32_t ci = blockIdx.x; ci < count; ci += gridDim.x) {
         const uint32_t slot = wl[ci];
         __syncthreads();
         if (tid < ROWW) s_cw[tid] = ((const uint32_t*)(cand_rows + (uint64_t)slot * (ROWW * 4)))[tid];
         if (tid == 0) s_best = ~0ull;
         __syncthreads();
-        uint64_t L = 0;
-        for (int d = 0; d < sm.n; ++d) L += (uint64_t)c[d] * sm.stride[d];
-        int found = 0;
-        for (int level = 2; level <= pm.levels && !found; ++level) {
-            uint64_t best = ~0ull;
-            for (uint32_t q = tid; q < C2; q += blockDim.x) {
-                const uint32_t pr = __ldg(&pm.pairs[q]);
-                const uint32_t e1 = __ldg(&pm.tgt[pr & 0xFFFFu]), e2 = __ldg(&pm.tgt[pr >> 16]);
-                const uint32_t d1 = e1 >> 8, d2 = e2 >> 8;
-                const int dv1 = (int)(e1 & 255) - (int)c[d1], dv2 = (int)(e2 & 255) - (int)c[d2];
-                if (dv1 == 0 || dv2 == 0) continue;
-                const uint64_t L2 = L + (int64_t)dv1 * (int64_t)sm.stride[d1] + (int64_t)dv2 * (int64_t)sm.stride[d2];
-                const uint32_t s2 = (uint32_t)(abs(dv1) + abs(dv2));
-                if (level == 2) {
-                    if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)s2 << 40) | L2; best = k < best ? k : best; }
-                } else {
-#pragma unroll 4
-                    for (uint32_t t3 = pm.dim_first[d2 + 1]; t3 < T; ++t3) {
-                        const uint32_t e3 = __ldg(&pm.tgt[t3]), d3 = e3 >> 8;
-                        const int dv3 = (int)(e3 & 255) - (int)c[d3];
-                        const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
-                        if (dv3 != 0 && bit_test(sm.bitmap, L3)) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
-                    }
-                }
-            }
-            best = warp_min_u64(best);
-            if ((tid & 31) == 0 && best != ~0ull) atomicMin(&s_best, best);
-            __syncthreads();
-            if (s_best != ~0ull) found = level;
-        }
+        const int found = probe23_cta<ROWW>(sm, pm, s_cw, &s_best);
         if (tid == 0) {
             const uint64_t best = s_best;
             if (found) key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));

@@ -10,7 +10,8 @@ struct cao_runs {
     SpaceMeta sm{};
     RunsMeta rm{};
     uint32_t gen = 0;
-    unsigned block = 32;
+    unsigned block = 32, block_fused = 128;
+    int mode = 1;                      // 1 = fused persistent k_gen, 0 = phased (k_op / k_probe23 / k_scan / k_finish)
     size_t smem_init = 0, smem_op = 0, smem_fin = 0;
     // raw state views for cao_runs_debug_state
     uint64_t bytes_idx = 0, bytes_pi = 0, bytes_pn = 0;
@@ -206,6 +207,7 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     const uint64_t RP = (uint64_t)n_runs * pop;
     r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
     r->block = (unsigned)((pop + 31) / 32 * 32);
+    r->block_fused = std::max(r->block, 128u);
     const size_t P = (size_t)pop, n = (size_t)s->meta.n;
     r->smem_init = P * 4;
     r->smem_op = algo == CAO_GA ? P * 12 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
@@ -233,6 +235,19 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
     if (!r) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_step: NULL runs");
     cudaStream_t st = (cudaStream_t)stream;
     const int algo = r->rm.algo, roww = r->sm.rowB / 4;
+    if (r->mode == 1) {                                                 // fused: one launch for all the generations
+        const uint32_t left = r->rm.max_gens - r->gen, ng = std::min(n_generations, left);   // g <= max_gens (O10)
+        if (ng == 0) return CAO_OK;
+        const uint32_t scratch_words = (uint32_t)((std::max(r->smem_op, r->smem_fin) + 3) / 4);
+        const size_t smem = (size_t)scratch_words * 4 + (size_t)r->rm.P * 4;
+#define CALL_GEN(A, W) \
+        if (smem > 48 * 1024) cudaFuncSetAttribute(k_gen<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        k_gen<A, W><<<r->rm.R, r->block_fused, smem, st>>>(r->sm, r->s->probe, r->rm, r->gen, ng, scratch_words)
+        { ProfScope ps(PK_GEN, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_GEN); }
+        CAO_LAUNCHED("k_gen");
+        r->gen += ng;
+        return CAO_OK;
+    }
     for (uint32_t it = 0; it < n_generations; ++it) {
         if (r->gen >= r->rm.max_gens) break;                            // g <= max_gens (O10)
         const uint32_t g = r->gen + 1;
@@ -253,6 +268,12 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
         CAO_LAUNCHED("k_finish");
         r->gen = g;
     }
+    return CAO_OK;
+}
+
+int cao_runs_set_mode(cao_runs* r, int32_t mode) {
+    if (!r || (mode != 0 && mode != 1)) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_set_mode: mode must be 0 (phased) or 1 (fused)");
+    r->mode = mode;
     return CAO_OK;
 }
 

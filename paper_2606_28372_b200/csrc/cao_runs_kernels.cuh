@@ -134,7 +134,8 @@ __global__ void __launch_bounds__(1024) k_init(const __grid_constant__ SpaceMeta
 // ---------------------------------------------------------------------------------------------
 // S4 + first half of S5 for the candidate held in w: store, validity, probe, worklist.
 template <int ROWW>
-__device__ __forceinline__ void candidate_tail(const SpaceMeta& sm, const RunsMeta& rm, uint64_t slot, const uint32_t (&w)[ROWW]) {
+__device__ __forceinline__ void candidate_tail(const SpaceMeta& sm, const RunsMeta& rm, uint64_t slot, const uint32_t (&w)[ROWW],
+                                               uint32_t* wl, uint32_t* wl_count, bool count_scans) {
     store_row<ROWW>(rm.cand + slot * (ROWW * 4), w);
     bool valid;
     uint64_t key = validate_probe<ROWW>(sm, w, rm.probe_levels >= 1, valid);
@@ -142,22 +143,19 @@ __device__ __forceinline__ void candidate_tail(const SpaceMeta& sm, const RunsMe
     rm.key[slot] = key;
     if (!valid) atomicAdd(&rm.counters[0], 1ull);
     if (key == CAO_KEY_NONE) {
-        worklist_push(rm.wl, rm.wl_count, (uint32_t)slot);
-        if (rm.probe_levels < 2) atomicAdd(&rm.counters[1], 1ull);       // straight to the scan
+        worklist_push(wl, wl_count, (uint32_t)slot);
+        if (count_scans) atomicAdd(&rm.counters[1], 1ull);               // straight to the scan
     }
 }
 
 #define ROW_BYTE(w, d) (((w)[(d) >> 2] >> (((d) & 3) * 8)) & 0xFFu)
 
+// S3 + S4 for an ACTIVE run k (block-uniform call, contains barriers).  Unresolved candidates go to (wl, wl_count).
 template <int ALGO, int ROWW>
-__global__ void __launch_bounds__(1024) k_op(const __grid_constant__ SpaceMeta sm, const __grid_constant__ RunsMeta rm, uint32_t g) {
-    extern __shared__ uint32_t s_dyn[];
-    __shared__ RunShared sh;
-    const uint32_t k = blockIdx.x, i = threadIdx.x, P = rm.P, run = rm.first_run + k;
+__device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, uint32_t k, uint32_t g, uint32_t* s_dyn,
+                                       RunShared& sh, uint32_t* wl, uint32_t* wl_count, bool count_scans) {
+    const uint32_t i = threadIdx.x, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
-    const bool active = rm.budget == 0 || rm.uniq[k] < rm.budget;       // O10 (g <= max_gens is enforced by the host)
-    if (i == 0) rm.active[k] = active ? 1 : 0;
-    if (!active) return;
     const uint64_t q = (uint64_t)k * P + i;
     uint32_t w[ROWW];
 #pragma unroll
@@ -286,25 +284,33 @@ __global__ void __launch_bounds__(1024) k_op(const __grid_constant__ SpaceMeta s
             }
         }
     }
-    if (i < P) candidate_tail<ROWW>(sm, rm, q, w);
+    if (i < P) candidate_tail<ROWW>(sm, rm, q, w, wl, wl_count, count_scans);
+}
+
+template <int ALGO, int ROWW>
+__global__ void __launch_bounds__(1024) k_op(const __grid_constant__ SpaceMeta sm, const __grid_constant__ RunsMeta rm, uint32_t g) {
+    extern __shared__ uint32_t s_dyn[];
+    __shared__ RunShared sh;
+    const uint32_t k = blockIdx.x;
+    const bool active = rm.budget == 0 || rm.uniq[k] < rm.budget;       // O10 (g <= max_gens is enforced by the host)
+    if (threadIdx.x == 0) rm.active[k] = active ? 1 : 0;
+    if (!active) return;
+    gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, rm.wl, rm.wl_count, rm.probe_levels < 2);
 }
 
 // ---------------------------------------------------------------------------------------------
 // S6 + S7 after the repair scan.
+__device__ __forceinline__ void frozen_row(const RunsMeta& rm, uint32_t k, uint32_t g) {      // thread 0: the row repeats (O10)
+    uint32_t* t = rm.traj + ((uint64_t)g * rm.R + k) * 3;
+    t[0] = fbits(rm.best_f[k]); t[1] = rm.best_rank[k]; t[2] = rm.uniq[k];
+}
+
+// S6 + S7 for an ACTIVE run k once every candidate has its repair key (block-uniform call, contains barriers).
 template <int ALGO, int ROWW>
-__global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMeta sm, const __grid_constant__ RunsMeta rm, uint32_t g) {
-    extern __shared__ uint32_t s_dyn[];
-    __shared__ RunShared sh;
-    const uint32_t k = blockIdx.x, i = threadIdx.x, P = rm.P, run = rm.first_run + k;
+__device__ __forceinline__ void gen_finish(const SpaceMeta& sm, const RunsMeta& rm, uint32_t k, uint32_t g, uint32_t* s_dyn,
+                                           RunShared& sh) {
+    const uint32_t i = threadIdx.x, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
-    if (k == 0 && i == 0) { *rm.wl_count = 0; *rm.wl2_count = 0; }                             // the scan of this generation is done
-    if (!rm.active[k]) {                                                // frozen run: its trajectory row repeats (O10)
-        if (i == 0) {
-            uint32_t* t = rm.traj + ((uint64_t)g * rm.R + k) * 3;
-            t[0] = fbits(rm.best_f[k]); t[1] = rm.best_rank[k]; t[2] = rm.uniq[k];
-        }
-        return;
-    }
     if (i == 0) eval_begin(rm, k, &sh);
     __syncthreads();
     const uint64_t q = (uint64_t)k * P + i;
@@ -401,5 +407,77 @@ __global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMe
         eval_end(rm, k, g, &sh);
         rm.gens_done[k] += 1;
         atomicAdd(&rm.counters[2], (unsigned long long)P);
+    }
+}
+
+template <int ALGO, int ROWW>
+__global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMeta sm, const __grid_constant__ RunsMeta rm, uint32_t g) {
+    extern __shared__ uint32_t s_dyn[];
+    __shared__ RunShared sh;
+    const uint32_t k = blockIdx.x;
+    if (k == 0 && threadIdx.x == 0) { *rm.wl_count = 0; *rm.wl2_count = 0; }       // the scan of this generation is done
+    if (!rm.active[k]) { if (threadIdx.x == 0) frozen_row(rm, k, g); return; }
+    gen_finish<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused persistent generation kernel: one CTA owns one run for n_gens generations (S3-S7 without leaving the
+// SM).  Per generation: operator + snap + validity + Hamming-1 probe by the P individual threads; the few
+// candidates still unresolved are repaired by the WHOLE block (Hamming-2/3 pair-table probe, then a
+// brute-force scan of the table in batches of GEN_NB candidates); then evaluation, selection and the trajectory
+// row.  The run's state stays in global memory but is private to the CTA, so it lives in L1/L2 between
+// generations; __syncthreads() orders the phases.
+#define GEN_NB 4
+template <int ALGO, int ROWW>
+__global__ void __launch_bounds__(1024) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
+                                              const __grid_constant__ RunsMeta rm, uint32_t g_first, uint32_t n_gens,
+                                              uint32_t scratch_words) {
+    extern __shared__ uint32_t s_dyn[];
+    __shared__ RunShared sh;
+    __shared__ uint32_t s_nwl;
+    __shared__ uint32_t s_cw[GEN_NB * ROWW];
+    __shared__ unsigned long long s_key[GEN_NB];
+    uint32_t* s_wl = s_dyn + scratch_words;                             // P slots
+    const uint32_t k = blockIdx.x, tid = threadIdx.x;
+    for (uint32_t g = g_first + 1; g <= g_first + n_gens; ++g) {
+        __syncthreads();
+        const bool active = rm.budget == 0 || rm.uniq[k] < rm.budget;   // O10
+        if (tid == 0) { rm.active[k] = active ? 1 : 0; s_nwl = 0; }
+        if (!active) { if (tid == 0) frozen_row(rm, k, g); continue; }
+        __syncthreads();
+        gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, s_wl, &s_nwl, false);
+        __syncthreads();
+        const uint32_t nwl = s_nwl;
+        uint32_t nscan = 0;
+        if (pm.levels >= 2) {
+            for (uint32_t f = 0; f < nwl; ++f) {
+                const uint32_t slot = s_wl[f];
+                __syncthreads();
+                if (tid < ROWW) s_cw[tid] = ((const uint32_t*)(rm.cand + (uint64_t)slot * (ROWW * 4)))[tid];
+                if (tid == 0) s_key[0] = ~0ull;
+                __syncthreads();
+                const int found = probe23_cta<ROWW>(sm, pm, s_cw, &s_key[0]);
+                if (tid == 0) {
+                    const uint64_t best = s_key[0];
+                    if (found) rm.key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
+                    else s_wl[nscan] = slot;                            // nscan <= f: compacts in place
+                }
+                if (!found) ++nscan;
+            }
+        } else {
+            nscan = nwl;
+        }
+        for (uint32_t f0 = 0; f0 < nscan; f0 += GEN_NB) {
+            const uint32_t nb = min((uint32_t)GEN_NB, nscan - f0);
+            __syncthreads();
+            if (tid < nb * ROWW) s_cw[tid] = ((const uint32_t*)(rm.cand + (uint64_t)s_wl[f0 + tid / ROWW] * (ROWW * 4)))[tid % ROWW];
+            if (tid < GEN_NB) s_key[tid] = ~0ull;
+            __syncthreads();
+            scan_cta<ROWW, GEN_NB>(sm, s_cw, (int)nb, s_key);
+            if (tid < nb) rm.key[s_wl[f0 + tid]] = s_key[tid];
+        }
+        if (tid == 0 && nscan) atomicAdd(&rm.counters[1], (unsigned long long)nscan);
+        __syncthreads();
+        gen_finish<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh);
     }
 }

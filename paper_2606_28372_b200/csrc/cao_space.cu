@@ -88,7 +88,7 @@ int cao_profile_read(int32_t cls, double* ms_total, uint64_t* launches) {
 }
 const char* cao_profile_name(int32_t cls) {
     static const char* names[PK_N] = {"k_build_table", "k_enum_pass1", "k_scan_reduce+partials+apply", "k_fill", "k_init",
-                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish", "k_probe23"};
+                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish", "k_probe23", "k_gen"};
     return cls >= 0 && cls < PK_N ? names[cls] : "";
 }
 
@@ -160,6 +160,7 @@ static int plan_space(cao_space* s) {
     s->n_words = (M.N + 63) / 64; s->nd = (M.N + 511) / 512;
     int64_t nb = (int64_t)(40960 / ((uint64_t)s->Wb * 8)) - 1;
     s->nb = (uint32_t)std::min<int64_t>(256, std::max<int64_t>(1, nb));
+    s->nb_tabled = s->nb;
     // per-constraint plan
     s->plan.assign(s->cons.size(), ConsPlan());
     uint64_t total_words = 0;
@@ -191,6 +192,8 @@ static int plan_space(cao_space* s) {
     for (size_t c = 0; c < s->cons.size(); ++c) (s->plan[c].tabled ? tab : res).push_back((int)c);
     std::stable_sort(tab.begin(), tab.end(), [&](int a, int b) { return s->plan[a].rows < s->plan[b].rows; });
     s->n_tab = (int)tab.size(); s->n_res = (int)res.size();
+    // residual constraints are evaluated by one warp per block: fewer blocks per CTA keep the CTAs balanced
+    if (s->n_res) s->nb = std::min<uint32_t>(s->nb, 32);
     std::vector<int32_t>& D = s->desc;
     D.assign(tab.size() + res.size() + s->cons.size(), 0);       // [tab offs][res offs][program offs of every constraint]
     // programs first, so that the tabled descriptors can point at them

@@ -70,15 +70,20 @@ def run_pair(cfg, algo, R, P, gens, budget=0, seed=0, first_run=0, step_sizes=No
     g = gpu_space(cfg, os_, sp, objective)
     kw = dict(n_runs=R, pop=P, budget=budget, max_gens=gens, seed=seed, first_run=first_run)
     orr = O.OracleRuns(os_, algo, hparams=hp, **kw)
-    gr = cao.Runs(g, algo, hparams=None if hp is None else cao.HParams(*[getattr(hp, f[0]) for f in hp._fields_]), **kw)
-    compare(gr, orr, sp.n)
+    ghp = None if hp is None else cao.HParams(*[getattr(hp, f[0]) for f in hp._fields_])
+    grs = [cao.Runs(g, algo, hparams=ghp, mode=m, **kw) for m in ("fused", "phased")]   # both execution modes
+    for gr in grs:
+        compare(gr, orr, sp.n)
     done = 0
     for k in (step_sizes or [1] * gens):
         k = min(k, gens - done)
         if k <= 0:
             break
-        gr.step(k); orr.step(k); done += k
-        compare(gr, orr, sp.n)
+        orr.step(k); done += k
+        for gr in grs:
+            gr.step(k)
+            compare(gr, orr, sp.n)
+    gr = grs[0]
     return gr, orr
 
 
@@ -173,10 +178,13 @@ def test_forced_probe_levels_give_identical_runs(levels):
     g.set_objective(os_._obj)
     for algo in ["de", "pso", "firefly", "ga"]:
         kw = dict(n_runs=30, pop=20, budget=0, max_gens=12, seed=3)
-        orr = O.OracleRuns(os_, algo, **kw); gr = cao.Runs(g, algo, **kw)
+        orr = O.OracleRuns(os_, algo, **kw)
+        grs = [cao.Runs(g, algo, mode=m, **kw) for m in ("fused", "phased")]
         for _ in range(4):
-            gr.step(3); orr.step(3)
-            compare(gr, orr, sp.n)
+            orr.step(3)
+            for gr in grs:
+                gr.step(3)
+                compare(gr, orr, sp.n)
 
 
 def test_auto_probe_levels():

@@ -191,7 +191,7 @@ def test_rebuild_reproduces_the_space(cfg):
     """cao_space_rebuild: all of S1 again, asynchronously, into the same (wiped) buffers."""
     sp, os_ = oracle_space(cfg, with_objective=False)
     gs = _gpu_space(sp)
-    gs._bitmap.zero_(); gs._table.zero_()
+    gs._bitmap.zero_(); gs.rows().zero_(); gs.Ltab().zero_(); gs.rank_dir().zero_()
     gs.rebuild()
     torch.cuda.synchronize()
     _check_space(sp, os_, gs)
