@@ -124,12 +124,21 @@ __device__ __forceinline__ int de_mutate_index(float F, int ibest, int ia, int i
 __device__ __forceinline__ bool bit_test(const uint64_t* __restrict__ bitmap, uint64_t L) {
     return (__ldg(&bitmap[L >> 6]) >> (L & 63)) & 1ull;
 }
-// rank of a VALID L: directory entry of its 512-block + popcount of the bits below it in the block.
+// rank of a VALID L: directory entry of its 512-block + popcount of the bits below it in the block.  The eight
+// words of the block (one 64-byte line; the bitmap buffer is padded to 256 bytes) are loaded unconditionally
+// as four 128-bit loads, so the rank costs one round trip instead of a dependent chain.
 __device__ __forceinline__ uint32_t rank_of(const SpaceMeta& sm, uint64_t L) {
-    uint64_t w = L >> 6, w0 = w & ~7ull;
+    const uint32_t wi = (uint32_t)(L >> 6) & 7u;
+    const ulonglong2* blk = (const ulonglong2*)(sm.bitmap + ((L >> 6) & ~7ull));
     uint32_t r = __ldg(&sm.dir[L >> CAO_DIR_SHIFT]);
-    for (uint64_t q = w0; q < w; ++q) r += __popcll(__ldg(&sm.bitmap[q]));
-    r += __popcll(__ldg(&sm.bitmap[w]) & ((1ull << (L & 63)) - 1ull));
+    const uint64_t below_mask = (1ull << (L & 63)) - 1ull;
+#pragma unroll
+    for (int h = 0; h < 4; ++h) {
+        const ulonglong2 v = __ldg(&blk[h]);
+        const uint32_t q0 = 2 * h, q1 = 2 * h + 1;
+        r += q0 < wi ? __popcll(v.x) : q0 == wi ? __popcll(v.x & below_mask) : 0;
+        r += q1 < wi ? __popcll(v.y) : q1 == wi ? __popcll(v.y & below_mask) : 0;
+    }
     return r;
 }
 

@@ -15,16 +15,22 @@
 template <int ROWW>
 __device__ __forceinline__ uint64_t probe_h1(const SpaceMeta& sm, const uint32_t (&w)[ROWW], uint64_t L) {
     for (int delta = 1; delta < sm.M; ++delta) {
-        uint64_t bestL = ~0ull;
+        // all bit tests of one |delta| level are independent loads (no short-circuit), so they overlap in flight
+        uint64_t cand[ROWW * 8];
+        bool hit[ROWW * 8];
 #pragma unroll
         for (int d = 0; d < ROWW * 4; ++d) {
-            if (d < sm.n) {
-                int c = (int)((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu);
-                uint64_t step = (uint64_t)delta * sm.stride[d];
-                if (c >= delta) { uint64_t L2 = L - step; if (L2 < bestL && bit_test(sm.bitmap, L2)) bestL = L2; }
-                if (c + delta < (int)sm.m[d]) { uint64_t L2 = L + step; if (L2 < bestL && bit_test(sm.bitmap, L2)) bestL = L2; }
-            }
+            const int c = (int)((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu);
+            const uint64_t step = d < sm.n ? (uint64_t)delta * sm.stride[d] : 0;
+            const bool okm = d < sm.n && c >= delta, okp = d < sm.n && c + delta < (int)sm.m[d];
+            cand[2 * d] = okm ? L - step : L;  cand[2 * d + 1] = okp ? L + step : L;
+            hit[2 * d] = okm;                  hit[2 * d + 1] = okp;
         }
+#pragma unroll
+        for (int e = 0; e < ROWW * 8; ++e) hit[e] = hit[e] && bit_test(sm.bitmap, cand[e]);
+        uint64_t bestL = ~0ull;
+#pragma unroll
+        for (int e = 0; e < ROWW * 8; ++e) if (hit[e] && cand[e] < bestL) bestL = cand[e];
         if (bestL != ~0ull) return make_key(1u, (uint32_t)delta, rank_of(sm, bestL));
     }
     return CAO_KEY_NONE;
@@ -87,12 +93,13 @@ __device__ __forceinline__ int probe23_cta(const SpaceMeta& sm, const ProbeMeta&
             if (level == 2) {
                 if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)s2 << 40) | L2; best = k < best ? k : best; }
             } else {
-#pragma unroll 4
+#pragma unroll 8
                 for (uint32_t t3 = pm.dim_first[d2 + 1]; t3 < T; ++t3) {
                     const uint32_t e3 = __ldg(&pm.tgt[t3]), d3 = e3 >> 8;
                     const int dv3 = (int)(e3 & 255) - (int)c[d3];
                     const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
-                    if (dv3 != 0 && bit_test(sm.bitmap, L3)) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
+                    const bool bit3 = bit_test(sm.bitmap, L3);              // unconditional: dv3 == 0 re-reads L2 (a legal index)
+                    if (dv3 != 0 && bit3) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
                 }
             }
         }
@@ -117,20 +124,30 @@ __device__ __forceinline__ void scan_cta(const SpaceMeta& sm, const uint32_t* s_
     uint64_t best[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) best[b] = ~0ull;
-    for (uint32_t r = threadIdx.x; r < sm.V; r += blockDim.x) {
-        uint32_t v[ROWW];
-        load_row<ROWW>(sm.rows + (uint64_t)r * (ROWW * 4), v);
+    constexpr int RU = ROWW == 4 ? 8 : 4;                              // rows in flight per thread (128 bytes of loads)
+    for (uint32_t r0 = threadIdx.x; r0 < sm.V; r0 += RU * blockDim.x) {
+        uint32_t v[RU][ROWW];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            uint32_t sad = 0, ham = 0;
+        for (int u = 0; u < RU; ++u) {
+            const uint32_t r = r0 + u * blockDim.x;
+            load_row<ROWW>(sm.rows + (uint64_t)(r < sm.V ? r : r0) * (ROWW * 4), v[u]);    // clamped: never out of the table
+        }
 #pragma unroll
-            for (int k = 0; k < ROWW; ++k) {
-                sad = sad4_acc(c[b][k], v[k], sad);
-                const uint32_t x = c[b][k] ^ v[k];
-                ham += __popc((((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x) & 0x80808080u);
+        for (int u = 0; u < RU; ++u) {
+            const uint32_t r = r0 + u * blockDim.x;
+            if (r >= sm.V) break;
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                uint32_t sad = 0, ham = 0;
+#pragma unroll
+                for (int k = 0; k < ROWW; ++k) {
+                    sad = sad4_acc(c[b][k], v[u][k], sad);
+                    const uint32_t x = c[b][k] ^ v[u][k];
+                    ham += __popc((((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x) & 0x80808080u);
+                }
+                const uint64_t key = ((uint64_t)((ham << 13) + sad) << 32) | r;
+                best[b] = key < best[b] ? key : best[b];
             }
-            const uint64_t key = ((uint64_t)((ham << 13) + sad) << 32) | r;
-            best[b] = key < best[b] ? key : best[b];
         }
     }
 #pragma unroll

@@ -123,7 +123,7 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
 // ---------------------------------------------------------------------------------------------
 struct RunsLayout {
     uint64_t cand, key, valid, rep_rank, eval_rank, tap_f, accept, active, idx, rank, f, x, v, pb, pbf, dedup,
-        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl2, wl_count, counters, total;
+        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl2, wl_count, counters, rcache, total;
     uint64_t zero_from, zero_bytes;       // region that must start as zero: dedup .. stagn
     uint32_t dedup_words;
 };
@@ -150,6 +150,7 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
     L.traj = take((max_gens + 1) * R * 12);
     L.wl = take(RP * 4);
     L.wl2 = take(RP * 4);
+    L.rcache = take(R * CAO_RCACHE * 16);
     L.total = off;
     return L;
 }
@@ -204,6 +205,7 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     m.traj = (uint32_t*)(w + L.traj); m.wl = (uint32_t*)(w + L.wl); m.wl_count = (uint32_t*)(w + L.wl_count);
     m.wl2 = (uint32_t*)(w + L.wl2); m.wl2_count = m.wl_count + 1;
     m.counters = (unsigned long long*)(w + L.counters);
+    m.rcache = (ulonglong2*)(w + L.rcache);
     const uint64_t RP = (uint64_t)n_runs * pop;
     r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
     r->block = (unsigned)((pop + 31) / 32 * 32);
@@ -217,6 +219,8 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.zero_from, 0, L.zero_bytes, st), "memset state"))) break;
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.best_rank, 0xFF, (uint64_t)n_runs * 4, st), "memset best_rank"))) break;
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.cand, 0, L.idx - L.cand, st), "memset taps"))) break;
+        if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.key, 0xFF, RP * 8, st), "memset keys"))) break;   // no key yet
+        if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.rcache, 0xFF, (uint64_t)n_runs * CAO_RCACHE * 16, st), "memset repair cache"))) break;
 #define CALL_INIT(A, W) \
         if (r->smem_op > 48 * 1024) cudaFuncSetAttribute(k_op<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
         k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
@@ -241,8 +245,13 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
         const uint32_t scratch_words = (uint32_t)((std::max(r->smem_op, r->smem_fin) + 3) / 4);
         const size_t smem = (size_t)scratch_words * 4 + (size_t)r->rm.P * 4;
 #define CALL_GEN(A, W) \
-        if (smem > 48 * 1024) cudaFuncSetAttribute(k_gen<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-        k_gen<A, W><<<r->rm.R, r->block_fused, smem, st>>>(r->sm, r->s->probe, r->rm, r->gen, ng, scratch_words)
+        if (r->block_fused <= 256) { \
+            if (smem > 48 * 1024) cudaFuncSetAttribute(k_gen<A, W, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            k_gen<A, W, 256><<<r->rm.R, r->block_fused, smem, st>>>(r->sm, r->s->probe, r->rm, r->gen, ng, scratch_words); \
+        } else { \
+            if (smem > 48 * 1024) cudaFuncSetAttribute(k_gen<A, W, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            k_gen<A, W, 1024><<<r->rm.R, r->block_fused, smem, st>>>(r->sm, r->s->probe, r->rm, r->gen, ng, scratch_words); \
+        }
         { ProfScope ps(PK_GEN, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_GEN); }
         CAO_LAUNCHED("k_gen");
         r->gen += ng;

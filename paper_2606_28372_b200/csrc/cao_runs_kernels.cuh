@@ -11,6 +11,9 @@
 #include "cao_host.h"
 #include "cao_repair_kernels.cuh"
 
+#define CAO_RCACHE 256                                  // direct-mapped entries per run
+__device__ __forceinline__ uint32_t rcache_slot(uint64_t L) { return (uint32_t)((L * 0x9E3779B97F4A7C15ull) >> 56); }
+
 struct RunsMeta {
     uint32_t R, first_run, P, budget, max_gens, dedup_words;
     int32_t algo, probe_levels;
@@ -26,6 +29,7 @@ struct RunsMeta {
     uint32_t* traj;                                    // [gen][run]{f32 bits, rank, uniq}
     uint32_t* wl; uint32_t* wl_count;                  // candidates without a valid Hamming-1 neighbour
     uint32_t* wl2; uint32_t* wl2_count;                // ... and none up to the probed level: table scan
+    ulonglong2* rcache;                                // [run][CAO_RCACHE] {L, key}: repairs at Hamming >= 2 already resolved (fused mode)
     unsigned long long* counters;                      // n_repaired, n_scanned, n_evaluated
 };
 
@@ -33,7 +37,7 @@ struct RunsMeta {
 struct RunShared {
     unsigned long long best;                           // (f bits << 32 | rank) of the best-so-far
     unsigned long long aux;                            // PSO: (pbest_f bits << 32 | i) of gbest
-    uint32_t n_new, flag;
+    uint32_t n_new, flag, n_inv;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -135,13 +139,31 @@ __global__ void __launch_bounds__(1024) k_init(const __grid_constant__ SpaceMeta
 // S4 + first half of S5 for the candidate held in w: store, validity, probe, worklist.
 template <int ROWW>
 __device__ __forceinline__ void candidate_tail(const SpaceMeta& sm, const RunsMeta& rm, uint64_t slot, const uint32_t (&w)[ROWW],
-                                               uint32_t* wl, uint32_t* wl_count, bool count_scans) {
-    store_row<ROWW>(rm.cand + slot * (ROWW * 4), w);
+                                               uint32_t* wl, uint32_t* wl_count, bool count_scans, RunShared& sh, bool use_cache) {
+    // Repair is a pure function of the row: if this individual produced the same post-snap row in the generation
+    // before (a particle that stopped moving, a repeated trial), last generation's key is still in the taps.
+    uint32_t prev[ROWW];
+    load_row_rw<ROWW>(rm.cand + slot * (ROWW * 4), prev);
+    const uint64_t prev_key = rm.key[slot];
+    bool same = prev_key != CAO_KEY_NONE;
+#pragma unroll
+    for (int z = 0; z < ROWW; ++z) same = same && prev[z] == w[z];
     bool valid;
-    uint64_t key = validate_probe<ROWW>(sm, w, rm.probe_levels >= 1, valid);
+    uint64_t key;
+    if (same) {
+        key = prev_key; valid = (key >> 45) == 0;
+    } else {
+        store_row<ROWW>(rm.cand + slot * (ROWW * 4), w);
+        key = validate_probe<ROWW>(sm, w, rm.probe_levels >= 1, valid);
+        if (key == CAO_KEY_NONE && use_cache) {                         // memoised repair of this run (L268 in spirit): exact,
+            const uint64_t L = row_lin<ROWW>(sm, w);                    // repair(c) depends on c only
+            const ulonglong2 e = rm.rcache[(slot / rm.P) * CAO_RCACHE + rcache_slot(L)];
+            if (e.x == L) key = e.y;
+        }
+        rm.key[slot] = key;
+    }
     rm.valid[slot] = valid ? 1 : 0;
-    rm.key[slot] = key;
-    if (!valid) atomicAdd(&rm.counters[0], 1ull);
+    if (!valid) atomicAdd(&sh.n_inv, 1u);                               // flushed once per run and generation
     if (key == CAO_KEY_NONE) {
         worklist_push(wl, wl_count, (uint32_t)slot);
         if (count_scans) atomicAdd(&rm.counters[1], 1ull);               // straight to the scan
@@ -153,7 +175,7 @@ __device__ __forceinline__ void candidate_tail(const SpaceMeta& sm, const RunsMe
 // S3 + S4 for an ACTIVE run k (block-uniform call, contains barriers).  Unresolved candidates go to (wl, wl_count).
 template <int ALGO, int ROWW>
 __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, uint32_t k, uint32_t g, uint32_t* s_dyn,
-                                       RunShared& sh, uint32_t* wl, uint32_t* wl_count, bool count_scans) {
+                                       RunShared& sh, uint32_t* wl, uint32_t* wl_count, bool count_scans, bool use_cache) {
     const uint32_t i = threadIdx.x, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
     const uint64_t q = (uint64_t)k * P + i;
@@ -161,6 +183,8 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
 #pragma unroll
     for (int z = 0; z < ROWW; ++z) w[z] = 0;
     Draws dr(rm.seed, run, g, i, S_OP);
+    if (i == 0) sh.n_inv = 0;
+    __syncthreads();
 
     if (ALGO == CAO_DE) {                                               // O5: best1bin on indices
         if (i < P) {
@@ -264,12 +288,25 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
                 for (int d = 0; d < ROWW * 4; ++d)
                     if (d < n) { float df = __fsub_rn(xj[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
                 float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
+                // the n noise draws of this j are slots j*n .. j*n+n-1: all their Philox blocks are computed up
+                // front as independent chains, then word (o + d) is picked with selects (o = first slot & 3)
+                const uint32_t s0 = j * (uint32_t)n, b0 = s0 >> 2, o = s0 & 3;
+                uint32_t nw[(ROWW + 1) * 4];
+#pragma unroll
+                for (int qb = 0; qb < ROWW + 1; ++qb) {
+                    uint4 rr = make_uint4(0, 0, 0, 0);
+                    if ((uint32_t)(qb * 4) < o + (uint32_t)n)
+                        rr = philox4x32_10(make_uint4(run, g, i, (S_OP << 24) | (b0 + qb)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
+                    nw[qb * 4] = rr.x; nw[qb * 4 + 1] = rr.y; nw[qb * 4 + 2] = rr.z; nw[qb * 4 + 3] = rr.w;
+                }
 #pragma unroll
                 for (int d = 0; d < ROWW * 4; ++d) {
                     if (d < n) {
+                        const uint32_t lo = (o & 1) ? nw[d + 1] : nw[d], hi = (o & 1) ? nw[d + 3] : nw[d + 2];
+                        const uint32_t word = (o & 2) ? hi : lo;
                         float df = __fsub_rn(xj[d], xi[d]);
                         xi[d] = __fadd_rn(xi[d], __fmul_rn(beta, df));
-                        float e = __fsub_rn(u01(dr(j * (uint32_t)n + d)), 0.5f);
+                        float e = __fsub_rn(u01(word), 0.5f);
                         xi[d] = __fadd_rn(xi[d], __fmul_rn(rm.hp.ff_alpha, e));
                     }
                 }
@@ -284,7 +321,9 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
             }
         }
     }
-    if (i < P) candidate_tail<ROWW>(sm, rm, q, w, wl, wl_count, count_scans);
+    if (i < P) candidate_tail<ROWW>(sm, rm, q, w, wl, wl_count, count_scans, sh, use_cache);
+    __syncthreads();
+    if (i == 0 && sh.n_inv) atomicAdd(&rm.counters[0], (unsigned long long)sh.n_inv);
 }
 
 template <int ALGO, int ROWW>
@@ -295,7 +334,7 @@ __global__ void __launch_bounds__(1024) k_op(const __grid_constant__ SpaceMeta s
     const bool active = rm.budget == 0 || rm.uniq[k] < rm.budget;       // O10 (g <= max_gens is enforced by the host)
     if (threadIdx.x == 0) rm.active[k] = active ? 1 : 0;
     if (!active) return;
-    gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, rm.wl, rm.wl_count, rm.probe_levels < 2);
+    gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, rm.wl, rm.wl_count, rm.probe_levels < 2, false);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -428,8 +467,8 @@ __global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMe
 // row.  The run's state stays in global memory but is private to the CTA, so it lives in L1/L2 between
 // generations; __syncthreads() orders the phases.
 #define GEN_NB 4
-template <int ALGO, int ROWW>
-__global__ void __launch_bounds__(1024) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
+template <int ALGO, int ROWW, int MAXT>
+__global__ void __launch_bounds__(MAXT) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
                                               const __grid_constant__ RunsMeta rm, uint32_t g_first, uint32_t n_gens,
                                               uint32_t scratch_words) {
     extern __shared__ uint32_t s_dyn[];
@@ -445,7 +484,7 @@ __global__ void __launch_bounds__(1024) k_gen(const __grid_constant__ SpaceMeta 
         if (tid == 0) { rm.active[k] = active ? 1 : 0; s_nwl = 0; }
         if (!active) { if (tid == 0) frozen_row(rm, k, g); continue; }
         __syncthreads();
-        gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, s_wl, &s_nwl, false);
+        gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, s_wl, &s_nwl, false, true);
         __syncthreads();
         const uint32_t nwl = s_nwl;
         uint32_t nscan = 0;
@@ -459,8 +498,15 @@ __global__ void __launch_bounds__(1024) k_gen(const __grid_constant__ SpaceMeta 
                 const int found = probe23_cta<ROWW>(sm, pm, s_cw, &s_key[0]);
                 if (tid == 0) {
                     const uint64_t best = s_key[0];
-                    if (found) rm.key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
-                    else s_wl[nscan] = slot;                            // nscan <= f: compacts in place
+                    if (found) {
+                        const uint64_t key = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
+                        rm.key[slot] = key;
+                        uint64_t L = 0;
+                        for (int d = 0; d < sm.n; ++d) L += (uint64_t)((const uint8_t*)s_cw)[d] * sm.stride[d];
+                        rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)] = make_ulonglong2(L, key);
+                    } else {
+                        s_wl[nscan] = slot;                             // nscan <= f: compacts in place
+                    }
                 }
                 if (!found) ++nscan;
             }
@@ -473,8 +519,14 @@ __global__ void __launch_bounds__(1024) k_gen(const __grid_constant__ SpaceMeta 
             if (tid < nb * ROWW) s_cw[tid] = ((const uint32_t*)(rm.cand + (uint64_t)s_wl[f0 + tid / ROWW] * (ROWW * 4)))[tid % ROWW];
             if (tid < GEN_NB) s_key[tid] = ~0ull;
             __syncthreads();
-            scan_cta<ROWW, GEN_NB>(sm, s_cw, (int)nb, s_key);
-            if (tid < nb) rm.key[s_wl[f0 + tid]] = s_key[tid];
+            if (nb == 1) scan_cta<ROWW, 1>(sm, s_cw, 1, s_key);
+            else scan_cta<ROWW, GEN_NB>(sm, s_cw, (int)nb, s_key);
+            if (tid < nb) {
+                rm.key[s_wl[f0 + tid]] = s_key[tid];
+                uint64_t L = 0;
+                for (int d = 0; d < sm.n; ++d) L += (uint64_t)((const uint8_t*)(s_cw + tid * ROWW))[d] * sm.stride[d];
+                rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)] = make_ulonglong2(L, s_key[tid]);   // same slot twice: either entry is exact
+            }
         }
         if (tid == 0 && nscan) atomicAdd(&rm.counters[1], (unsigned long long)nscan);
         __syncthreads();
