@@ -166,7 +166,9 @@ def gpu_arm(args):
     pk = peaks()
     wl = workload(args.config, args.runs)
     sp, R, P, G = wl["space"], wl["runs"], wl["pop"], wl["gens"]
-    first_run = rank * R
+    from paper_2606_28372_b200.shard import shard_runs, max_over_ranks
+    first_run, _n_local = shard_runs(world * R, world, rank)         # weak scaling: R runs per rank, global run indices
+    assert _n_local == R
 
     # inputs resident in HBM before the timed region: the objective table (indexed by valid rank, so it is
     # derived once from a first build of the same space) on the device and in pinned host memory
@@ -235,10 +237,7 @@ def gpu_arm(args):
         if profile:
             cao.profile_enable(False)
         launches = cao.launch_count() - l0
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(ms, dev)
         return ms, wall, prof, launches, kept
 
     for _ in range(args.warmup):
@@ -288,7 +287,8 @@ def gpu_arm(args):
                 "peak_source": pk["source"], "traffic": None}
     else:
         # k_op / k_finish / k_init: sector-granular bytes per candidate: state + bitmap + dir + obj + dedup
-        per = {"k_op": 2 * rb + 8 + 32 + 32, "k_finish": 8 + 32 + 64 + rb + 24, "k_init": 32 + 64 + rb + 8}.get(top, 64)
+        per = {"k_op": 2 * rb + 8 + 32 + 32, "k_finish": 8 + 32 + 64 + rb + 24, "k_init": 32 + 64 + rb + 8,
+               "k_gen": 2 * (rb + 8) + 32 + 32 + 32 + 64}.get(top, 64)
         by = per * cands_step / max(top_n, 1)
         roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                 "peak_source": pk["source"], "traffic": None}
@@ -325,6 +325,27 @@ def gpu_arm(args):
                              "algorithmic_bytes": enum_bytes(Nx, Vx, rbx), "kernel_us": kp}
         del gx
 
+    # ---- BASELINE configs[4]: candidates/s against the number of runs (same space, no budget, 200 generations)
+    sweep = {}
+    if not args.no_sweep:
+        space4 = cao.Space.from_space(sp).build(); space4.set_objective(obj_d)
+        for Rs in [100, 1000, 10000, 100000][:args.sweep_points]:
+            row = {}
+            for algo in wl["algos"]:
+                best_ms, cands = None, 0
+                for _ in range(2):
+                    r4 = cao.Runs(space4, algo, n_runs=Rs, pop=P, budget=0, max_gens=200, seed=wl["seed"])
+                    torch.cuda.synchronize(); flush.zero_()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(); r4.step(200); e1.record(); e1.synchronize()
+                    t4 = e0.elapsed_time(e1); best_ms = t4 if best_ms is None else min(best_ms, t4)
+                    cands = Rs * P * 200
+                    del r4
+                row[algo] = {"ms": best_ms, "candidates_per_s": cands / (best_ms / 1e3),
+                             "hbm_frac_204B": cands * 204 / (best_ms / 1e3) / 1e9 / pk["hbm_gbs"]}
+            sweep[str(Rs)] = row
+        del space4
+
     # ---- CPU oracle on a bounded sample of the same workload (rank 0, N=1 only)
     cpu = None
     if world == 1 and not args.no_cpu:
@@ -350,7 +371,7 @@ def gpu_arm(args):
         "cpu_baseline": cpu,
         "extra": {"candidates_per_step": int(cands_step), "invalid_post_snap_per_step": int(repaired_step),
                   "scanned_per_step": int(scanned_step), "generations_done_sum": gens_done,
-                  "kernels": kern, "enumeration": enum, "wall_s_timed_region": wall, "peaks": pk},
+                  "kernels": kern, "enumeration": enum, "sweep_cfg4": sweep, "wall_s_timed_region": wall, "peaks": pk},
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -369,6 +390,8 @@ def main():
     ap.add_argument("--streams", type=int, default=4, help="1 = all algorithms on one stream, >1 = one stream per algorithm")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-enum", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--sweep-points", type=int, default=4, help="how many of the run counts 1e2, 1e3, 1e4, 1e5 to sweep")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_arm(args)

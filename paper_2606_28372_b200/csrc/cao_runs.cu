@@ -209,7 +209,9 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     const uint64_t RP = (uint64_t)n_runs * pop;
     r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
     r->block = (unsigned)((pop + 31) / 32 * 32);
-    r->block_fused = std::max(r->block, 128u);
+    // fused CTAs: 128 threads help the block-cooperative repairs while all runs fit one wave (148 SMs x 8 CTAs of
+    // <= 64 registers x 128 threads); beyond that, one warp per run keeps 32 runs resident per SM
+    r->block_fused = n_runs <= 148u * 8u ? std::max(r->block, 128u) : r->block;
     const size_t P = (size_t)pop, n = (size_t)s->meta.n;
     r->smem_init = P * 4;
     r->smem_op = algo == CAO_GA ? P * 12 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
