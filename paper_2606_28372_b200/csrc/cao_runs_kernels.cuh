@@ -468,7 +468,7 @@ __global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMe
 // generations; __syncthreads() orders the phases.
 #define GEN_NB 4
 template <int ALGO, int ROWW, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1024 / MAXT) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
+__global__ void __launch_bounds__(MAXT) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
                                               const __grid_constant__ RunsMeta rm, uint32_t g_first, uint32_t n_gens,
                                               uint32_t scratch_words) {
     extern __shared__ uint32_t s_dyn[];
