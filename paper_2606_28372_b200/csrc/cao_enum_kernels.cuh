@@ -8,36 +8,61 @@
 #pragma once
 #include "cao_host.h"
 
-// All constraint tables in one launch: blockIdx.y = tabled constraint, one thread per (row, inner pattern);
-// a warp ballot assembles 32 patterns into one half word of the row.
-// Tabled descriptor: {toff_lo, toff_hi, n_outer, (digit, cstride) x n_outer, prog_off, prog_len, rows}.
+// All constraint tables in one launch: blockIdx.y = tabled constraint; a CTA takes groups of RPC rows.
+// Phase A: one thread per (row, combination of the INNER scope digits) interprets the program (the inner pattern
+// of a row depends on those digits only); results go to shared memory.  Phase B: one thread per (row, inner
+// pattern) looks its combination up and a warp ballot assembles 32 patterns into one half word of the row.
+// Tabled descriptor: {toff_lo, toff_hi, n_outer, (digit, cstride) x n_outer, prog_off, prog_len, rows,
+//                     n_inner, Ci, (digit, istride) x n_inner}.
 __global__ void __launch_bounds__(256) k_build_tables(const __grid_constant__ SpaceMeta sm, const int64_t* __restrict__ dom,
                                                       const int32_t* __restrict__ desc, uint64_t* tables, uint64_t B,
                                                       uint32_t Wb, int32_t t) {
+    extern __shared__ uint8_t s_ev[];                                   // RPC x Ci results
     const int32_t* ds = desc + desc[blockIdx.y];
     const uint64_t toff = (uint32_t)ds[0] | ((uint64_t)(uint32_t)ds[1] << 32);
     const int no = ds[2];
     const int32_t* prog = desc + ds[3 + 2 * no];
     const int nw = ds[4 + 2 * no];
-    const uint64_t rows = (uint32_t)ds[5 + 2 * no];
-    const uint64_t per_row = (uint64_t)Wb * 64, total = rows * per_row;
+    const uint32_t rows = (uint32_t)ds[5 + 2 * no];
+    const int ni = ds[6 + 2 * no];
+    const uint32_t Ci = (uint32_t)ds[7 + 2 * no];
+    const int32_t* din = ds + 8 + 2 * no;
+    const uint32_t per_row = Wb * 64;
+    // rows per CTA pass: at most 256 program runs (phase A) and 2048 patterns (phase B, 8 per thread)
+    const uint32_t RPC = max(1u, min(Ci >= 256 ? 1u : 256u / Ci, 2048u / per_row));
     uint32_t* out32 = (uint32_t*)(tables + toff);
-    for (uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; gid < total; gid += (uint64_t)gridDim.x * blockDim.x) {
-        const uint64_t row = gid / per_row, p = gid - row * per_row;          // per_row is a multiple of 64: a warp stays in one row
-        int ok = 0;
-        if (p < B) {
+    for (uint32_t row0 = blockIdx.x * RPC; row0 < rows; row0 += gridDim.x * RPC) {
+        const uint32_t nr = min(RPC, rows - row0);
+        __syncthreads();
+        for (uint32_t e = threadIdx.x; e < nr * Ci; e += blockDim.x) {  // phase A
+            const uint32_t rr = e / Ci, c = e - rr * Ci, row = row0 + rr;
             int64_t x[CAO_MAX_DIMS];
             for (int d = 0; d < sm.n; ++d) x[d] = dom[d * 256];
             for (int k = 0; k < no; ++k) {
                 const int d = ds[3 + 2 * k];
-                x[d] = dom[d * 256 + (uint32_t)((row / (uint32_t)ds[4 + 2 * k]) % sm.m[d])];
+                x[d] = dom[d * 256 + (row / (uint32_t)ds[4 + 2 * k]) % sm.m[d]];
             }
-            uint64_t q = p;
-            for (int d = sm.n - 1; d >= t; --d) { const uint32_t m = sm.m[d]; x[d] = dom[d * 256 + (uint32_t)(q % m)]; q /= m; }
-            ok = eval_program(prog, nw, x);
+            for (int k = 0; k < ni; ++k) {
+                const int d = din[2 * k];
+                x[d] = dom[d * 256 + (c / (uint32_t)din[2 * k + 1]) % sm.m[d]];
+            }
+            s_ev[e] = (uint8_t)eval_program(prog, nw, x);
         }
-        const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
-        if ((threadIdx.x & 31) == 0) out32[gid >> 5] = word;
+        __syncthreads();
+        for (uint32_t e = threadIdx.x; e < nr * per_row; e += blockDim.x) {     // phase B; per_row is a multiple of 64
+            const uint32_t rr = e / per_row, p = e - rr * per_row;
+            int ok = 0;
+            if (p < B) {
+                uint32_t q = p, c = 0;
+                for (int d = sm.n - 1; d >= t; --d) {                   // inner digits of p, least significant first
+                    const uint32_t m = sm.m[d], idx = q % m; q /= m;
+                    for (int k = 0; k < ni; ++k) if (din[2 * k] == d) c += idx * (uint32_t)din[2 * k + 1];
+                }
+                ok = s_ev[rr * Ci + c];
+            }
+            const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
+            if ((threadIdx.x & 31) == 0) out32[((uint64_t)(row0 + rr) * per_row + p) >> 5] = word;
+        }
     }
 }
 

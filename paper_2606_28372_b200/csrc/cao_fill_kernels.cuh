@@ -21,54 +21,67 @@ __device__ __forceinline__ void decode_row(const SpaceMeta& sm, uint64_t L, uint
     }
 }
 
-// One lane per 32-bit half word of the bitmap to find where the warp's rows start (the 16 lanes of a
-// 512-config group share a directory entry; a 16-lane shuffle scan gives each half word its first rank).  The
-// warp's W rows are contiguous in the table, so they are then produced one row per lane: output j belongs to
-// the last lane t with offset o_t <= j (binary search over the 32 offsets in shared memory), its config is the
-// (j - o_t)-th set bit of that lane's half word.  Row and Ltab stores are therefore fully coalesced.
+// A warp owns 32 consecutive 512-config groups per pass (grid-stride): lane l reads the directory count of
+// group g0 + l, so sparse regions cost one directory word per 512 configs and nothing else.  Groups are then
+// processed in pairs (32 half words of the bitmap = 1024 configs): a shuffle scan gives each half word its
+// first rank; the pair's W rows are contiguous in the table and are produced one row per lane -- output j
+// belongs to the last lane t with offset o_t <= j (binary search over the 32 offsets in shared memory), its
+// config is the (j - o_t)-th set bit of that lane's half word.  Row and Ltab stores are fully coalesced.
 template <int ROWW>
 __global__ void __launch_bounds__(256) k_fill(const __grid_constant__ SpaceMeta sm, uint64_t n_words,
                                               uint8_t* rows, uint64_t* Ltab, uint32_t* dir_out,
-                                              const uint32_t* __restrict__ dir, uint64_t nd) {
+                                              const uint32_t* __restrict__ dir, uint64_t nd, uint32_t gpw) {
+    // gpw = groups per warp pass: 2 for dense spaces (one pair per warp, maximum parallelism), 32 for sparse ones
     __shared__ uint32_t s_off[8][33];
     __shared__ uint32_t s_bits[8][32];
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const uint64_t hw = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t g = hw >> 4;
-    uint32_t base = 0, cnt = 0;
-    if (g < nd) {
-        base = dir[g]; cnt = dir[g + 1] - base;
-        if ((hw & 15) == 0) { dir_out[g] = base; if (g + 1 == nd) dir_out[nd] = base + cnt; }
-    }
-    uint32_t bits = 0;
-    if (cnt && hw < 2 * n_words) bits = ((const uint32_t*)sm.bitmap)[hw];
-    const uint32_t pc = __popc(bits);
-    uint32_t inc = pc;
+    const uint64_t nwarps = (uint64_t)gridDim.x * 8, wid = (uint64_t)blockIdx.x * 8 + wib;
+    for (uint64_t g0 = wid * gpw; g0 < nd; g0 += nwarps * gpw) {
+        const uint64_t gl = g0 + lane;
+        uint32_t gbase = 0, gcnt = 0;
+        if (lane < gpw && gl < nd) {
+            gbase = dir[gl]; gcnt = dir[gl + 1] - gbase;
+            dir_out[gl] = gbase;
+            if (gl + 1 == nd) dir_out[nd] = gbase + gcnt;
+        }
+        const uint32_t nonempty = __ballot_sync(0xFFFFFFFFu, gcnt != 0);
+        for (uint32_t pp = 0; pp < gpw / 2; ++pp) {
+            if (!((nonempty >> (2 * pp)) & 3u)) continue;               // both groups of the pair are empty
+            const uint64_t g = g0 + 2 * pp + (lane >> 4);                // this lane's group
+            const uint32_t base = __shfl_sync(0xFFFFFFFFu, gbase, 2 * pp + (lane >> 4));
+            const uint32_t cnt = __shfl_sync(0xFFFFFFFFu, gcnt, 2 * pp + (lane >> 4));
+            const uint64_t hw = g * 16 + (lane & 15);
+            uint32_t bits = 0;
+            if (cnt && g < nd && hw < 2 * n_words) bits = ((const uint32_t*)sm.bitmap)[hw];
+            const uint32_t pc = __popc(bits);
+            uint32_t inc = pc;
 #pragma unroll
-    for (int o = 1; o < 16; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o, 16); if ((lane & 15) >= o) inc += t; }
-    const uint32_t r = base + inc - pc;                                  // rank of this half word's first valid config
-    const uint32_t r0 = __shfl_sync(0xFFFFFFFFu, r, 0);
-    const uint32_t off = g < nd ? r - r0 : 0xFFFFFFFFu;                  // lanes past the directory own no rows
-    s_off[wib][lane] = off; s_bits[wib][lane] = bits;
-    // total rows of the warp = sum of pc (lanes beyond the directory have pc = 0)
-    uint32_t tot = pc;
+            for (int o = 1; o < 16; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o, 16); if ((lane & 15) >= o) inc += t; }
+            const uint32_t r = base + inc - pc;                          // rank of this half word's first valid config
+            const uint32_t r0 = __shfl_sync(0xFFFFFFFFu, r, 0);
+            const uint32_t off = g < nd ? r - r0 : 0xFFFFFFFFu;          // lanes past the directory own no rows
+            __syncwarp();
+            s_off[wib][lane] = off; s_bits[wib][lane] = bits;
+            uint32_t tot = pc;
 #pragma unroll
-    for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(0xFFFFFFFFu, tot, o);
-    __syncwarp();
-    const uint64_t hw0 = hw - lane;
-    for (uint32_t j = lane; j < tot; j += 32) {
-        uint32_t t = 0;                                                  // last lane with off <= j
+            for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(0xFFFFFFFFu, tot, o);
+            __syncwarp();
+            const uint64_t hw0 = (g0 + 2 * pp) * 16;
+            for (uint32_t j = lane; j < tot; j += 32) {
+                uint32_t t = 0;                                          // last lane with off <= j
 #pragma unroll
-        for (int step = 16; step; step >>= 1) { const uint32_t c = t + step; if (c < 32 && s_off[wib][c] <= j) t = c; }
-        const uint32_t b = (uint32_t)kth_set_bit32(s_bits[wib][t], j - s_off[wib][t]);
-        const uint64_t L = (hw0 + t) * 32 + b;
-        uint32_t w[ROWW];
-        decode_row<ROWW>(sm, L, w);
-        const uint64_t rr = (uint64_t)r0 + j;
-        uint4* dst = (uint4*)(rows + rr * (ROWW * 4));
-        dst[0] = make_uint4(w[0], w[1], w[2], w[3]);
-        if (ROWW == 8) dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
-        Ltab[rr] = L;
+                for (int step = 16; step; step >>= 1) { const uint32_t c = t + step; if (c < 32 && s_off[wib][c] <= j) t = c; }
+                const uint32_t b = (uint32_t)kth_set_bit32(s_bits[wib][t], j - s_off[wib][t]);
+                const uint64_t L = (hw0 + t) * 32 + b;
+                uint32_t w[ROWW];
+                decode_row<ROWW>(sm, L, w);
+                const uint64_t rr = (uint64_t)r0 + j;
+                uint4* dst = (uint4*)(rows + rr * (ROWW * 4));
+                dst[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                if (ROWW == 8) dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
+                Ltab[rr] = L;
+            }
+        }
     }
 }
 

@@ -52,7 +52,7 @@ struct cao_space {
     int n_tab = 0, n_res = 0;
     // scratch layout (byte offsets)
     uint64_t off_dom = 0, off_desc = 0, off_tables = 0, off_cnt = 0, off_part = 0, off_V = 0, scratch_bytes = 0;
-    uint64_t tables_words = 0, n_part = 0, max_table_threads = 0;
+    uint64_t tables_words = 0, n_part = 0, max_table_threads = 0, max_table_ci = 1;
     uint64_t bitmap_bytes = 0;
     void* d_scratch = nullptr;
     void* d_table = nullptr;

@@ -203,7 +203,7 @@ static int plan_space(cao_space* s) {
         D[tab.size() + res.size() + c] = (int32_t)D.size();
         D.insert(D.end(), s->cons[c].begin(), s->cons[c].end());
     }
-    s->max_table_threads = 0;
+    s->max_table_threads = 0; s->max_table_ci = 1;
     for (size_t k = 0; k < tab.size(); ++k) {
         const ConsPlan& p = s->plan[tab[k]];
         D[k] = (int32_t)D.size();
@@ -211,7 +211,16 @@ static int plan_space(cao_space* s) {
         D.push_back((int32_t)p.outer.size());
         for (size_t e = 0; e < p.outer.size(); ++e) { D.push_back(p.outer[e]); D.push_back((int32_t)p.cstride[e]); }
         D.push_back(prog_off[tab[k]]); D.push_back((int32_t)s->cons[tab[k]].size()); D.push_back((int32_t)p.rows);
+        // inner scope: the digits >= t the program reads; the inner pattern of a row depends on them only, so the
+        // program runs once per (row, inner-scope combination) and the result is replicated over the block
+        std::vector<int> inner; uint64_t Ci = 1;
+        for (int d : p.scope) if (d >= t) inner.push_back(d);           // scope is descending in d
+        std::vector<uint32_t> istride(inner.size());
+        for (size_t e = 0; e < inner.size(); ++e) { istride[e] = (uint32_t)Ci; Ci *= M.m[inner[e]]; }
+        D.push_back((int32_t)inner.size()); D.push_back((int32_t)Ci);
+        for (size_t e = 0; e < inner.size(); ++e) { D.push_back(inner[e]); D.push_back((int32_t)istride[e]); }
         s->max_table_threads = std::max<uint64_t>(s->max_table_threads, p.rows * s->Wb * 64);
+        s->max_table_ci = std::max<uint64_t>(s->max_table_ci, Ci);
     }
     for (size_t k = 0; k < res.size(); ++k) {
         D[tab.size() + k] = (int32_t)D.size();
@@ -250,7 +259,9 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     if (s->n_tab) {
         ProfScope ps(PK_TABLE, st);
         dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 255) / 256, 148 * 16), (unsigned)s->n_tab);
-        k_build_tables<<<grid, 256, 0, st>>>(s->meta, d_dom, d_desc, d_tables, s->B, s->Wb, s->t);
+        const size_t tsm = (size_t)std::max<uint64_t>(256, s->max_table_ci);      // <= B <= 65,280 bytes
+        if (tsm > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_build_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
+        k_build_tables<<<grid, 256, tsm, st>>>(s->meta, d_dom, d_desc, d_tables, s->B, s->Wb, s->t);
         CAO_LAUNCHED("k_build_tables");
     }
     EnumArgs ea{};
@@ -282,12 +293,15 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
 static int launch_fill(cao_space* s, uint8_t* tb, cudaStream_t st) {
     uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
     const uint32_t* cnt = (const uint32_t*)((uint8_t*)s->d_scratch + s->off_cnt);
-    uint64_t threads = s->nd * 16;
-    unsigned grid = (unsigned)((threads + 255) / 256);
+    // groups (512 configs) per warp pass.  One pair per warp measured fastest on dense AND sparse spaces (valid
+    // configs cluster, so a warp that skims 32 directory entries serialises the few non-empty pairs it meets).
+    const uint32_t gpw = 2u;
+    unsigned grid = (unsigned)((s->nd + 8ull * gpw - 1) / (8ull * gpw));
+    if (grid == 0) grid = 1;
     {
         ProfScope ps(PK_FILL, st);
-        if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
-        else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd);
+        if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd, gpw);
+        else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd, gpw);
     }
     CAO_LAUNCHED("k_fill");
     return CAO_OK;
