@@ -66,6 +66,64 @@ __global__ void __launch_bounds__(256) k_build_tables(const __grid_constant__ Sp
     }
 }
 
+// Value classes of a residual constraint (residual descriptor r: {nw, words...}).
+// k_res_prefix: one thread per block of configs runs the program up to its first inner parameter; the single
+// stack value left is the block's class key, entered into a small open-addressing table with atomicCAS.
+__global__ void __launch_bounds__(256) k_res_prefix(const __grid_constant__ SpaceMeta sm, const int64_t* __restrict__ dom,
+                                                    const int32_t* __restrict__ desc, int r, const ResClassArgs rc,
+                                                    uint64_t n_blocks, int32_t t) {
+    const uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= n_blocks) return;
+    const int32_t* ds = desc + desc[r];
+    int64_t x[CAO_MAX_DIMS];
+    uint64_t q = o;
+    for (int d = t - 1; d >= 0; --d) {
+        const uint32_t m = sm.m[d]; uint32_t idx = 0;
+        if (m > 1) { const uint64_t q2 = div_magic(q, sm.magic[d]); idx = (uint32_t)(q - q2 * m); q = q2; }
+        x[d] = dom[d * 256 + idx];
+    }
+    int64_t st[CAO_MAX_STACK];
+    int pc0 = 0, sp0 = 0;
+    const int pre = eval_core(ds + 1, ds[0], x, 0, st, 0, t, &pc0, &sp0);
+    uint32_t cls = CAO_CLS_FALSE;                                       // a zero divisor in the prefix: all false
+    if (pre == 2) {
+        const long long key = st[0];
+        uint32_t h = (uint32_t)(((uint64_t)key * 0x9E3779B97F4A7C15ull) >> 40) & (CAO_HS - 1);
+        cls = CAO_CLS_OVERFLOW;
+        for (int probe = 0; probe < 64; ++probe) {
+            const long long old = atomicCAS((unsigned long long*)&rc.keys[h], (unsigned long long)CAO_CLS_EMPTY, (unsigned long long)key);
+            if (old == CAO_CLS_EMPTY || old == key) { cls = h; break; }
+            h = (h + 1) & (CAO_HS - 1);
+        }
+        if (cls == CAO_CLS_OVERFLOW) *rc.overflow = 1;
+    }
+    rc.blk_class[o] = cls;
+}
+// k_res_class_table: one thread per (hash slot, inner pattern) resumes the program from the class key.
+__global__ void __launch_bounds__(256) k_res_class_table(const __grid_constant__ SpaceMeta sm, const int64_t* __restrict__ dom,
+                                                         const int32_t* __restrict__ desc, int r, const ResClassArgs rc,
+                                                         uint64_t B, uint32_t Wb, int32_t t) {
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t per_row = Wb * 64;
+    if (gid >= (uint64_t)CAO_HS * per_row) return;                      // whole warps: the bound is a multiple of 64
+    const uint32_t slot = (uint32_t)(gid / per_row), p = (uint32_t)(gid - (uint64_t)slot * per_row);
+    const long long key = rc.keys[slot];
+    int ok = 0;
+    if (key != CAO_CLS_EMPTY && p < B) {
+        const int32_t* ds = desc + desc[r];
+        int64_t x[CAO_MAX_DIMS];
+        for (int d = 0; d < sm.n; ++d) x[d] = dom[d * 256];
+        uint32_t q = p;
+        for (int d = sm.n - 1; d >= t; --d) { const uint32_t m = sm.m[d]; x[d] = dom[d * 256 + q % m]; q /= m; }
+        int64_t st[CAO_MAX_STACK];
+        st[0] = key;
+        int u0, u1;
+        ok = eval_core(ds + 1, ds[0], x, rc.pc0, st, 1, -1, &u0, &u1);
+    }
+    const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
+    if ((threadIdx.x & 31) == 0) ((uint32_t*)rc.table)[gid >> 5] = word;
+}
+
 __device__ __forceinline__ uint64_t get64(const uint64_t* mk, uint32_t r, uint32_t Wb) {
     uint32_t j = r >> 6, s = r & 63;
     if (j >= Wb) return 0;
@@ -108,11 +166,23 @@ __global__ void __launch_bounds__(256) k_enum_pass1(const __grid_constant__ Spac
             any = 0;
             for (uint32_t j = 0; j < a.Wb; ++j) { uint64_t v = mk[j] & __ldg(&tab[j]); mk[j] = v; any |= v; }
         }
+        for (int c = 0; c < a.n_rc && any; ++c) {                       // residual constraints with value classes
+            if (__ldg(a.rc[c].overflow)) continue;                      // (handled in phase 1b)
+            const uint32_t cls = __ldg(&a.rc[c].blk_class[o]);
+            any = 0;
+            if (cls == CAO_CLS_FALSE) { for (uint32_t j = 0; j < a.Wb; ++j) mk[j] = 0; }
+            else {
+                const uint64_t* tab = a.rc[c].table + (uint64_t)cls * a.Wb;
+                for (uint32_t j = 0; j < a.Wb; ++j) { uint64_t v = mk[j] & __ldg(&tab[j]); mk[j] = v; any |= v; }
+            }
+        }
     }
     // Phase 1b: residual constraints (too wide for a table, or plain mode).  One warp per block of configs: the
     // program prefix that reads only outer digits runs once per block, the lanes then share the surviving bits
     // of each mask word (warp-level compaction by k-th-set-bit selection) and clear the ones that fail.
-    if (a.n_res) {
+    bool need_1b = a.n_res > a.n_rc;
+    for (int c = 0; c < a.n_rc; ++c) need_1b = need_1b || __ldg(a.rc[c].overflow) != 0;
+    if (need_1b) {
         __syncthreads();
         const uint32_t lane = tid & 31, warp = tid >> 5, nwarp = bd >> 5;
         for (uint32_t i = warp; i <= a.nb; i += nwarp) {
@@ -132,6 +202,7 @@ __global__ void __launch_bounds__(256) k_enum_pass1(const __grid_constant__ Spac
                 }
             }
             for (int r = 0; r < a.n_res; ++r) {
+                if (r < a.n_rc && !__ldg(a.rc[r].overflow)) continue;  // already applied through its classes
                 const int32_t* ds = a.desc + __ldg(&a.desc[a.n_tab + r]);
                 const int nw = __ldg(&ds[0]);
                 int64_t st0[CAO_MAX_STACK];

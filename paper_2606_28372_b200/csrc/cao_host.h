@@ -49,7 +49,9 @@ struct cao_space {
     uint32_t Wb = 0, nb = 0, nb_tabled = 0;           // u64 words per block mask; blocks per CTA
     std::vector<ConsPlan> plan;
     std::vector<int32_t> desc;         // descriptor words uploaded to the device
-    int n_tab = 0, n_res = 0;
+    int n_tab = 0, n_res = 0, n_rc = 0;
+    int rc_pc0[4] = {0, 0, 0, 0};
+    uint64_t off_rc[4] = {0, 0, 0, 0}, rc_bytes = 0;
     // scratch layout (byte offsets)
     uint64_t off_dom = 0, off_desc = 0, off_tables = 0, off_cnt = 0, off_part = 0, off_V = 0, scratch_bytes = 0;
     uint64_t tables_words = 0, n_part = 0, max_table_threads = 0, max_table_ci = 1;
@@ -67,6 +69,21 @@ struct cao_space {
 };
 
 // Arguments of the pass-1 kernel, passed by value.
+// Residual constraint handled through value classes: blocks whose program prefix leaves the
+// same single stack value share one inner mask.
+#define CAO_HS 4096                         // hash slots = maximum number of distinct prefix values
+#define CAO_MAX_RC 4
+#define CAO_CLS_EMPTY ((long long)0x8080808080808080ll)   // below -2^62: never a saturated value
+#define CAO_CLS_FALSE 0xFFFFFFFFu
+#define CAO_CLS_OVERFLOW 0xFFFFFFFEu
+struct ResClassArgs {
+    long long* keys;                   // CAO_HS prefix values (CAO_CLS_EMPTY = free)
+    uint64_t* table;                   // CAO_HS x Wb inner masks
+    uint32_t* blk_class;               // n_blocks: hash slot of the block's prefix value
+    int32_t* overflow;                 // set if more than the table holds: the constraint falls back to phase 1b
+    int32_t pc0;                       // first token of the suffix
+};
+
 struct EnumArgs {
     uint64_t B, magicB, n_blocks, n_words;
     const int64_t* dom;                // [n][256]
@@ -75,7 +92,8 @@ struct EnumArgs {
     uint64_t* bitmap;
     uint32_t* cnt;                     // per-512 counts (zeroed)
     uint32_t Wb, nb;
-    int32_t t, n_tab, n_res;
+    int32_t t, n_tab, n_res, n_rc;     // the first n_rc residual constraints use value classes
+    ResClassArgs rc[CAO_MAX_RC];
 };
 
 struct cao_runs;

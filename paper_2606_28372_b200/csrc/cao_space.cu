@@ -192,8 +192,34 @@ static int plan_space(cao_space* s) {
     for (size_t c = 0; c < s->cons.size(); ++c) (s->plan[c].tabled ? tab : res).push_back((int)c);
     std::stable_sort(tab.begin(), tab.end(), [&](int a, int b) { return s->plan[a].rows < s->plan[b].rows; });
     s->n_tab = (int)tab.size(); s->n_res = (int)res.size();
-    // residual constraints are evaluated by one warp per block: fewer blocks per CTA keep the CTAs balanced
-    if (s->n_res) s->nb = std::min<uint32_t>(s->nb, 32);
+    // Value classes: a residual program whose tokens before the first inner parameter leave exactly one stack
+    // value, and whose remaining tokens read inner parameters only, depends on the outer digits through that one
+    // value.  Such constraints come first in the residual list.
+    std::vector<int> cls_pc0(s->cons.size(), -1);
+    if (s->mode == 0 && (uint64_t)CAO_HS * s->Wb * 8 <= (32ull << 20)) {
+        for (int c : res) {
+            const auto& w = s->cons[c];
+            int sp = 0, pc0 = -1; bool ok = true;
+            for (size_t pc = 0; pc < w.size(); ++pc) {
+                const int op = w[pc];
+                if (op == CAO_OP_PUSH_PARAM) {
+                    const int d = w[pc + 1];
+                    if (pc0 < 0 && d >= t) { pc0 = (int)pc; if (sp != 1) ok = false; }
+                    else if (pc0 >= 0 && d < t) ok = false;               // the suffix reads an outer parameter
+                    ++pc; ++sp;
+                } else if (op == CAO_OP_PUSH_CONST) { pc += 2; ++sp; }
+                else if (op == CAO_OP_NEG || op == CAO_OP_NOT) {}
+                else --sp;
+            }
+            if (ok && pc0 > 0) cls_pc0[c] = pc0;
+        }
+        std::stable_sort(res.begin(), res.end(), [&](int a, int b) { return (cls_pc0[a] >= 0) > (cls_pc0[b] >= 0); });
+    }
+    s->n_rc = 0;
+    for (int c : res) if (cls_pc0[c] >= 0 && s->n_rc < CAO_MAX_RC) s->rc_pc0[s->n_rc++] = cls_pc0[c];
+    // residual constraints outside the classes are evaluated by one warp per block: fewer blocks per CTA keep
+    // the CTAs balanced
+    if (s->n_res > s->n_rc) s->nb = std::min<uint32_t>(s->nb, 32);
     std::vector<int32_t>& D = s->desc;
     D.assign(tab.size() + res.size() + s->cons.size(), 0);       // [tab offs][res offs][program offs of every constraint]
     // programs first, so that the tabled descriptors can point at them
@@ -236,6 +262,8 @@ static int plan_space(cao_space* s) {
     s->n_part = (s->nd + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK;
     s->off_part = off; off = align256(off + s->n_part * 4);
     s->off_V = off; off = align256(off + 8);
+    s->rc_bytes = align256((uint64_t)CAO_HS * 8) + align256((uint64_t)CAO_HS * s->Wb * 8) + align256(s->n_blocks * 4) + 256;
+    for (int k = 0; k < s->n_rc; ++k) { s->off_rc[k] = off; off += s->rc_bytes; }
     s->scratch_bytes = off;
     s->bitmap_bytes = align256(s->n_words * 8);
     s->planned = true;
@@ -265,6 +293,24 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         CAO_LAUNCHED("k_build_tables");
     }
     EnumArgs ea{};
+    ea.n_rc = s->n_rc;
+    for (int k = 0; k < s->n_rc; ++k) {
+        uint8_t* b = sc + s->off_rc[k];
+        ResClassArgs& rc = ea.rc[k];
+        rc.keys = (long long*)b; b += align256((uint64_t)CAO_HS * 8);
+        rc.table = (uint64_t*)b; b += align256((uint64_t)CAO_HS * s->Wb * 8);
+        rc.blk_class = (uint32_t*)b; b += align256(s->n_blocks * 4);
+        rc.overflow = (int32_t*)b;
+        rc.pc0 = s->rc_pc0[k];
+        CAO_CUDA(cudaMemsetAsync(rc.keys, 0x80, (uint64_t)CAO_HS * 8, st));
+        CAO_CUDA(cudaMemsetAsync(rc.overflow, 0, 4, st));
+        ProfScope ps(PK_TABLE, st);
+        k_res_prefix<<<(unsigned)((s->n_blocks + 255) / 256), 256, 0, st>>>(s->meta, d_dom, d_desc, s->n_tab + k, rc, s->n_blocks, s->t);
+        CAO_LAUNCHED("k_res_prefix");
+        const uint64_t threads = (uint64_t)CAO_HS * s->Wb * 64;
+        k_res_class_table<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(s->meta, d_dom, d_desc, s->n_tab + k, rc, s->B, s->Wb, s->t);
+        CAO_LAUNCHED("k_res_class_table");
+    }
     ea.B = s->B; ea.magicB = s->B > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + s->B - 1) / s->B) : 0;
     ea.n_blocks = s->n_blocks; ea.n_words = s->n_words; ea.dom = d_dom; ea.desc = d_desc; ea.tables = d_tables;
     ea.bitmap = (uint64_t*)d_bitmap; ea.cnt = (uint32_t*)(sc + s->off_cnt);
