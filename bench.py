@@ -30,6 +30,7 @@ import numpy as np
 ALGO_GENS_CAP = {1: 200, 0: 50, 2: 150, 3: 100, 4: 200}
 ISSUE_LANES_PER_SM_CLK = 128          # 4 SMSP x 32 lanes: one warp instruction per SMSP per clock (B300_MICROARCH.md)
 N_SM = 148
+NCU_KGEN_DRAM_BYTES_PER_LAUNCH = 18.35e6   # (26.2 + 28.7 + 8.1 + 10.4) MB / 4, profiles/r1b_fused.md
 
 
 def peaks():
@@ -291,7 +292,14 @@ def gpu_arm(args):
                "k_gen": 2 * (rb + 8) + 32 + 32 + 32 + 64}.get(top, 64)
         by = per * cands_step / max(top_n, 1)
         roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "peak_source": pk["source"], "traffic": None}
+                "peak_source": pk["source"], "traffic": None,
+                "algorithmic_bytes_per_candidate": per}
+        if top == "k_gen" and args.config == 1 and R == 1000:
+            # dram__bytes_read.sum + dram__bytes_write.sum per launch, mean of the four k_gen launches of one step,
+            # from the ncu --set full capture summarised in profiles/r1b_fused.md
+            roof["traffic"] = NCU_KGEN_DRAM_BYTES_PER_LAUNCH
+            roof["note"] = ("at 1000 runs k_gen is bound by per-run latency and the longest run (issue 15-23 %, DRAM 0.1 %): "
+                            "profiles/r1b_fused.md; extra.sweep_cfg4 shows candidates/s against the number of runs")
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_us"] = dur_s * 1e6
     roof["share_of_step"] = top_ms / (ms_prof / args.steps)
