@@ -106,56 +106,11 @@ __device__ __forceinline__ int probe23_cta(const SpaceMeta& sm, const ProbeMeta&
         best = warp_min_u64(best);
         if ((tid & 31) == 0 && best != ~0ull) atomicMin(s_best, best);
         __syncthreads();
-        if (*s_best != ~0ull) found = level;
+        const bool hit = *s_best != ~0ull;
+        __syncthreads();                                                // everyone has read the slot before the next level writes it
+        if (hit) found = level;
     }
     return found;
-}
-
-// Block-cooperative brute-force scan of the whole valid table for up to NB candidates at once (rows in shared
-// memory, s_cw[b * ROWW ..]); the rows are read straight from L2, coalesced, every thread keeps NB running minima.
-// s_key[b] must be ~0 on entry; on exit it holds ham << 45 | sad << 32 | rank.  Ends with a barrier.
-template <int ROWW, int NB>
-__device__ __forceinline__ void scan_cta(const SpaceMeta& sm, const uint32_t* s_cw, int nb, unsigned long long* s_key) {
-    uint32_t c[NB][ROWW];
-#pragma unroll
-    for (int b = 0; b < NB; ++b)
-#pragma unroll
-        for (int k = 0; k < ROWW; ++k) c[b][k] = b < nb ? s_cw[b * ROWW + k] : 0;
-    uint64_t best[NB];
-#pragma unroll
-    for (int b = 0; b < NB; ++b) best[b] = ~0ull;
-    constexpr int RU = ROWW == 4 ? 8 : 4;                              // rows in flight per thread (128 bytes of loads)
-    for (uint32_t r0 = threadIdx.x; r0 < sm.V; r0 += RU * blockDim.x) {
-        uint32_t v[RU][ROWW];
-#pragma unroll
-        for (int u = 0; u < RU; ++u) {
-            const uint32_t r = r0 + u * blockDim.x;
-            load_row<ROWW>(sm.rows + (uint64_t)(r < sm.V ? r : r0) * (ROWW * 4), v[u]);    // clamped: never out of the table
-        }
-#pragma unroll
-        for (int u = 0; u < RU; ++u) {
-            const uint32_t r = r0 + u * blockDim.x;
-            if (r >= sm.V) break;
-#pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                uint32_t sad = 0, ham = 0;
-#pragma unroll
-                for (int k = 0; k < ROWW; ++k) {
-                    sad = sad4_acc(c[b][k], v[u][k], sad);
-                    const uint32_t x = c[b][k] ^ v[u][k];
-                    ham += __popc((((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x) & 0x80808080u);
-                }
-                const uint64_t key = ((uint64_t)((ham << 13) + sad) << 32) | r;
-                best[b] = key < best[b] ? key : best[b];
-            }
-        }
-    }
-#pragma unroll
-    for (int b = 0; b < NB; ++b) {
-        const uint64_t m = warp_min_u64(best[b]);
-        if ((threadIdx.x & 31) == 0 && b < nb) atomicMin(&s_key[b], m);
-    }
-    __syncthreads();
 }
 
 template <int ROWW>
@@ -263,7 +218,7 @@ __global__ void __launch_bounds__(256) k_repair_probe(const __grid_constant__ Sp
     if (k == CAO_KEY_NONE) { if (in_dom && wl2 != wl) worklist_push(wl, wl_count, (uint32_t)i); else worklist_push(wl2, wl2_count, (uint32_t)i); }
 }
 
-__global__ void __launch_bounds__(256) k_repair_finish(const unsigned long long* __restrict__ key, uint64_t count,
+static __global__ void __launch_bounds__(256) k_repair_finish(const unsigned long long* __restrict__ key, uint64_t count,
                                                        uint32_t* rank_out, uint64_t* key_out) {
     uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;

@@ -3,6 +3,15 @@
 #include <cstring>
 #include "cao_runs_kernels.cuh"
 
+// Fused generation kernel, one object per algorithm (cao_gen_algo.cu).
+struct GenLayout;
+#define CAO_GEN_DECL(A)                                                                                                   \
+    int cao_gen_setup_##A(int roww, unsigned threads, size_t smem, int* occ);                                             \
+    int cao_gen_launch_##A(int roww, unsigned grid, unsigned threads, size_t smem, cudaStream_t st, const SpaceMeta& sm,  \
+                           const ProbeMeta& pm, const RunsMeta& rm, const GenLayout& lay, uint32_t g_first, uint32_t n_gens);
+CAO_GEN_DECL(0) CAO_GEN_DECL(1) CAO_GEN_DECL(2) CAO_GEN_DECL(3)
+#include "cao_gen_layout.h"
+
 #define SCAN_GRID (148 * 8)
 
 struct cao_runs {
@@ -10,8 +19,11 @@ struct cao_runs {
     SpaceMeta sm{};
     RunsMeta rm{};
     uint32_t gen = 0;
-    unsigned block = 32, block_fused = 128;
+    unsigned block = 32;
     int mode = 1;                      // 1 = fused persistent k_gen, 0 = phased (k_op / k_probe23 / k_scan / k_finish)
+    GenLayout lay{};                   // shared-memory slice of one group of the fused kernel
+    unsigned gen_threads = 256, gen_grid = 0;
+    size_t gen_smem = 0;
     size_t smem_init = 0, smem_op = 0, smem_fin = 0;
     // raw state views for cao_runs_debug_state
     uint64_t bytes_idx = 0, bytes_pi = 0, bytes_pn = 0;
@@ -120,10 +132,34 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
     return CAO_OK;
 }
 
+// Shared-memory slice of one group of the fused kernel (cao_gen_kernels.cuh): word offsets.
+static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P) {
+    GenLayout L{};
+    const uint32_t n = (uint32_t)s->meta.n, roww = (uint32_t)s->meta.rowB / 4;
+    uint32_t off = GRP_SHARED_WORDS;
+    auto take = [&](uint32_t words) { uint32_t o = off; off = (off + std::max(1u, words) + 3u) & ~3u; return o; };
+    L.rank = take(P); L.f = take(P);
+    const bool cont = algo == CAO_PSO || algo == CAO_FIREFLY;
+    L.idx = take(cont ? 0 : P * roww);
+    L.x = take(cont ? n * P : 0);
+    L.v = take(algo == CAO_PSO ? n * P : 0); L.pb = take(algo == CAO_PSO ? n * P : 0); L.pbf = take(algo == CAO_PSO ? P : 0);
+    L.cand = take(P * roww); L.key = take(2 * P);
+    L.scr = take(algo == CAO_GA ? 3 * P : P);
+    L.wl = take(P); L.cw = take(GEN_NB * roww); L.skey = take(2 * GEN_NB); L.bestrow = take(roww);
+    L.words = off;
+    L.G = (P + 31) / 32 * 32;
+    L.NG = L.G <= 256 ? 256 / L.G : 1;
+    const uint64_t tab_bytes = (uint64_t)s->probe.C2 * 4 + (uint64_t)s->probe.T * 2;
+    L.cta_words = (s->probe.levels >= 2 && tab_bytes <= 16384) ? (uint32_t)((tab_bytes + 15) / 16 * 4) : 0;
+    // keep one CTA below the 227 KB opt-in limit: fewer groups per CTA for large populations / many dimensions
+    while (L.NG > 1 && ((uint64_t)L.cta_words + (uint64_t)L.NG * L.words) * 4 > 200 * 1024) --L.NG;
+    return L;
+}
+
 // ---------------------------------------------------------------------------------------------
 struct RunsLayout {
     uint64_t cand, key, valid, rep_rank, eval_rank, tap_f, accept, active, idx, rank, f, x, v, pb, pbf, dedup,
-        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl2, wl_count, counters, rcache, total;
+        uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl2, wl_count, counters, rcache, ticket, total;
     uint64_t zero_from, zero_bytes;       // region that must start as zero: dedup .. stagn
     uint32_t dedup_words;
 };
@@ -144,7 +180,7 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
     L.zero_from = off;
     L.dedup = take(R * L.dedup_words * 4);
     L.uniq = take(R * 4); L.gens_done = take(R * 4); L.stagn = take(R * 4);
-    L.wl_count = take(8); L.counters = take(4 * 8);
+    L.wl_count = take(8); L.counters = take(4 * 8); L.ticket = take(8);
     L.zero_bytes = off - L.zero_from;
     L.best_rank = take(R * 4); L.best_f = take(R * 4);
     L.traj = take((max_gens + 1) * R * 12);
@@ -206,12 +242,14 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     m.wl2 = (uint32_t*)(w + L.wl2); m.wl2_count = m.wl_count + 1;
     m.counters = (unsigned long long*)(w + L.counters);
     m.rcache = (ulonglong2*)(w + L.rcache);
+    m.ticket = (uint32_t*)(w + L.ticket);
     const uint64_t RP = (uint64_t)n_runs * pop;
     r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
     r->block = (unsigned)((pop + 31) / 32 * 32);
-    // fused CTAs: 128 threads help the block-cooperative repairs while all runs fit one wave (148 SMs x 8 CTAs of
-    // <= 64 registers x 128 threads); beyond that, one warp per run keeps 32 runs resident per SM
-    r->block_fused = n_runs <= 148u * 8u ? std::max(r->block, 128u) : r->block;
+    r->lay = gen_layout(s, algo, (uint32_t)pop);
+    r->gen_threads = r->lay.G * r->lay.NG;
+    r->gen_smem = ((size_t)r->lay.cta_words + (size_t)r->lay.NG * r->lay.words) * 4;
+    if (r->gen_smem > 227 * 1024) r->mode = 0;                         // the population does not fit one SM: phased only
     const size_t P = (size_t)pop, n = (size_t)s->meta.n;
     r->smem_init = P * 4;
     r->smem_op = algo == CAO_GA ? P * 12 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
@@ -244,18 +282,34 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
     if (r->mode == 1) {                                                 // fused: one launch for all the generations
         const uint32_t left = r->rm.max_gens - r->gen, ng = std::min(n_generations, left);   // g <= max_gens (O10)
         if (ng == 0) return CAO_OK;
-        const uint32_t scratch_words = (uint32_t)((std::max(r->smem_op, r->smem_fin) + 3) / 4);
-        const size_t smem = (size_t)scratch_words * 4 + (size_t)r->rm.P * 4;
-#define CALL_GEN(A, W) \
-        if (r->block_fused <= 256) { \
-            if (smem > 48 * 1024) cudaFuncSetAttribute(k_gen<A, W, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            k_gen<A, W, 256><<<r->rm.R, r->block_fused, smem, st>>>(r->sm, r->s->probe, r->rm, r->gen, ng, scratch_words); \
-        } else { \
-            if (smem > 48 * 1024) cudaFuncSetAttribute(k_gen<A, W, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            k_gen<A, W, 1024><<<r->rm.R, r->block_fused, smem, st>>>(r->sm, r->s->probe, r->rm, r->gen, ng, scratch_words); \
+        if (r->gen_grid == 0) {                                         // first launch: opt-in shared memory, persistent grid size
+            int occ = 0, dev = 0, sms = 0;
+            CAO_CUDA(cudaGetDevice(&dev));
+            CAO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            int rc = CAO_OK;
+            switch (algo) {
+                case CAO_DE: rc = cao_gen_setup_0(roww, r->gen_threads, r->gen_smem, &occ); break;
+                case CAO_PSO: rc = cao_gen_setup_1(roww, r->gen_threads, r->gen_smem, &occ); break;
+                case CAO_FIREFLY: rc = cao_gen_setup_2(roww, r->gen_threads, r->gen_smem, &occ); break;
+                default: rc = cao_gen_setup_3(roww, r->gen_threads, r->gen_smem, &occ); break;
+            }
+            if (rc) return rc;
+            if (occ < 1) return cao_fail(CAO_E_TOO_LARGE, "cao_runs_step: the population state does not fit the shared memory of one SM");
+            const uint64_t need = ((uint64_t)r->rm.R + r->lay.NG - 1) / r->lay.NG;
+            r->gen_grid = (unsigned)std::min<uint64_t>(need, (uint64_t)sms * (uint64_t)occ);
         }
-        { ProfScope ps(PK_GEN, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_GEN); }
-        CAO_LAUNCHED("k_gen");
+        int rc = CAO_OK;
+        {
+            ProfScope ps(PK_GEN, st);
+            switch (algo) {
+#define CALL_GEN(A) rc = cao_gen_launch_##A(roww, r->gen_grid, r->gen_threads, r->gen_smem, st, r->sm, r->s->probe, r->rm, r->lay, r->gen, ng)
+                case CAO_DE: CALL_GEN(0); break;
+                case CAO_PSO: CALL_GEN(1); break;
+                case CAO_FIREFLY: CALL_GEN(2); break;
+                default: CALL_GEN(3); break;
+            }
+        }
+        if (rc) return rc;
         r->gen += ng;
         return CAO_OK;
     }
@@ -284,6 +338,8 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
 
 int cao_runs_set_mode(cao_runs* r, int32_t mode) {
     if (!r || (mode != 0 && mode != 1)) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_set_mode: mode must be 0 (phased) or 1 (fused)");
+    if (mode == 1 && r->gen_smem > 227 * 1024)
+        return cao_fail(CAO_E_TOO_LARGE, "cao_runs_set_mode: the population state does not fit the shared memory of one SM (fused mode)");
     r->mode = mode;
     return CAO_OK;
 }

@@ -30,6 +30,7 @@ struct RunsMeta {
     uint32_t* wl; uint32_t* wl_count;                  // candidates without a valid Hamming-1 neighbour
     uint32_t* wl2; uint32_t* wl2_count;                // ... and none up to the probed level: table scan
     ulonglong2* rcache;                                // [run][CAO_RCACHE] {L, key}: repairs at Hamming >= 2 already resolved (fused mode)
+    uint32_t* ticket;                                  // [2] run ticket + finished-group counter of the fused kernel (self re-arming)
     unsigned long long* counters;                      // n_repaired, n_scanned, n_evaluated
 };
 
@@ -459,77 +460,4 @@ __global__ void __launch_bounds__(1024) k_finish(const __grid_constant__ SpaceMe
     gen_finish<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh);
 }
 
-// ---------------------------------------------------------------------------------------------
-// Fused persistent generation kernel: one CTA owns one run for n_gens generations (S3-S7 without leaving the
-// SM).  Per generation: operator + snap + validity + Hamming-1 probe by the P individual threads; the few
-// candidates still unresolved are repaired by the WHOLE block (Hamming-2/3 pair-table probe, then a
-// brute-force scan of the table in batches of GEN_NB candidates); then evaluation, selection and the trajectory
-// row.  The run's state stays in global memory but is private to the CTA, so it lives in L1/L2 between
-// generations; __syncthreads() orders the phases.
-#define GEN_NB 4
-template <int ALGO, int ROWW, int MAXT>
-__global__ void __launch_bounds__(MAXT) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
-                                              const __grid_constant__ RunsMeta rm, uint32_t g_first, uint32_t n_gens,
-                                              uint32_t scratch_words) {
-    extern __shared__ uint32_t s_dyn[];
-    __shared__ RunShared sh;
-    __shared__ uint32_t s_nwl;
-    __shared__ uint32_t s_cw[GEN_NB * ROWW];
-    __shared__ unsigned long long s_key[GEN_NB];
-    uint32_t* s_wl = s_dyn + scratch_words;                             // P slots
-    const uint32_t k = blockIdx.x, tid = threadIdx.x;
-    for (uint32_t g = g_first + 1; g <= g_first + n_gens; ++g) {
-        __syncthreads();
-        const bool active = rm.budget == 0 || rm.uniq[k] < rm.budget;   // O10
-        if (tid == 0) { rm.active[k] = active ? 1 : 0; s_nwl = 0; }
-        if (!active) { if (tid == 0) frozen_row(rm, k, g); continue; }
-        __syncthreads();
-        gen_op<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh, s_wl, &s_nwl, false, true);
-        __syncthreads();
-        const uint32_t nwl = s_nwl;
-        uint32_t nscan = 0;
-        if (pm.levels >= 2) {
-            for (uint32_t f = 0; f < nwl; ++f) {
-                const uint32_t slot = s_wl[f];
-                __syncthreads();
-                if (tid < ROWW) s_cw[tid] = ((const uint32_t*)(rm.cand + (uint64_t)slot * (ROWW * 4)))[tid];
-                if (tid == 0) s_key[0] = ~0ull;
-                __syncthreads();
-                const int found = probe23_cta<ROWW>(sm, pm, s_cw, &s_key[0]);
-                if (tid == 0) {
-                    const uint64_t best = s_key[0];
-                    if (found) {
-                        const uint64_t key = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
-                        rm.key[slot] = key;
-                        uint64_t L = 0;
-                        for (int d = 0; d < sm.n; ++d) L += (uint64_t)((const uint8_t*)s_cw)[d] * sm.stride[d];
-                        rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)] = make_ulonglong2(L, key);
-                    } else {
-                        s_wl[nscan] = slot;                             // nscan <= f: compacts in place
-                    }
-                }
-                if (!found) ++nscan;
-            }
-        } else {
-            nscan = nwl;
-        }
-        for (uint32_t f0 = 0; f0 < nscan; f0 += GEN_NB) {
-            const uint32_t nb = min((uint32_t)GEN_NB, nscan - f0);
-            __syncthreads();
-            if (tid < nb * ROWW) s_cw[tid] = ((const uint32_t*)(rm.cand + (uint64_t)s_wl[f0 + tid / ROWW] * (ROWW * 4)))[tid % ROWW];
-            if (tid < GEN_NB) s_key[tid] = ~0ull;
-            __syncthreads();
-            if (nb == 1) scan_cta<ROWW, 1>(sm, s_cw, 1, s_key);
-            else scan_cta<ROWW, GEN_NB>(sm, s_cw, (int)nb, s_key);
-            if (tid < nb) {
-                rm.key[s_wl[f0 + tid]] = s_key[tid];
-                uint64_t L = 0;
-                for (int d = 0; d < sm.n; ++d) L += (uint64_t)((const uint8_t*)(s_cw + tid * ROWW))[d] * sm.stride[d];
-                rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)] = make_ulonglong2(L, s_key[tid]);   // same slot twice: either entry is exact
-            }
-        }
-        if (tid == 0 && nscan) atomicAdd(&rm.counters[1], (unsigned long long)nscan);
-        __syncthreads();
-        gen_finish<ALGO, ROWW>(sm, rm, k, g, s_dyn, sh);
-    }
-}
+#define GEN_NB 4                                          // candidates per batch of the in-group table scan (cao_gen_kernels.cuh)
