@@ -158,6 +158,12 @@ int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, u
  * candidates that needed the table scan, candidates evaluated. */
 int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uint64_t* n_scanned,
                       uint64_t* n_evaluated);
+/* All sixteen 64-bit statistics words since create (synchronises `stream`): 0 n_repaired, 1 n_scanned (candidates that
+ * needed the table scan), 2 n_evaluated; fused mode only: 3 candidates that went to the Hamming-2 probe, 4 ... to the
+ * Hamming-3 probe, 5 invalid candidates resolved by the previous generation's memo, 6 ... by the per-run repair cache;
+ * 7 reserved; 8-13 clock cycles of thread 0 of every group in operator / tail / probe-2 / probe-3 / scan / finish
+ * (only in builds with -DCAO_GEN_STATS, else 0); 14-15 reserved.  L268 (memoisation) is what 5 and 6 count. */
+int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out16);
 /* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
 uint64_t cao_launch_count(void);
 

@@ -68,6 +68,7 @@ SIGNATURES = {
     "cao_runs_debug_last": (C.c_int, [vp, pvp, pvp, pvp, pvp, pvp, pvp, pvp]),
     "cao_runs_debug_state": (C.c_int, [vp, i32, pvp, pu64]),
     "cao_runs_counters": (C.c_int, [vp, vp, pu64, pu64, pu64]),
+    "cao_runs_stats": (C.c_int, [vp, vp, pu64]),
     "cao_launch_count": (u64, []),
     "cao_profile_enable": (C.c_int, [i32]),
     "cao_profile_read": (C.c_int, [i32, C.POINTER(C.c_double), pu64]),
@@ -372,6 +373,14 @@ class Runs:
         a, b, c = u64(), u64(), u64()
         _check(lib().cao_runs_counters(self._h, _stream(), C.byref(a), C.byref(b), C.byref(c)))
         return dict(n_repaired=a.value, n_scanned=b.value, n_evaluated=c.value)
+
+    def stats(self):
+        """cao_runs_stats: the sixteen statistics words as a dict."""
+        a = (C.c_uint64 * 16)()
+        _check(lib().cao_runs_stats(self._h, _stream(), a))
+        names = ["n_repaired", "n_scanned", "n_evaluated", "n_probe2", "n_probe3", "n_memo", "n_rcache", "r7",
+                 "cyc_op", "cyc_tail", "cyc_probe2", "cyc_probe3", "cyc_scan", "cyc_finish", "cyc_max_run", "cyc_max_scan"]
+        return {k: int(v) for k, v in zip(names, a)}
 
     def __del__(self):
         try:

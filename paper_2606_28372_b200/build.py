@@ -48,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         os.makedirs(OBJ, exist_ok=True)
-        extra = ["-Xptxas", "-v"] if verbose else []
+        extra = (["-Xptxas", "-v"] if verbose else []) + os.environ.get("CAO_NVCC_EXTRA", "").split()
 
         def compile_one(u):
             src, obj, flags = u

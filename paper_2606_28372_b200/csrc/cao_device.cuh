@@ -26,13 +26,16 @@ struct SpaceMeta {
     uint16_t m[CAO_MAX_DIMS];
 };
 
-// Targets of the Hamming-2/3 probes: every (dimension, value index) pair, sorted by dimension then value.
+// Neighbour lists of the Hamming-level probes (S5).  A point has NB = sum (m_d - 1) Hamming-1 neighbours; neighbour
+// t = (dimension d, k) with k = 0 .. m_d - 2 stands for the value index v = k + (k >= c_d) != c_d of a candidate c, so
+// no probe is ever wasted on the candidate's own value.  Entries are sorted by (d, k).
+#define CAO_MAX_PROBE_LEVEL 6
 struct ProbeMeta {
-    const uint16_t* tgt;                // T entries: d << 8 | v
+    const uint16_t* nb;                 // NB entries: d << 8 | k
     const uint32_t* pairs;              // C2 entries: t1 | t2 << 16, dimension(t1) < dimension(t2)
-    uint32_t T, C2;
-    int32_t levels;                     // highest Hamming level probed in the bitmap before the table scan (1..3)
-    uint16_t dim_first[CAO_MAX_DIMS + 1];   // first target of dimension d; dim_first[n] = T
+    uint32_t NB, C2;
+    int32_t levels;                     // highest Hamming level probed in the bitmap before the table scan (0..6)
+    uint16_t nb_first[CAO_MAX_DIMS + 1];    // first neighbour of dimension d; nb_first[n..] = NB
 };
 
 // ---------------------------------------------------------------------------------------------

@@ -19,46 +19,32 @@ struct GrpShared {                   // first words of every group slice
     unsigned long long best;         // (f bits << 32 | rank) of the best-so-far
     unsigned long long aux;          // PSO: (pbest_f bits << 32 | i) of gbest; probe: level minimum
     uint32_t run, uniq, stagn, n_new, flag, nwl, bestrow_rank, gens;
-    uint32_t n_inv, n_scan, n_eval, pad;
+    uint32_t n_inv, n_scan, n_eval, n_p2, n_p3, n_memo, n_rc, pad;   // statistics of this run in this launch
+    unsigned long long cyc[6];       // CAO_GEN_STATS builds: clock cycles in operator / tail / probe-2 / probe-3 / scan / finish
 };
+#ifdef CAO_GEN_STATS
+#define CAO_TICK(slot) do { if (g.t == 0) { const long long now_ = clock64(); gs->cyc[slot] += (unsigned long long)(now_ - t_mark); t_mark = now_; } } while (0)
+#else
+#define CAO_TICK(slot) do { } while (0)
+#endif
 static_assert(sizeof(GrpShared) == GRP_SHARED_WORDS * 4, "GrpShared layout");
 
-struct Grp {
-    uint32_t t, G, id;               // thread within the group, group size, group within the CTA
-    __device__ __forceinline__ void sync() const {
-        if (G == 32) __syncwarp();
-        else asm volatile("bar.sync %0, %1;" ::"r"(id + 1), "r"(G) : "memory");
-    }
-    __device__ __forceinline__ bool sync_or(bool p) const {
-        if (G == 32) return __any_sync(0xFFFFFFFFu, p);
-        uint32_t r;
-        asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %1, 0;\n\tbar.red.or.pred q, %2, %3, p;\n\tselp.u32 %0, 1, 0, q;\n\t}"
-                     : "=r"(r) : "r"((uint32_t)p), "r"(id + 1), "r"(G) : "memory");
-        return r != 0;
-    }
+// CTA-wide tables in shared memory (built once per CTA in the kernel prologue).
+struct CtaTabs {
+    const uint16_t* nb;              // Hamming-1 neighbour list: d << 8 | k, k = 0 .. m_d - 2, sorted by (d, k)
+    const uint64_t* stride;          // stride[d]
+    const float* hi;                 // coord(m_d - 1) (O6)
+    const uint32_t* pairs;           // pair list of the Hamming >= 2 probes (shared or global memory)
+    uint32_t NB;
 };
-
-// Minimum of a 64-bit key over the warp: two REDUX on the halves (the high half decides, then the low half among the
-// lanes that hold the minimal high half).
-__device__ __forceinline__ uint64_t warp_min_key(uint64_t v) {
-    const uint32_t hi = (uint32_t)(v >> 32), lo = (uint32_t)v;
-    const uint32_t mh = __reduce_min_sync(0xFFFFFFFFu, hi);
-    const uint32_t ml = __reduce_min_sync(0xFFFFFFFFu, hi == mh ? lo : 0xFFFFFFFFu);
-    return ((uint64_t)mh << 32) | ml;
-}
-// Group-wide minimum into *slot (which must hold ~0 / a running minimum visible to the group); ends with a barrier.
-__device__ __forceinline__ void grp_min_key(const Grp& g, uint64_t v, unsigned long long* slot) {
-    const uint64_t m = warp_min_key(v);
-    if ((g.t & 31) == 0 && m != ~0ull) atomicMin(slot, (unsigned long long)m);
-    g.sync();
-}
 
 // Validity and rank of linear index L in ONE round trip: the directory entry and the 64-byte bitmap block of L are
 // loaded together; the rank is only meaningful when the bit is set.
-__device__ __forceinline__ uint32_t valid_rank(const SpaceMeta& sm, uint64_t L, bool& valid) {
+static __device__ __noinline__ uint32_t valid_rank(const uint64_t* __restrict__ bitmap, const uint32_t* __restrict__ dir, uint64_t L,
+                                                   uint32_t* valid) {
     const uint32_t wi = (uint32_t)(L >> 6) & 7u;
-    const ulonglong2* blk = (const ulonglong2*)(sm.bitmap + ((L >> 6) & ~7ull));
-    uint32_t r = __ldg(&sm.dir[L >> CAO_DIR_SHIFT]);
+    const ulonglong2* blk = (const ulonglong2*)(bitmap + ((L >> 6) & ~7ull));
+    uint32_t r = __ldg(&dir[L >> CAO_DIR_SHIFT]);
     const ulonglong2 v0 = __ldg(&blk[0]), v1 = __ldg(&blk[1]), v2 = __ldg(&blk[2]), v3 = __ldg(&blk[3]);
     const uint64_t wd[8] = {v0.x, v0.y, v1.x, v1.y, v2.x, v2.y, v3.x, v3.y};
     const uint64_t below_mask = (1ull << (L & 63)) - 1ull;
@@ -69,92 +55,45 @@ __device__ __forceinline__ uint32_t valid_rank(const SpaceMeta& sm, uint64_t L, 
         mine = q == wi ? wd[q] : mine;
     }
     r += __popcll(mine & below_mask);
-    valid = (mine >> (L & 63)) & 1ull;
+    *valid = (uint32_t)((mine >> (L & 63)) & 1ull);
     return r;
 }
 
-// Hamming-1 probe of an invalid in-domain row (exact: Hamming is the primary key, |delta| the secondary, L the third):
-// level |delta| = 1, 2, ... until a level has a valid neighbour.  All bit tests of a level are independent loads.
-template <int ROWW>
-__device__ __forceinline__ uint64_t probe_h1_v2(const SpaceMeta& sm, const uint32_t (&w)[ROWW], uint64_t L) {
-    for (int delta = 1; delta < sm.M; ++delta) {
-        uint64_t bestL = ~0ull;
-        if (delta <= 2) {
-            uint64_t cand[ROWW * 8];
-            bool hit[ROWW * 8];
+// Group-cooperative Hamming-1 probe (exact: Hamming is the primary key, |delta| the secondary, L the third).  The
+// `nopen` open candidates (list ol, linear indices Lc, rows8 = the group's candidate rows, RB bytes each) times their NB
+// neighbours form one flat index space that the threads stride over, four independent bit tests in flight each; hits
+// go to hkey[candidate] with a shared-memory atomicMin on (|delta| << 40 | L').  The caller synchronises afterwards.
+template <int RB>
+__device__ __forceinline__ void probe_h1_flat(const Grp& g, const uint64_t* __restrict__ bitmap, const CtaTabs& tb, const uint8_t* rows8,
+                                              const uint32_t* ol, const uint64_t* Lc, unsigned long long* hkey, uint32_t nopen) {
+    const uint32_t NB = tb.NB, total = nopen * NB;
+    uint32_t jj = g.t / NB, t = g.t - jj * NB;
+    const uint32_t sj = g.G / NB, st = g.G - sj * NB;
+    for (uint32_t q0 = g.t; q0 < total; q0 += 4 * g.G) {
+        uint64_t Lp[4]; uint32_t sd[4], who[4]; bool bit[4];
 #pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) {
-                const int c = (int)ROW_BYTE(w, d);
-                const uint64_t step = d < sm.n ? (uint64_t)delta * sm.stride[d] : 0;
-                const bool okm = d < sm.n && c >= delta, okp = d < sm.n && c + delta < (int)sm.m[d];
-                cand[2 * d] = okm ? L - step : L;  cand[2 * d + 1] = okp ? L + step : L;
-                hit[2 * d] = okm;                  hit[2 * d + 1] = okp;
-            }
-#pragma unroll
-            for (int e = 0; e < ROWW * 8; ++e) hit[e] = hit[e] && bit_test(sm.bitmap, cand[e]);
-#pragma unroll
-            for (int e = 0; e < ROWW * 8; ++e) if (hit[e] && cand[e] < bestL) bestL = cand[e];
-        } else {                                                        // few dimensions are this wide
-            for (int d = 0; d < sm.n; ++d) {
-                if ((int)sm.m[d] <= delta) continue;
-                const int c = (int)ROW_BYTE(w, d);
-                const uint64_t step = (uint64_t)delta * sm.stride[d];
-                if (c >= delta && bit_test(sm.bitmap, L - step) && L - step < bestL) bestL = L - step;
-                if (c + delta < (int)sm.m[d] && bit_test(sm.bitmap, L + step) && L + step < bestL) bestL = L + step;
-            }
+        for (int u = 0; u < 4; ++u) {
+            const bool live = q0 + u * g.G < total;
+            const uint32_t i2 = ol[live ? jj : 0], e = tb.nb[live ? t : 0], d = e >> 8, kq = e & 255u, cd = rows8[(size_t)i2 * RB + d];
+            const int dv = (int)(kq + (kq >= cd)) - (int)cd;
+            Lp[u] = Lc[i2] + (int64_t)dv * (int64_t)tb.stride[d];
+            sd[u] = (uint32_t)abs(dv); who[u] = i2;
+            bit[u] = bit_test(bitmap, Lp[u]) && live;
+            t += st; jj += sj;
+            if (t >= NB) { t -= NB; ++jj; }
         }
-        if (bestL != ~0ull) return make_key(1u, (uint32_t)delta, rank_of(sm, bestL));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (bit[u]) atomicMin(&hkey[who[u]], (unsigned long long)(((uint64_t)sd[u] << 40) | Lp[u]));
     }
-    return CAO_KEY_NONE;
-}
-
-// ---------------------------------------------------------------------------------------------
-// Group-cooperative Hamming-2/3 probe of ONE candidate (row in shared memory, s_cw).  *slot must be ~0 and visible to
-// the group on entry.  Returns the level that found a valid neighbour (0 = none), group-uniform, and leaves
-// (sad << 40 | L') in *slot.  tgt / pairs may point to shared or global memory.
-template <int ROWW>
-__device__ __forceinline__ int probe23_grp(const Grp& g, const SpaceMeta& sm, const ProbeMeta& pm, const uint16_t* tgt,
-                                           const uint32_t* pairs, const uint32_t* s_cw, unsigned long long* slot) {
-    const uint8_t* c = (const uint8_t*)s_cw;
-    const uint32_t T = pm.T, C2 = pm.C2;
-    uint64_t L = 0;
-    for (int d = 0; d < sm.n; ++d) L += (uint64_t)c[d] * sm.stride[d];
-    for (int level = 2; level <= pm.levels; ++level) {
-        uint64_t best = ~0ull;
-        for (uint32_t q = g.t; q < C2; q += g.G) {
-            const uint32_t pr = pairs[q];
-            const uint32_t e1 = tgt[pr & 0xFFFFu], e2 = tgt[pr >> 16];
-            const uint32_t d1 = e1 >> 8, d2 = e2 >> 8;
-            const int dv1 = (int)(e1 & 255) - (int)c[d1], dv2 = (int)(e2 & 255) - (int)c[d2];
-            if (dv1 == 0 || dv2 == 0) continue;
-            const uint64_t L2 = L + (int64_t)dv1 * (int64_t)sm.stride[d1] + (int64_t)dv2 * (int64_t)sm.stride[d2];
-            const uint32_t s2 = (uint32_t)(abs(dv1) + abs(dv2));
-            if (level == 2) {
-                if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)s2 << 40) | L2; best = k < best ? k : best; }
-            } else {
-#pragma unroll 8
-                for (uint32_t t3 = pm.dim_first[d2 + 1]; t3 < T; ++t3) {
-                    const uint32_t e3 = tgt[t3], d3 = e3 >> 8;
-                    const int dv3 = (int)(e3 & 255) - (int)c[d3];
-                    const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
-                    const bool bit3 = bit_test(sm.bitmap, L3);              // unconditional: dv3 == 0 re-reads L2 (a legal index)
-                    if (dv3 != 0 && bit3) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
-                }
-            }
-        }
-        grp_min_key(g, best, slot);                                     // barrier inside
-        const bool found = *slot != ~0ull;
-        g.sync();                                                       // everyone has read the slot before the next level writes it
-        if (found) return level;
-    }
-    return 0;
 }
 
 // Group-cooperative brute-force scan of the whole valid table for up to NB candidates (rows in shared memory); the
 // table rows come straight from L2, coalesced, RU rows in flight per thread.  s_key[b] must be ~0 on entry; on exit it
 // holds ham << 45 | sad << 32 | rank.  Ends with a barrier.
 template <int ROWW, int NB>
-__device__ __forceinline__ void scan_grp(const Grp& g, const SpaceMeta& sm, const uint32_t* s_cw, int nb, unsigned long long* s_key) {
+static __device__ __noinline__ void scan_grp(const Grp g, const uint8_t* __restrict__ rows, uint32_t V, const uint32_t* s_cw, int nb,
+                                             unsigned long long* s_key) {
     uint32_t c[NB][ROWW];
 #pragma unroll
     for (int b = 0; b < NB; ++b)
@@ -163,18 +102,18 @@ __device__ __forceinline__ void scan_grp(const Grp& g, const SpaceMeta& sm, cons
     uint64_t best[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) best[b] = ~0ull;
-    constexpr int RU = ROWW == 4 ? 8 : 4;
-    for (uint32_t r0 = g.t; r0 < sm.V; r0 += RU * g.G) {
+    constexpr int RU = ROWW == 4 ? 4 : 2;
+    for (uint32_t r0 = g.t; r0 < V; r0 += RU * g.G) {
         uint32_t v[RU][ROWW];
 #pragma unroll
         for (int u = 0; u < RU; ++u) {
             const uint32_t r = r0 + u * g.G;
-            load_row<ROWW>(sm.rows + (uint64_t)(r < sm.V ? r : r0) * (ROWW * 4), v[u]);
+            load_row<ROWW>(rows + (uint64_t)(r < V ? r : r0) * (ROWW * 4), v[u]);
         }
 #pragma unroll
         for (int u = 0; u < RU; ++u) {
             const uint32_t r = r0 + u * g.G;
-            if (r >= sm.V) break;
+            if (r >= V) break;
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 uint32_t sad = 0, ham = 0;
@@ -203,11 +142,12 @@ struct GrpMem {
     GrpShared* gs;
     uint32_t* rank; float* f; uint32_t* idx; float* x; float* v; float* pb; float* pbf;
     uint32_t* cand; unsigned long long* key; uint32_t* scr; uint32_t* wl; uint32_t* cw; unsigned long long* skey;
-    uint32_t* bestrow;
+    uint32_t* bestrow; uint64_t* Lc; uint32_t* aux4;
     __device__ __forceinline__ GrpMem(uint32_t* S, const GenLayout& l)
         : gs((GrpShared*)S), rank(S + l.rank), f((float*)(S + l.f)), idx(S + l.idx), x((float*)(S + l.x)), v((float*)(S + l.v)),
           pb((float*)(S + l.pb)), pbf((float*)(S + l.pbf)), cand(S + l.cand), key((unsigned long long*)(S + l.key)),
-          scr(S + l.scr), wl(S + l.wl), cw(S + l.cw), skey((unsigned long long*)(S + l.skey)), bestrow(S + l.bestrow) {}
+          scr(S + l.scr), wl(S + l.wl), cw(S + l.cw), skey((unsigned long long*)(S + l.skey)), bestrow(S + l.bestrow),
+          Lc((uint64_t*)(S + l.Lc)), aux4(S + l.aux4) {}
 };
 
 // O10: evaluate rank rk for run k.  Returns f; *is_new = this evaluation set the run's memo bit (L268).
@@ -231,7 +171,7 @@ __device__ __forceinline__ void fold_eval(const Grp& g, GrpShared* gs, bool has,
 // O4 inside the fused kernel (DE stagnation re-initialisation, L266): P distinct valid ranks, uniform with linear
 // probing; fills the shared-memory population and evaluates it.  Group-uniform call, ends with a barrier.
 template <int ROWW>
-__device__ void reinit_de_grp(const Grp& g, const SpaceMeta& sm, const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen) {
+static __device__ __noinline__ void reinit_de_grp(const Grp g, const SpaceMeta& sm, const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen) {
     const uint32_t i = g.t, P = rm.P, run = rm.first_run + k;
     uint32_t* s_r = S.scr;
     Draws dr(rm.seed, run, gen, i, S_REINIT);
@@ -279,6 +219,7 @@ __device__ __forceinline__ void load_state(const Grp& g, const SpaceMeta& sm, co
         S.key[i] = CAO_KEY_NONE;                                         // the memo starts empty (it is only a shortcut)
         if (ALGO == CAO_PSO) S.pbf[i] = rm.pbf[q0 + i];
     }
+    for (uint32_t e = g.t; e < P * ROWW; e += g.G) S.cand[e] = 0;       // padding bytes of the candidate rows stay zero
     if (ALGO == CAO_DE || ALGO == CAO_GA) {
         const uint32_t* src = (const uint32_t*)(rm.idx + q0 * (ROWW * 4));
         for (uint32_t e = g.t; e < P * ROWW; e += g.G) S.idx[e] = src[e];
@@ -295,6 +236,8 @@ __device__ __forceinline__ void load_state(const Grp& g, const SpaceMeta& sm, co
         gs->best = br == 0xFFFFFFFFu ? ~0ull : (((unsigned long long)fbits(rm.best_f[k]) << 32) | br);
         gs->uniq = rm.uniq[k]; gs->stagn = rm.stagn[k]; gs->bestrow_rank = 0xFFFFFFFFu;
         gs->n_inv = 0; gs->n_scan = 0; gs->n_eval = 0; gs->gens = 0;
+        gs->n_p2 = 0; gs->n_p3 = 0; gs->n_memo = 0; gs->n_rc = 0;
+        for (int z = 0; z < 6; ++z) gs->cyc[z] = 0;
     }
     g.sync();
 }
@@ -324,200 +267,218 @@ __device__ __forceinline__ void store_state(const Grp& g, const SpaceMeta& sm, c
         if (gs->n_inv) atomicAdd(&rm.counters[0], (unsigned long long)gs->n_inv);
         if (gs->n_scan) atomicAdd(&rm.counters[1], (unsigned long long)gs->n_scan);
         if (gs->n_eval) atomicAdd(&rm.counters[2], (unsigned long long)gs->n_eval);
+        if (gs->n_p2) atomicAdd(&rm.counters[3], (unsigned long long)gs->n_p2);
+        if (gs->n_p3) atomicAdd(&rm.counters[4], (unsigned long long)gs->n_p3);
+        if (gs->n_memo) atomicAdd(&rm.counters[5], (unsigned long long)gs->n_memo);
+        if (gs->n_rc) atomicAdd(&rm.counters[6], (unsigned long long)gs->n_rc);
+#ifdef CAO_GEN_STATS
+        unsigned long long tot = 0;
+        for (int z = 0; z < 6; ++z) { atomicAdd(&rm.counters[8 + z], gs->cyc[z]); tot += gs->cyc[z]; }
+        atomicMax(&rm.counters[14], tot);                               // slowest run (cycles)
+        atomicMax(&rm.counters[15], gs->cyc[4]);                        // most scan cycles in one run
+#endif
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// One generation g of run k, state in shared memory.  last = write the parity taps of this generation.
+// One generation `gen` of run k, state in shared memory.  last = write the parity taps of this generation.
+// Dimension loops are runtime loops over bytes in shared memory (compact code: the kernel is bound by instruction
+// issue and instruction fetch, not by memory).
 template <int ALGO, int ROWW>
-__device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, const ProbeMeta& pm, const uint16_t* tgt,
-                                           const uint32_t* pairs, const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen, bool last) {
+__device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, const ProbeMeta& pm, const CtaTabs& tb,
+                                           const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen, bool last) {
+    constexpr int RB = ROWW * 4;
     const uint32_t i = g.t, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
+    const bool has = i < P;
     GrpShared* gs = S.gs;
-    uint32_t w[ROWW];
-#pragma unroll
-    for (int z = 0; z < ROWW; ++z) w[z] = 0;
+    uint8_t* cand8 = (uint8_t*)S.cand + (size_t)i * RB;                 // this thread's candidate row
+    const uint8_t* idx8 = (const uint8_t*)S.idx;
     Draws dr(rm.seed, run, gen, i, S_OP);
-    if (i == 0) { gs->n_new = 0; gs->nwl = 0; gs->aux = ~0ull; }
+    if (i == 0) { gs->n_new = 0; gs->nwl = 0; gs->aux = ~0ull; gs->flag = 0; }
+#ifdef CAO_GEN_STATS
+    long long t_mark = clock64();
+#endif
+    // memo of the previous generation: repair is a pure function of the row, so a candidate that repeats keeps its key
+    uint64_t L = 0;
+    bool same = has && S.key[has ? i : 0] != CAO_KEY_NONE;
+#define PUT_DIM(d, ud)                                                                     \
+    do {                                                                                   \
+        const uint32_t ud_ = (ud);                                                         \
+        same = same && cand8[d] == ud_;                                                    \
+        cand8[d] = (uint8_t)ud_;                                                           \
+        L += (uint64_t)ud_ * sm.stride[d];                                                 \
+    } while (0)
 
     // ---- S3: operator
     if (ALGO == CAO_DE) {                                               // O5: best1bin on indices
         const uint32_t br = (uint32_t)gs->best;                         // best-so-far at generation start (A6)
         if (gs->bestrow_rank != br) {                                   // group-uniform
             g.sync();
-            if (i < ROWW) S.bestrow[i] = ((const uint32_t*)(sm.rows + (uint64_t)br * (ROWW * 4)))[i];
+            if (i < ROWW) S.bestrow[i] = ((const uint32_t*)(sm.rows + (uint64_t)br * RB))[i];
             if (i == 0) gs->bestrow_rank = br;
         }
         g.sync();
-        if (i < P) {
+        if (has) {
             uint32_t a = below(dr(0), P - 1); if (a >= i) a += 1;
             uint32_t b = below(dr(1), P - 2);
             const uint32_t lo = min(i, a), hi = max(i, a);
             if (b >= lo) b += 1;
             if (b >= hi) b += 1;
             const uint32_t jrand = below(dr(2), (uint32_t)n);
-            uint32_t wa[ROWW], wb[ROWW], wx[ROWW], wbest[ROWW];
-#pragma unroll
-            for (int z = 0; z < ROWW; ++z) { wa[z] = S.idx[a * ROWW + z]; wb[z] = S.idx[b * ROWW + z]; wx[z] = S.idx[i * ROWW + z]; wbest[z] = S.bestrow[z]; }
-#pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) {
-                if (d < n) {
-                    const int vd = de_mutate_index(rm.hp.de_F, (int)ROW_BYTE(wbest, d), (int)ROW_BYTE(wa, d), (int)ROW_BYTE(wb, d),
-                                                   (int)sm.m[d] - 1);
-                    const float rr = u01(dr(3 + d));
-                    const uint32_t ud = (rr < rm.hp.de_CR || (uint32_t)d == jrand) ? (uint32_t)vd : ROW_BYTE(wx, d);
-                    w[d >> 2] |= ud << ((d & 3) * 8);
-                }
+            const uint8_t* ra = idx8 + (size_t)a * RB; const uint8_t* rb = idx8 + (size_t)b * RB;
+            const uint8_t* rx = idx8 + (size_t)i * RB; const uint8_t* rbest = (const uint8_t*)S.bestrow;
+#pragma unroll 2
+            for (int d = 0; d < n; ++d) {
+                const int vd = de_mutate_index(rm.hp.de_F, (int)rbest[d], (int)ra[d], (int)rb[d], (int)sm.m[d] - 1);
+                const float rr = u01(dr(3 + d));
+                PUT_DIM(d, (rr < rm.hp.de_CR || (uint32_t)d == jrand) ? (uint32_t)vd : (uint32_t)rx[d]);
             }
         }
     } else if (ALGO == CAO_GA) {                                        // O8: sorted population, Beta(1,b) parents, single point
         unsigned long long* s_key = (unsigned long long*)S.scr;         // P keys
         uint32_t* s_order = S.scr + 2 * P;                              // P
         g.sync();
-        if (i < P) s_key[i] = ((unsigned long long)fbits(S.f[i]) << 32) | S.rank[i];
+        if (has) s_key[i] = ((unsigned long long)fbits(S.f[i]) << 32) | S.rank[i];
         g.sync();
-        if (i < P) {
+        if (has) {
             const unsigned long long me = s_key[i];
             uint32_t pos = 0;
             for (uint32_t j = 0; j < P; ++j) { const unsigned long long o = s_key[j]; pos += (o < me) || (o == me && j < i); }
             s_order[pos] = i;
         }
         g.sync();
-        if (i < P) {
+        if (has) {
             const uint32_t B = (uint32_t)rm.hp.ga_beta_b;
             uint32_t sa = P, sb = P;
             for (uint32_t z = 0; z < B; ++z) sa = min(sa, below(dr(z), P));
             for (uint32_t z = 0; z < B; ++z) sb = min(sb, below(dr(B + z), P));
             if (sb == sa) sb = sa + 1 == P ? 0 : sa + 1;
             const int cut = n > 1 ? 1 + (int)below(dr(2 * B), (uint32_t)(n - 1)) : 1;
-            const uint32_t pa = s_order[sa], pbq = s_order[sb];
-            uint32_t wa[ROWW], wb[ROWW];
-#pragma unroll
-            for (int z = 0; z < ROWW; ++z) { wa[z] = S.idx[pa * ROWW + z]; wb[z] = S.idx[pbq * ROWW + z]; }
-#pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d)
-                if (d < n) w[d >> 2] |= (d < cut ? ROW_BYTE(wa, d) : ROW_BYTE(wb, d)) << ((d & 3) * 8);
+            const uint8_t* ra = idx8 + (size_t)s_order[sa] * RB; const uint8_t* rb = idx8 + (size_t)s_order[sb] * RB;
+#pragma unroll 2
+            for (int d = 0; d < n; ++d) PUT_DIM(d, d < cut ? (uint32_t)ra[d] : (uint32_t)rb[d]);
         }
         g.sync();                                                       // every parent row is read before the population is replaced
     } else if (ALGO == CAO_PSO) {                                       // O6
         g.sync();
-        grp_min_key(g, i < P ? (((uint64_t)fbits(S.pbf[i]) << 32) | i) : ~0ull, &gs->aux);
-        const uint32_t gb = (uint32_t)gs->aux;
-        float gbest[ROWW * 4];
-#pragma unroll
-        for (int d = 0; d < ROWW * 4; ++d) gbest[d] = d < n ? S.pb[d * P + gb] : 0.0f;
-        g.sync();                                                       // gbest is read before any pbest moves (finish phase)
-        if (i < P) {
-#pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) {
-                if (d < n) {
-                    const uint32_t e = d * P + i;
-                    const float hi = coord_M(sm.M, (int)sm.m[d] - 1);
-                    const float r1 = u01(dr(2 * d)), r2 = u01(dr(2 * d + 1));
-                    const float xq = S.x[e], pbq = S.pb[e];
-                    const float a = __fmul_rn(rm.hp.pso_c1, r1);
-                    const float b = __fsub_rn(pbq, xq);
-                    const float t1 = __fmul_rn(a, b);
-                    const float c = __fmul_rn(rm.hp.pso_c2, r2);
-                    const float ee = __fsub_rn(gbest[d], xq);
-                    const float t2 = __fmul_rn(c, ee);
-                    float vv = __fmul_rn(rm.hp.pso_w, S.v[e]);
-                    vv = __fadd_rn(vv, t1);
-                    vv = __fadd_rn(vv, t2);
-                    float xx = __fadd_rn(xq, vv);
-                    xx = clamp_pos(xx, hi);
-                    S.v[e] = vv; S.x[e] = xx;
-                    w[d >> 2] |= (uint32_t)snap_M(sm.M, (int)sm.m[d], xx) << ((d & 3) * 8);
-                }
+        grp_min_key(g, has ? (((uint64_t)fbits(S.pbf[i]) << 32) | i) : ~0ull, &gs->aux);
+        const uint32_t gb = (uint32_t)gs->aux;                          // gbest = pbest of argmin (pbest_f, i) at generation start
+        if (has) {
+            const float fM = (float)(sm.M - 1);
+#pragma unroll 2
+            for (int d = 0; d < n; ++d) {
+                const uint32_t e = d * P + i;
+                const float r1 = u01(dr(2 * d)), r2 = u01(dr(2 * d + 1));
+                const float xq = S.x[e], pbq = S.pb[e], gbq = S.pb[d * P + gb];
+                const float a = __fmul_rn(rm.hp.pso_c1, r1);
+                const float b = __fsub_rn(pbq, xq);
+                const float t1 = __fmul_rn(a, b);
+                const float c = __fmul_rn(rm.hp.pso_c2, r2);
+                const float ee = __fsub_rn(gbq, xq);
+                const float t2 = __fmul_rn(c, ee);
+                float vv = __fmul_rn(rm.hp.pso_w, S.v[e]);
+                vv = __fadd_rn(vv, t1);
+                vv = __fadd_rn(vv, t2);
+                float xx = __fadd_rn(xq, vv);
+                xx = clamp_pos(xx, tb.hi[d]);
+                S.v[e] = vv; S.x[e] = xx;
+                int kq = __float2int_rn(__fmul_rn(xx, fM));             // snap (O6, A11)
+                kq = min(max(kq, 0), (int)sm.m[d] - 1);
+                PUT_DIM(d, (uint32_t)kq);
             }
         }
     } else {                                                            // O7: Firefly (Yang's rule, synchronous)
         g.sync();
-        float xi[ROWW * 4];
-        if (i < P) {
+        float xi[RB];
+        if (has) {
 #pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) xi[d] = d < n ? S.x[i * n + d] : 0.0f;
-            const float fi = S.f[i];
-            for (uint32_t j = 0; j < P; ++j) {
-                if (!(S.f[j] < fi)) continue;                           // only brighter (cheaper) fireflies attract
-                const float* xj = S.x + (size_t)j * n;
-                float r2 = 0.0f;
+            for (int d = 0; d < RB; ++d) xi[d] = d < n ? S.x[i * n + d] : 0.0f;
+        }
+        const float fi = has ? S.f[i] : 0.0f;
+        for (uint32_t j = 0; j < P; ++j) {
+            const bool brighter = has && S.f[j] < fi;                   // only brighter (cheaper) fireflies attract
+            if (!__any_sync(0xFFFFFFFFu, brighter)) continue;           // warp-uniform: draws are addressed by slot, skipping is free
+            const float* xj = S.x + (size_t)j * n;
+            float r2 = 0.0f;
 #pragma unroll
-                for (int d = 0; d < ROWW * 4; ++d)
-                    if (d < n) { const float df = __fsub_rn(xj[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
-                const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
-                // the n noise draws of this j are slots j*n .. j*n+n-1: their Philox blocks are computed up front as
-                // independent chains, then word (o + d) is picked with selects (o = first slot & 3)
-                const uint32_t s0 = j * (uint32_t)n, b0 = s0 >> 2, o = s0 & 3;
-                uint32_t nw[(ROWW + 1) * 4];
+            for (int d = 0; d < RB; ++d)
+                if (d < n) { const float df = __fsub_rn(xj[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
+            const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
+            const uint32_t s0 = j * (uint32_t)n;                        // noise slots j*n .. j*n+n-1, walked in order (cached blocks)
 #pragma unroll
-                for (int qb = 0; qb < ROWW + 1; ++qb) {
-                    uint4 rr = make_uint4(0, 0, 0, 0);
-                    if ((uint32_t)(qb * 4) < o + (uint32_t)n)
-                        rr = philox4x32_10(make_uint4(run, gen, i, (S_OP << 24) | (b0 + qb)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
-                    nw[qb * 4] = rr.x; nw[qb * 4 + 1] = rr.y; nw[qb * 4 + 2] = rr.z; nw[qb * 4 + 3] = rr.w;
-                }
-#pragma unroll
-                for (int d = 0; d < ROWW * 4; ++d) {
-                    if (d < n) {
-                        const uint32_t lo = (o & 1) ? nw[d + 1] : nw[d], hi = (o & 1) ? nw[d + 3] : nw[d + 2];
-                        const uint32_t word = (o & 2) ? hi : lo;
-                        const float df = __fsub_rn(xj[d], xi[d]);
-                        xi[d] = __fadd_rn(xi[d], __fmul_rn(beta, df));
-                        const float e = __fsub_rn(u01(word), 0.5f);
-                        xi[d] = __fadd_rn(xi[d], __fmul_rn(rm.hp.ff_alpha, e));
-                    }
-                }
-            }
-#pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) {
+            for (int d = 0; d < RB; ++d) {
                 if (d < n) {
-                    xi[d] = clamp_pos(xi[d], coord_M(sm.M, (int)sm.m[d] - 1));
-                    w[d >> 2] |= (uint32_t)snap_M(sm.M, (int)sm.m[d], xi[d]) << ((d & 3) * 8);
+                    const uint32_t word = dr(s0 + d);
+                    const float df = __fsub_rn(xj[d], xi[d]);
+                    float t = __fadd_rn(xi[d], __fmul_rn(beta, df));
+                    const float e = __fsub_rn(u01(word), 0.5f);
+                    t = __fadd_rn(t, __fmul_rn(rm.hp.ff_alpha, e));
+                    xi[d] = brighter ? t : xi[d];
                 }
             }
         }
         g.sync();                                                       // all start-of-generation positions are consumed
-        if (i < P) {
+        if (has) {
+            const float fM = (float)(sm.M - 1);
 #pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) if (d < n) S.x[i * n + d] = xi[d];
-        }
-    }
-
-    // ---- S4 + first part of S5: memo of the previous generation, validity, Hamming-1 probe, per-run repair cache
-    uint64_t key = CAO_KEY_NONE;
-    bool valid = false;
-    uint64_t L = 0;
-    if (i < P) {
-        const uint64_t prev_key = S.key[i];
-        bool same = prev_key != CAO_KEY_NONE;
-#pragma unroll
-        for (int z = 0; z < ROWW; ++z) same = same && S.cand[i * ROWW + z] == w[z];
-        if (same) {
-            key = prev_key; valid = (key >> 45) == 0;
-        } else {
-#pragma unroll
-            for (int z = 0; z < ROWW; ++z) S.cand[i * ROWW + z] = w[z];
-            L = row_lin<ROWW>(sm, w);                                   // operator outputs are in-domain by construction
-            const uint32_t rk0 = valid_rank(sm, L, valid);
-            if (valid) key = make_key(0, 0, rk0);
-            else {
-                if (pm.levels >= 1) key = probe_h1_v2<ROWW>(sm, w, L);
-                if (key == CAO_KEY_NONE) {                              // memoised repairs of this run (L268 in spirit)
-                    const ulonglong2 e = rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)];
-                    if (e.x == L) key = e.y;
+            for (int d = 0; d < RB; ++d) {
+                if (d < n) {
+                    const float xx = clamp_pos(xi[d], tb.hi[d]);
+                    S.x[i * n + d] = xx;
+                    int kq = __float2int_rn(__fmul_rn(xx, fM));
+                    kq = min(max(kq, 0), (int)sm.m[d] - 1);
+                    PUT_DIM(d, (uint32_t)kq);
                 }
             }
-            S.key[i] = key;
         }
-        if (key == CAO_KEY_NONE) S.wl[atomicAdd(&gs->nwl, 1u)] = i;
     }
+#undef PUT_DIM
+    CAO_TICK(0);
+
+    // ---- S4 + first part of S5: validity, warp-cooperative Hamming-1 probe, per-run repair cache
+    uint64_t key = CAO_KEY_NONE;
+    uint32_t valid = 0;
+    if (has) {
+        if (same) {
+            key = S.key[i]; valid = (key >> 45) == 0;
+            if (!valid) atomicAdd(&gs->n_memo, 1u);
+        } else {
+            const uint32_t rk0 = valid_rank(sm.bitmap, sm.dir, L, &valid);   // operator outputs are in-domain by construction
+            if (valid) key = make_key(0, 0, rk0);
+        }
+    }
+    const bool open = has && !same && !valid;
+    if (pm.levels >= 1) {
+        unsigned long long* hkey = (unsigned long long*)S.aux4;
+        uint32_t* ol = S.scr;
+        if (open) { ol[atomicAdd(&gs->flag, 1u)] = i; S.Lc[i] = L; hkey[i] = ~0ull; }
+        g.sync();                                                       // candidate rows, list and linear indices are visible
+        const uint32_t nopen = gs->flag;
+        if (nopen) {
+            probe_h1_flat<RB>(g, sm.bitmap, tb, (const uint8_t*)S.cand, ol, S.Lc, hkey, nopen);
+            g.sync();
+            if (open) {
+                const uint64_t hit = hkey[i];
+                if (hit != ~0ull) {
+                    uint32_t dummy;
+                    key = make_key(1u, (uint32_t)(hit >> 40), valid_rank(sm.bitmap, sm.dir, hit & ((1ull << 40) - 1), &dummy));
+                }
+            }
+        }
+    }
+    if (open && key == CAO_KEY_NONE) {                                  // memoised repairs of this run (L268 in spirit)
+        const ulonglong2 e = rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)];
+        if (e.x == L) { key = e.y; atomicAdd(&gs->n_rc, 1u); }
+    }
+    if (has && !same) S.key[i] = key;
+    if (has && key == CAO_KEY_NONE) S.wl[atomicAdd(&gs->nwl, 1u)] = i;
     {
-        const uint32_t ninv = __popc(__ballot_sync(0xFFFFFFFFu, i < P && !valid));
+        const uint32_t ninv = __popc(__ballot_sync(0xFFFFFFFFu, has && !valid));
         if ((i & 31) == 0 && ninv) atomicAdd(&gs->n_inv, ninv);
     }
     g.sync();
+    CAO_TICK(1);
 
     // ---- rest of S5: the few unresolved candidates, by the whole group (Hamming-2/3 probes, then the table scan)
     const uint32_t nwl = gs->nwl;
@@ -526,17 +487,21 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
         if (pm.levels >= 2) {
             for (uint32_t fq = 0; fq < nwl; ++fq) {
                 const uint32_t slot = S.wl[fq];
-                if (i < ROWW) S.cw[i] = S.cand[slot * ROWW + i];
+                const uint8_t* c = (const uint8_t*)S.cand + (size_t)slot * RB;
                 if (i == 0) gs->aux = ~0ull;
                 g.sync();
-                const int found = probe23_grp<ROWW>(g, sm, pm, tgt, pairs, S.cw, &gs->aux);
+                const int found = probe_levels_grp(g, sm.bitmap, tb.stride, n, pm, tb.nb, tb.pairs, c, &gs->aux);
+                if (found == 2) CAO_TICK(2); else CAO_TICK(3);
                 if (i == 0) {
+                    gs->n_p2 += 1; gs->n_p3 += found != 2 && pm.levels >= 3;   // went to the Hamming-2 probe / beyond it
                     if (found) {
                         const uint64_t best = gs->aux;
-                        const uint64_t kk = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));
+                        uint32_t dummy;
+                        const uint64_t kk = make_key((uint32_t)found, (uint32_t)(best >> 40),
+                                                     valid_rank(sm.bitmap, sm.dir, best & ((1ull << 40) - 1), &dummy));
                         S.key[slot] = kk;
                         uint64_t Lc = 0;
-                        for (int d = 0; d < n; ++d) Lc += (uint64_t)((const uint8_t*)S.cw)[d] * sm.stride[d];
+                        for (int d = 0; d < n; ++d) Lc += (uint64_t)c[d] * tb.stride[d];
                         rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(Lc)] = make_ulonglong2(Lc, kk);
                     } else {
                         S.wl[nscan] = slot;                             // nscan <= fq: compacts in place
@@ -553,118 +518,199 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             for (uint32_t e = i; e < nb * ROWW; e += g.G) S.cw[e] = S.cand[S.wl[f0 + e / ROWW] * ROWW + e % ROWW];
             if (i < GEN_NB) S.skey[i] = ~0ull;
             g.sync();
-            if (nb == 1) scan_grp<ROWW, 1>(g, sm, S.cw, 1, S.skey);
-            else scan_grp<ROWW, GEN_NB>(g, sm, S.cw, (int)nb, S.skey);
+            scan_grp<ROWW, GEN_NB>(g, sm.rows, sm.V, S.cw, (int)nb, S.skey);
             if (i == 0) {                                               // one writer: cache entries are never torn
                 for (uint32_t b = 0; b < nb; ++b) {
                     const uint64_t kk = S.skey[b];
                     S.key[S.wl[f0 + b]] = kk;
                     uint64_t Lc = 0;
-                    for (int d = 0; d < n; ++d) Lc += (uint64_t)((const uint8_t*)(S.cw + b * ROWW))[d] * sm.stride[d];
+                    for (int d = 0; d < n; ++d) Lc += (uint64_t)((const uint8_t*)(S.cw + b * ROWW))[d] * tb.stride[d];
                     rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(Lc)] = make_ulonglong2(Lc, kk);
                 }
             }
             g.sync();
         }
         if (i == 0 && nscan) gs->n_scan += nscan;
-        key = i < P ? S.key[i] : key;
+        key = has ? S.key[i] : key;
+        CAO_TICK(4);
     }
 
     // ---- S6 + S7
     uint32_t rk = (uint32_t)key;
     const uint32_t rep = rk;
     float f = 0.0f; bool is_new = false;
-    uint32_t row[ROWW];
-    if (i < P) {
-        if (ALGO == CAO_GA) {                                           // L290, L311, L393: 1-in-X mutation after repair
-            Draws dm(rm.seed, run, gen, i, S_MUT);
-            if (below(dm(0), (uint32_t)rm.hp.ga_mutation_chance) == 0) {
-                uint32_t cur[ROWW];
-                load_row<ROWW>(sm.rows + (uint64_t)rk * (ROWW * 4), cur);
-                const uint64_t Lr = row_lin<ROWW>(sm, cur);
-                uint32_t K = 0;                                         // valid Hamming-1 neighbours, (d asc, value asc)
+    if (ALGO == CAO_GA) {                                               // L288: the children replace the population ...
+        uint64_t Lr = 0;
+        if (has) {
+            uint32_t row[ROWW];
+            load_row<ROWW>(sm.rows + (uint64_t)rk * RB, row);
+            Lr = __ldg(&sm.Ltab[rk]);
 #pragma unroll
-                for (int d = 0; d < ROWW * 4; ++d) {
-                    if (d < n) {
-                        const int c = (int)ROW_BYTE(cur, d);
-                        for (int val = 0; val < (int)sm.m[d]; ++val)
-                            if (val != c && bit_test(sm.bitmap, Lr + (int64_t)(val - c) * (int64_t)sm.stride[d])) ++K;
+            for (int z = 0; z < ROWW; ++z) S.idx[i * ROWW + z] = row[z];
+        }
+        // ... after the 1-in-X mutation into a uniformly drawn valid Hamming-1 neighbour (L290, L311, L393), listed in
+        // (dimension ascending, value ascending) order = neighbour-list order.  All neighbours of all mutating children
+        // are tested in one flat pass (bit masks in shared memory), then each child picks its own.
+        Draws dm(rm.seed, run, gen, i, S_MUT);
+        const bool mutate = has && below(dm(0), (uint32_t)rm.hp.ga_mutation_chance) == 0;
+        uint64_t Lnew = ~0ull;
+        const uint32_t MW = (tb.NB + 31) >> 5;                          // mask words per child
+        if (MW <= 4) {
+            uint32_t* ol = S.scr; uint32_t* mm = S.aux4;
+            if (i == 0) gs->flag = 0;
+            g.sync();
+            if (mutate) {
+                ol[atomicAdd(&gs->flag, 1u)] = i; S.Lc[i] = Lr;
+                for (uint32_t w = 0; w < MW; ++w) mm[i * 4 + w] = 0;
+            }
+            g.sync();
+            const uint32_t nmut = gs->flag, NB = tb.NB, total = nmut * NB;
+            if (nmut) {
+                uint32_t jj = g.t / NB, t = g.t - jj * NB;
+                const uint32_t sj = g.G / NB, st = g.G - sj * NB;
+                for (uint32_t q0 = g.t; q0 < total; q0 += 4 * g.G) {
+                    uint32_t who[4], tt[4]; bool bit[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const bool live = q0 + u * g.G < total;
+                        const uint32_t i2 = ol[live ? jj : 0], tq = live ? t : 0, e = tb.nb[tq], d = e >> 8, kq = e & 255u;
+                        const uint32_t cd = idx8[(size_t)i2 * RB + d];
+                        const int dv = (int)(kq + (kq >= cd)) - (int)cd;
+                        who[u] = i2; tt[u] = tq;
+                        bit[u] = bit_test(sm.bitmap, S.Lc[i2] + (int64_t)dv * (int64_t)tb.stride[d]) && live;
+                        t += st; jj += sj;
+                        if (t >= NB) { t -= NB; ++jj; }
                     }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) if (bit[u]) atomicOr(&mm[who[u] * 4 + (tt[u] >> 5)], 1u << (tt[u] & 31));
+                }
+                g.sync();
+                if (mutate) {
+                    uint32_t K = 0;
+                    for (uint32_t w = 0; w < MW; ++w) K += __popc(mm[i * 4 + w]);
+                    if (K) {
+                        uint32_t pick = below(dm(1), K), w = 0;
+                        for (; w < MW; ++w) { const uint32_t c2 = __popc(mm[i * 4 + w]); if (pick < c2) break; pick -= c2; }
+                        const uint32_t t2 = w * 32 + (uint32_t)kth_set_bit32(mm[i * 4 + w], pick);
+                        const uint32_t e = tb.nb[t2], d = e >> 8, kq = e & 255u, cd = idx8[(size_t)i * RB + d];
+                        const int dv = (int)(kq + (kq >= cd)) - (int)cd;
+                        Lnew = Lr + (int64_t)dv * (int64_t)tb.stride[d];
+                    }
+                }
+            }
+        } else {                                                        // very wide spaces: one child at a time, two passes
+            uint32_t todo = __ballot_sync(0xFFFFFFFFu, mutate);
+            const uint32_t lane = i & 31;
+            if (todo) __syncwarp();
+            while (todo) {
+                const int j = __ffs(todo) - 1;
+                todo &= todo - 1;
+                const uint64_t Lj = __shfl_sync(0xFFFFFFFFu, Lr, j);
+                const uint8_t* c = idx8 + (size_t)((i & ~31u) + j) * RB;
+                uint32_t K = 0;
+                for (uint32_t t0 = 0; t0 < tb.NB; t0 += 32) {           // pass 1: count
+                    const uint32_t t = t0 + lane;
+                    bool bit = false;
+                    if (t < tb.NB) {
+                        const uint32_t e = tb.nb[t], d = e >> 8, kq = e & 255u, cd = c[d];
+                        const int dv = (int)(kq + (kq >= cd)) - (int)cd;
+                        bit = bit_test(sm.bitmap, Lj + (int64_t)dv * (int64_t)tb.stride[d]);
+                    }
+                    K += __popc(__ballot_sync(0xFFFFFFFFu, bit));
                 }
                 if (K) {
-                    const uint32_t pick = below(dm(1), K); uint32_t seen = 0;
-                    uint64_t Lp = Lr; bool done = false;
-#pragma unroll
-                    for (int d = 0; d < ROWW * 4; ++d) {
-                        if (d < n && !done) {
-                            const int c = (int)ROW_BYTE(cur, d);
-                            for (int val = 0; val < (int)sm.m[d] && !done; ++val) {
-                                if (val == c) continue;
-                                const uint64_t L2 = Lr + (int64_t)(val - c) * (int64_t)sm.stride[d];
-                                if (bit_test(sm.bitmap, L2)) { if (seen == pick) { Lp = L2; done = true; } ++seen; }
-                            }
+                    uint32_t pick = below(__shfl_sync(0xFFFFFFFFu, dm(1), j), K);
+                    for (uint32_t t0 = 0; t0 < tb.NB; t0 += 32) {       // pass 2: the pick-th valid neighbour
+                        const uint32_t t = t0 + lane;
+                        bool bit = false; uint64_t Lp = 0;
+                        if (t < tb.NB) {
+                            const uint32_t e = tb.nb[t], d = e >> 8, kq = e & 255u, cd = c[d];
+                            const int dv = (int)(kq + (kq >= cd)) - (int)cd;
+                            Lp = Lj + (int64_t)dv * (int64_t)tb.stride[d];
+                            bit = bit_test(sm.bitmap, Lp);
                         }
+                        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, bit);
+                        const uint32_t cnt = __popc(bal);
+                        if (pick < cnt) {
+                            const int src = kth_set_bit32(bal, pick);
+                            const uint64_t Lsel = __shfl_sync(0xFFFFFFFFu, Lp, src);
+                            if ((int)lane == j) Lnew = Lsel;
+                            break;
+                        }
+                        pick -= cnt;
                     }
-                    rk = rank_of(sm, Lp);
                 }
             }
         }
-        f = evaluate_v2(sm, rm, k, rk, is_new);
-        if (ALGO == CAO_DE || ALGO == CAO_GA) load_row<ROWW>(sm.rows + (uint64_t)rk * (ROWW * 4), row);   // speculative for DE
-    }
-    fold_eval(g, gs, i < P, is_new, f, rk);
-
-    bool acc = false;
-    if (ALGO == CAO_DE) {                                               // Alg.1; A7
-        uint32_t* s_u = S.scr;                                          // P trial ranks; S.rank = old ranks
-        if (i < P) s_u[i] = rk;
-        g.sync();
-        if (i < P) {
-            acc = f <= S.f[i];
-            for (uint32_t j = 0; j < P && acc; ++j) if (S.rank[j] == rk) acc = false;
-            for (uint32_t j = 0; j < i && acc; ++j) if (s_u[j] == rk) acc = false;
-        }
-        const bool any = g.sync_or(acc);                                // barrier: all membership tests done before the updates
-        if (acc) {
+        if (has) {
+            if (Lnew != ~0ull) {
+                uint32_t dummy;
+                rk = valid_rank(sm.bitmap, sm.dir, Lnew, &dummy);
+                uint32_t row[ROWW];
+                load_row<ROWW>(sm.rows + (uint64_t)rk * RB, row);
 #pragma unroll
-            for (int z = 0; z < ROWW; ++z) S.idx[i * ROWW + z] = row[z];
-            S.f[i] = f; S.rank[i] = rk;
-        }
-        // L266: nothing accepted in two consecutive generations -> re-initialise (evaluated in this step)
-        const uint32_t st = any ? 0 : gs->stagn + 1;
-        g.sync();
-        if (st == 2) {
-            reinit_de_grp<ROWW>(g, sm, rm, S, k, gen);
-            if (i == 0) gs->n_eval += P;
-        }
-        if (i == 0) gs->stagn = st == 2 ? 0 : st;
-    } else if (ALGO == CAO_GA) {                                        // L288: the children replace the population
-        if (i < P) {
-#pragma unroll
-            for (int z = 0; z < ROWW; ++z) S.idx[i * ROWW + z] = row[z];
-            S.f[i] = f; S.rank[i] = rk;
-        }
-    } else if (ALGO == CAO_PSO) {                                       // L282: repair affects the evaluation only
-        if (i < P) {
-            S.f[i] = f; S.rank[i] = rk;
-            acc = f < S.pbf[i];                                         // strict (A13)
-            if (acc) {
-                S.pbf[i] = f;
-                for (int d = 0; d < n; ++d) S.pb[d * P + i] = S.x[d * P + i];
+                for (int z = 0; z < ROWW; ++z) S.idx[i * ROWW + z] = row[z];
             }
+            f = evaluate_v2(sm, rm, k, rk, is_new);
+            S.f[i] = f; S.rank[i] = rk;
         }
+        fold_eval(g, gs, has, is_new, f, rk);
     } else {
-        if (i < P) { S.f[i] = f; S.rank[i] = rk; }
+        uint32_t row[ROWW];
+        if (has) {
+            f = evaluate_v2(sm, rm, k, rk, is_new);
+            if (ALGO == CAO_DE) load_row<ROWW>(sm.rows + (uint64_t)rk * RB, row);   // speculative: only accepted trials keep it
+        }
+        fold_eval(g, gs, has, is_new, f, rk);
+        if (ALGO == CAO_DE) {                                           // Alg.1; A7
+            uint32_t* s_u = S.scr;                                      // P trial ranks; S.rank = old ranks
+            if (has) s_u[i] = rk;
+            g.sync();
+            bool acc = false;
+            if (has) {
+                acc = f <= S.f[i];
+                for (uint32_t j = 0; j < P && acc; ++j) if (S.rank[j] == rk) acc = false;
+                for (uint32_t j = 0; j < i && acc; ++j) if (s_u[j] == rk) acc = false;
+            }
+            const bool any = g.sync_or(acc);                            // barrier: all membership tests done before the updates
+            if (acc) {
+#pragma unroll
+                for (int z = 0; z < ROWW; ++z) S.idx[i * ROWW + z] = row[z];
+                S.f[i] = f; S.rank[i] = rk;
+            }
+            if (last && has) rm.accept[(uint64_t)k * P + i] = acc ? 1 : 0;
+            // L266: nothing accepted in two consecutive generations -> re-initialise (evaluated in this step)
+            const uint32_t st = any ? 0 : gs->stagn + 1;
+            g.sync();
+            if (st == 2) {
+                reinit_de_grp<ROWW>(g, sm, rm, S, k, gen);
+                if (i == 0) gs->n_eval += P;
+            }
+            if (i == 0) gs->stagn = st == 2 ? 0 : st;
+        } else if (ALGO == CAO_PSO) {                                   // L282: repair affects the evaluation only
+            if (has) {
+                S.f[i] = f; S.rank[i] = rk;
+                const bool acc = f < S.pbf[i];                          // strict (A13)
+                if (acc) {
+                    S.pbf[i] = f;
+                    for (int d = 0; d < n; ++d) S.pb[d * P + i] = S.x[d * P + i];
+                }
+                if (last) rm.accept[(uint64_t)k * P + i] = acc ? 1 : 0;
+            }
+        } else {
+            if (has) { S.f[i] = f; S.rank[i] = rk; }
+        }
     }
-    if (last && i < P) {                                                // parity taps of the last stepped generation
+    if (last && has) {                                                  // parity taps of the last stepped generation
         const uint64_t q = (uint64_t)k * P + i;
-        uint4* dst = (uint4*)(rm.cand + q * (ROWW * 4));
+        uint4* dst = (uint4*)(rm.cand + q * RB);
         dst[0] = make_uint4(S.cand[i * ROWW], S.cand[i * ROWW + 1], S.cand[i * ROWW + 2], S.cand[i * ROWW + 3]);
         if (ROWW == 8) dst[1] = make_uint4(S.cand[i * ROWW + 4], S.cand[i * ROWW + 5], S.cand[i * ROWW + 6], S.cand[i * ROWW + 7]);
         rm.key[q] = key; rm.valid[q] = (key >> 45) == 0 ? 1 : 0; rm.rep_rank[q] = rep; rm.eval_rank[q] = rk; rm.tap_f[q] = f;
-        rm.accept[q] = acc ? 1 : 0;
+        if (ALGO == CAO_GA || ALGO == CAO_FIREFLY) rm.accept[q] = 0;
     }
     g.sync();
+    CAO_TICK(5);
     if (i == 0) {                                                       // O10: trajectory row
         const uint32_t u = gs->uniq + gs->n_new;
         gs->uniq = u; gs->gens += 1; gs->n_eval += P;
@@ -676,18 +722,31 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
 
 // ---------------------------------------------------------------------------------------------
 template <int ALGO, int ROWW, int MAXT>
-__global__ void __launch_bounds__(MAXT) k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
-                                              const __grid_constant__ RunsMeta rm, const __grid_constant__ GenLayout lay,
-                                              uint32_t g_first, uint32_t n_gens) {
+__global__ void __launch_bounds__(MAXT, MAXT == 256 ? 3 : 1)
+k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm, const __grid_constant__ RunsMeta rm,
+      const __grid_constant__ GenLayout lay, uint32_t g_first, uint32_t n_gens) {
     extern __shared__ __align__(16) uint32_t s_dyn[];
-    // probe target / pair lists: CTA-wide copy in shared memory when they fit
-    const uint16_t* tgt = pm.tgt; const uint32_t* pairs = pm.pairs;
-    if (lay.cta_words) {
-        uint32_t* s_pairs = s_dyn;
-        uint16_t* s_tgt = (uint16_t*)(s_dyn + pm.C2);
-        for (uint32_t e = threadIdx.x; e < pm.C2; e += blockDim.x) s_pairs[e] = __ldg(&pm.pairs[e]);
-        for (uint32_t e = threadIdx.x; e < pm.T; e += blockDim.x) s_tgt[e] = __ldg(&pm.tgt[e]);
-        tgt = s_tgt; pairs = s_pairs;
+    // CTA-wide tables: strides, upper coordinates, Hamming-1 neighbour list, and (when they fit) the probe target / pair lists
+    CtaTabs tb;
+    {
+        uint64_t* s_stride = (uint64_t*)s_dyn;                          // CAO_MAX_DIMS
+        float* s_hi = (float*)(s_dyn + 2 * CAO_MAX_DIMS);               // CAO_MAX_DIMS
+        uint16_t* s_nb = (uint16_t*)(s_dyn + 3 * CAO_MAX_DIMS);         // lay.nb_words words
+        uint32_t* s_pairs = s_dyn + 3 * CAO_MAX_DIMS + lay.nb_words;
+        if (threadIdx.x < (uint32_t)sm.n) {
+            const uint32_t d = threadIdx.x;
+            s_stride[d] = sm.stride[d];
+            s_hi[d] = coord_M(sm.M, (int)sm.m[d] - 1);
+            uint32_t off = 0;
+            for (uint32_t e = 0; e < d; ++e) off += sm.m[e] - 1u;
+            for (uint32_t kq = 0; kq + 1 < sm.m[d]; ++kq) s_nb[off + kq] = (uint16_t)(d << 8 | kq);
+        }
+        tb.nb = s_nb; tb.stride = s_stride; tb.hi = s_hi; tb.NB = lay.NB;
+        tb.pairs = pm.pairs;
+        if (lay.probe_in_smem) {
+            for (uint32_t e = threadIdx.x; e < pm.C2; e += blockDim.x) s_pairs[e] = __ldg(&pm.pairs[e]);
+            tb.pairs = s_pairs;
+        }
         __syncthreads();
     }
     const Grp g{threadIdx.x % lay.G, lay.G, threadIdx.x / lay.G};
@@ -701,10 +760,11 @@ __global__ void __launch_bounds__(MAXT) k_gen(const __grid_constant__ SpaceMeta 
         if (k >= rm.R) break;
         load_state<ALGO, ROWW>(g, sm, rm, S, k);
         uint32_t gen = g_first + 1;
+#pragma unroll 1
         for (; gen <= g_last; ++gen) {
             const bool active = rm.budget == 0 || gs->uniq < rm.budget;  // O10 (gen <= max_gens is enforced by the host)
             if (!active) break;
-            generation<ALGO, ROWW>(g, sm, pm, tgt, pairs, rm, S, k, gen, gen == g_last);
+            generation<ALGO, ROWW>(g, sm, pm, tb, rm, S, k, gen, gen == g_last);
         }
         // a run that reached its budget stays frozen: its trajectory row repeats (O10)
         for (uint32_t q = gen + g.t; q <= g_last; q += g.G) {

@@ -62,7 +62,7 @@ struct cao_space {
     uint64_t off_rows = 0, off_Ltab = 0, off_dir = 0, off_tgt = 0, table_bytes = 0;
     // Hamming-level probes (S5)
     ProbeMeta probe{};
-    std::vector<uint16_t> h_tgt;
+    std::vector<uint16_t> h_nb;
     std::vector<uint32_t> h_pairs;
     uint64_t off_pairs = 0;
     int probe_levels_req = -1;         // -1 = cost model

@@ -57,78 +57,150 @@ __device__ __forceinline__ void worklist_push(uint32_t* wl, uint32_t* wl_count, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Hamming-2 / Hamming-3 probe of the worklist: one CTA per candidate.  All index rows at Hamming distance
-// exactly h are enumerated as h targets (dimension, value) of strictly increasing dimension; the outer
-// targets are walked by the whole warp, the innermost one is spread over the lanes.  Each probe is one bit
-// test at L + sum (v - c) * stride; the level minimum of (sum |v - c|, L') is exact because Hamming is the
-// primary key.  Candidates without a valid neighbour up to `levels` go on to the table scan (wl_out).
+// Thread groups: G threads (a multiple of 32) that synchronise among themselves -- __syncwarp() for one warp, a named
+// barrier otherwise.  The fused generation kernel runs several groups per CTA; the standalone probe kernel one.
+struct Grp {
+    uint32_t t, G, id;               // thread within the group, group size, group within the CTA
+    __device__ __forceinline__ void sync() const {
+        if (G == 32) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" ::"r"(id + 1), "r"(G) : "memory");
+    }
+    __device__ __forceinline__ bool sync_or(bool p) const {
+        if (G == 32) return __any_sync(0xFFFFFFFFu, p);
+        uint32_t r;
+        asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %1, 0;\n\tbar.red.or.pred q, %2, %3, p;\n\tselp.u32 %0, 1, 0, q;\n\t}"
+                     : "=r"(r) : "r"((uint32_t)p), "r"(id + 1), "r"(G) : "memory");
+        return r != 0;
+    }
+};
 __device__ __forceinline__ uint64_t warp_min_u64(uint64_t v) {
 #pragma unroll
     for (int o = 16; o; o >>= 1) { uint64_t t = __shfl_xor_sync(0xFFFFFFFFu, v, o); v = t < v ? t : v; }
     return v;
 }
+// Minimum of a 64-bit key over the warp: two REDUX on the halves (the high half decides, then the low half among the
+// lanes that hold the minimal high half).
+__device__ __forceinline__ uint64_t warp_min_key(uint64_t v) {
+    const uint32_t hi = (uint32_t)(v >> 32), lo = (uint32_t)v;
+    const uint32_t mh = __reduce_min_sync(0xFFFFFFFFu, hi);
+    const uint32_t ml = __reduce_min_sync(0xFFFFFFFFu, hi == mh ? lo : 0xFFFFFFFFu);
+    return ((uint64_t)mh << 32) | ml;
+}
+// Group-wide minimum into *slot (which must hold ~0 / a running minimum visible to the group); ends with a barrier.
+__device__ __forceinline__ void grp_min_key(const Grp& g, uint64_t v, unsigned long long* slot) {
+    const uint64_t m = warp_min_key(v);
+    if ((g.t & 31) == 0 && m != ~0ull) atomicMin(slot, (unsigned long long)m);
+    g.sync();
+}
 
-// Block-cooperative probe of ONE candidate whose row sits in shared memory (s_cw, ROWW words).  *s_best must be
-// ~0 and visible to the block on entry.  Threads walk the flattened list of target pairs (t1 < t2, different
-// dimensions); level 3 adds a serial walk over the targets of the dimensions after t2's.  Returns the level
-// that found a valid neighbour (0 = none) -- block-uniform -- and leaves (sad << 40 | L') in *s_best.
-template <int ROWW>
-__device__ __forceinline__ int probe23_cta(const SpaceMeta& sm, const ProbeMeta& pm, const uint32_t* s_cw,
-                                           unsigned long long* s_best) {
-    const uint8_t* c = (const uint8_t*)s_cw;
-    const uint32_t tid = threadIdx.x, T = pm.T, C2 = pm.C2;
+// Group-cooperative probe of ONE candidate c (n index bytes, in-domain) at Hamming levels 2 .. pm.levels, in turn.  A row
+// at Hamming distance exactly h is h neighbours (d, v != c_d) of strictly increasing dimension: the first two come from
+// the flattened pair list (spread over the threads), levels >= 4 add a depth-first walk over the middle ones, the last
+// one is a serial loop with four independent bit tests in flight.  The level minimum of (sum |v - c|, L') is exact
+// because Hamming is the primary key.  *slot must be ~0 and visible to the group on entry.  Returns the level that
+// found a valid neighbour (0 = none), group-uniform, and leaves (sad << 40 | L') in *slot.
+static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t* __restrict__ bitmap, const uint64_t* stride, int n,
+                                                    const ProbeMeta& pm, const uint16_t* nb, const uint32_t* pairs,
+                                                    const uint8_t* c, unsigned long long* slot) {
+    const uint32_t NB = pm.NB, C2 = pm.C2;
     uint64_t L = 0;
-    for (int d = 0; d < sm.n; ++d) L += (uint64_t)c[d] * sm.stride[d];
-    int found = 0;
-    for (int level = 2; level <= pm.levels && !found; ++level) {
+    for (int d = 0; d < n; ++d) L += (uint64_t)c[d] * stride[d];
+    for (int level = 2; level <= pm.levels; ++level) {
         uint64_t best = ~0ull;
-        for (uint32_t q = tid; q < C2; q += blockDim.x) {
-            const uint32_t pr = __ldg(&pm.pairs[q]);
-            const uint32_t e1 = __ldg(&pm.tgt[pr & 0xFFFFu]), e2 = __ldg(&pm.tgt[pr >> 16]);
-            const uint32_t d1 = e1 >> 8, d2 = e2 >> 8;
-            const int dv1 = (int)(e1 & 255) - (int)c[d1], dv2 = (int)(e2 & 255) - (int)c[d2];
-            if (dv1 == 0 || dv2 == 0) continue;
-            const uint64_t L2 = L + (int64_t)dv1 * (int64_t)sm.stride[d1] + (int64_t)dv2 * (int64_t)sm.stride[d2];
-            const uint32_t s2 = (uint32_t)(abs(dv1) + abs(dv2));
-            if (level == 2) {
-                if (bit_test(sm.bitmap, L2)) { uint64_t k = ((uint64_t)s2 << 40) | L2; best = k < best ? k : best; }
-            } else {
-#pragma unroll 8
-                for (uint32_t t3 = pm.dim_first[d2 + 1]; t3 < T; ++t3) {
-                    const uint32_t e3 = __ldg(&pm.tgt[t3]), d3 = e3 >> 8;
-                    const int dv3 = (int)(e3 & 255) - (int)c[d3];
-                    const uint64_t L3 = L2 + (int64_t)dv3 * (int64_t)sm.stride[d3];
-                    const bool bit3 = bit_test(sm.bitmap, L3);              // unconditional: dv3 == 0 re-reads L2 (a legal index)
-                    if (dv3 != 0 && bit3) { uint64_t k = ((uint64_t)(s2 + (uint32_t)abs(dv3)) << 40) | L3; best = k < best ? k : best; }
+        if (level == 2) {
+            for (uint32_t q0 = 0; q0 < C2; q0 += 4 * g.G) {             // four independent bit tests per thread and pass
+                uint64_t L2[4]; uint32_t s2[4]; bool bit[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t q = q0 + u * g.G + g.t;
+                    const uint32_t pr = pairs[q < C2 ? q : 0];
+                    const uint32_t e1 = nb[pr & 0xFFFFu], e2 = nb[pr >> 16];
+                    const uint32_t d1 = e1 >> 8, d2 = e2 >> 8, k1 = e1 & 255u, k2 = e2 & 255u, c1 = c[d1], c2 = c[d2];
+                    const int dv1 = (int)(k1 + (k1 >= c1)) - (int)c1, dv2 = (int)(k2 + (k2 >= c2)) - (int)c2;
+                    L2[u] = L + (int64_t)dv1 * (int64_t)stride[d1] + (int64_t)dv2 * (int64_t)stride[d2];
+                    s2[u] = (uint32_t)(abs(dv1) + abs(dv2));
+                    bit[u] = bit_test(bitmap, L2[u]) && q < C2;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (bit[u]) { const uint64_t k = ((uint64_t)s2[u] << 40) | L2[u]; best = k < best ? k : best; }
+            }
+        } else {
+            const int extra = level - 3;                                // middle neighbours walked depth-first (0 .. 3)
+            for (uint32_t q = g.t; q < C2; q += g.G) {
+                const uint32_t pr = pairs[q];
+                const uint32_t e1 = nb[pr & 0xFFFFu], e2 = nb[pr >> 16];
+                const uint32_t d1 = e1 >> 8, d2 = e2 >> 8, k1 = e1 & 255u, k2 = e2 & 255u, c1 = c[d1], c2 = c[d2];
+                const int dv1 = (int)(k1 + (k1 >= c1)) - (int)c1, dv2 = (int)(k2 + (k2 >= c2)) - (int)c2;
+                uint64_t Lst[CAO_MAX_PROBE_LEVEL - 2]; uint32_t sst[CAO_MAX_PROBE_LEVEL - 2], tcur[CAO_MAX_PROBE_LEVEL - 2];
+                Lst[0] = L + (int64_t)dv1 * (int64_t)stride[d1] + (int64_t)dv2 * (int64_t)stride[d2];
+                sst[0] = (uint32_t)(abs(dv1) + abs(dv2));
+                tcur[0] = pm.nb_first[d2 + 1];
+                int depth = 0;
+                for (;;) {
+                    if (depth == extra) {                               // innermost neighbour: serial loop, 4 loads in flight
+                        const uint64_t Lb = Lst[depth]; const uint32_t sb = sst[depth];
+                        for (uint32_t t0 = tcur[depth]; t0 < NB; t0 += 4) {
+                            uint64_t L3[4]; uint32_t s3[4]; bool bit[4];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                const uint32_t t = t0 + u < NB ? t0 + u : t0;
+                                const uint32_t e3 = nb[t], d3 = e3 >> 8, k3 = e3 & 255u, c3 = c[d3];
+                                const int dv3 = (int)(k3 + (k3 >= c3)) - (int)c3;
+                                L3[u] = Lb + (int64_t)dv3 * (int64_t)stride[d3];
+                                s3[u] = sb + (uint32_t)abs(dv3);
+                                bit[u] = bit_test(bitmap, L3[u]) && t0 + u < NB;
+                            }
+#pragma unroll
+                            for (int u = 0; u < 4; ++u)
+                                if (bit[u]) { const uint64_t k = ((uint64_t)s3[u] << 40) | L3[u]; best = k < best ? k : best; }
+                        }
+                        if (depth == 0) break;
+                        --depth; ++tcur[depth];
+                        continue;
+                    }
+                    if (tcur[depth] >= NB) {                            // this middle position is exhausted
+                        if (depth == 0) break;
+                        --depth; ++tcur[depth];
+                        continue;
+                    }
+                    const uint32_t em = nb[tcur[depth]], dm = em >> 8, km = em & 255u, cm = c[dm];
+                    const int dvm = (int)(km + (km >= cm)) - (int)cm;
+                    Lst[depth + 1] = Lst[depth] + (int64_t)dvm * (int64_t)stride[dm];
+                    sst[depth + 1] = sst[depth] + (uint32_t)abs(dvm);
+                    tcur[depth + 1] = pm.nb_first[dm + 1];
+                    ++depth;
                 }
             }
         }
-        best = warp_min_u64(best);
-        if ((tid & 31) == 0 && best != ~0ull) atomicMin(s_best, best);
-        __syncthreads();
-        const bool hit = *s_best != ~0ull;
-        __syncthreads();                                                // everyone has read the slot before the next level writes it
-        if (hit) found = level;
+        grp_min_key(g, best, slot);                                     // barrier inside
+        const bool found = *slot != ~0ull;
+        g.sync();                                                       // everyone has read the slot before the next level writes it
+        if (found) return level;
     }
-    return found;
+    return 0;
 }
 
+// Hamming >= 2 probe of the worklist: one CTA per candidate.  Candidates without a valid neighbour up to `pm.levels`
+// go on to the table scan (wl_out).
 template <int ROWW>
 __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm,
                                                  const uint8_t* __restrict__ cand_rows, const uint32_t* __restrict__ wl,
                                                  const uint32_t* __restrict__ wl_count, unsigned long long* key,
                                                  uint32_t* wl_out, uint32_t* wl_out_count, unsigned long long* n_scanned) {
-    // One CTA per worklist candidate.
-    __shared__ uint32_t s_cw[ROWW];
+    __shared__ __align__(16) uint32_t s_cw[ROWW];
     __shared__ unsigned long long s_best;
+    __shared__ uint64_t s_stride[CAO_MAX_DIMS];
     const uint32_t count = *wl_count, tid = threadIdx.x;
+    if (tid < (uint32_t)sm.n) s_stride[tid] = sm.stride[tid];
+    const Grp g{tid, blockDim.x, 0};
     for (uint32_t ci = blockIdx.x; ci < count; ci += gridDim.x) {
         const uint32_t slot = wl[ci];
         __syncthreads();
         if (tid < ROWW) s_cw[tid] = ((const uint32_t*)(cand_rows + (uint64_t)slot * (ROWW * 4)))[tid];
         if (tid == 0) s_best = ~0ull;
         __syncthreads();
-        const int found = probe23_cta<ROWW>(sm, pm, s_cw, &s_best);
+        const int found = probe_levels_grp(g, sm.bitmap, s_stride, sm.n, pm, pm.nb, pm.pairs, (const uint8_t*)s_cw, &s_best);
         if (tid == 0) {
             const uint64_t best = s_best;
             if (found) key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));

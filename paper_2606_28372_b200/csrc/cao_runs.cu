@@ -113,7 +113,7 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
     uint32_t* wl_count = (uint32_t*)(sc + align256(count * 8) + 2 * align256(count * 4));
     uint32_t* wl2_count = wl_count + 1;
     CAO_CUDA(cudaMemsetAsync(wl_count, 0, 8, st));
-    const int levels = use_probe < 0 || use_probe > 3 ? s->probe.levels : use_probe;
+    const int levels = use_probe < 0 || use_probe > CAO_MAX_PROBE_LEVEL ? s->probe.levels : (s->probe.C2 == 0 ? std::min(use_probe, 1) : use_probe);
     const bool two = levels >= 2;
     unsigned grid = (unsigned)((count + 255) / 256);
     {   // without Hamming-2/3 probes everything unresolved goes to the scan list directly
@@ -146,11 +146,16 @@ static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P) {
     L.cand = take(P * roww); L.key = take(2 * P);
     L.scr = take(algo == CAO_GA ? 3 * P : P);
     L.wl = take(P); L.cw = take(GEN_NB * roww); L.skey = take(2 * GEN_NB); L.bestrow = take(roww);
+    L.Lc = take(2 * P); L.aux4 = take(4 * P);
     L.words = off;
     L.G = (P + 31) / 32 * 32;
     L.NG = L.G <= 256 ? 256 / L.G : 1;
-    const uint64_t tab_bytes = (uint64_t)s->probe.C2 * 4 + (uint64_t)s->probe.T * 2;
-    L.cta_words = (s->probe.levels >= 2 && tab_bytes <= 16384) ? (uint32_t)((tab_bytes + 15) / 16 * 4) : 0;
+    L.NB = 0;
+    for (uint32_t d = 0; d < n; ++d) L.NB += (uint32_t)s->meta.m[d] - 1u;
+    L.nb_words = (L.NB / 2 + 4) & ~3u;
+    const uint64_t tab_bytes = (uint64_t)s->probe.C2 * 4;
+    L.probe_in_smem = s->probe.levels >= 2 && tab_bytes <= 16384;
+    L.cta_words = 3 * CAO_MAX_DIMS + L.nb_words + (L.probe_in_smem ? (uint32_t)((tab_bytes + 15) / 16 * 4) : 0);
     // keep one CTA below the 227 KB opt-in limit: fewer groups per CTA for large populations / many dimensions
     while (L.NG > 1 && ((uint64_t)L.cta_words + (uint64_t)L.NG * L.words) * 4 > 200 * 1024) --L.NG;
     return L;
@@ -180,7 +185,7 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
     L.zero_from = off;
     L.dedup = take(R * L.dedup_words * 4);
     L.uniq = take(R * 4); L.gens_done = take(R * 4); L.stagn = take(R * 4);
-    L.wl_count = take(8); L.counters = take(4 * 8); L.ticket = take(8);
+    L.wl_count = take(8); L.counters = take(16 * 8); L.ticket = take(8);
     L.zero_bytes = off - L.zero_from;
     L.best_rank = take(R * 4); L.best_f = take(R * 4);
     L.traj = take((max_gens + 1) * R * 12);
@@ -400,6 +405,13 @@ int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uin
     if (n_repaired) *n_repaired = h[0];
     if (n_scanned) *n_scanned = h[1];
     if (n_evaluated) *n_evaluated = h[2];
+    return CAO_OK;
+}
+
+int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out16) {
+    if (!r || !h_out16) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_stats: NULL argument");
+    CAO_CUDA(cudaMemcpyAsync(h_out16, r->rm.counters, 16 * 8, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CAO_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
     return CAO_OK;
 }
 

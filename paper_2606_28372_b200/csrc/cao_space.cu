@@ -124,7 +124,7 @@ int cao_space_set_build_mode(cao_space* s, int32_t mode) {
 }
 
 int cao_space_set_probe_levels(cao_space* s, int32_t levels) {
-    if (!s || levels < -1 || levels > 3) return cao_fail(CAO_E_INVALID_ARG, "cao_space_set_probe_levels: levels must be -1 (auto) or 0..3");
+    if (!s || levels < -1 || levels > CAO_MAX_PROBE_LEVEL) return cao_fail(CAO_E_INVALID_ARG, "cao_space_set_probe_levels: levels must be -1 (auto) or 0..6");
     if (s->counted) return cao_fail(CAO_E_STATE, "cao_space_set_probe_levels: call before cao_space_build_count");
     s->probe_levels_req = levels;
     return CAO_OK;
@@ -378,33 +378,33 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
     s->off_rows = off; off = align256(off + std::max<uint64_t>(1, V) * rowB);
     s->off_Ltab = off; off = align256(off + std::max<uint64_t>(1, V) * 8);
     s->off_dir = off; off = align256(off + (s->nd + 1) * 4);
-    // probe targets and the cost model that decides how many Hamming levels are probed before the scan:
-    // C_h = number of index rows at Hamming distance exactly h from a point (upper bound, e_h of the m_d)
+    // neighbour lists and the cost model that decides how many Hamming levels are probed before the scan:
+    // e_h = number of index rows at Hamming distance exactly h from a point (elementary symmetric polynomial of m_d - 1)
     {
         const int n = s->meta.n;
-        s->h_tgt.clear();
+        s->h_nb.clear();
         for (int d = 0; d < n; ++d) {
-            s->probe.dim_first[d] = (uint16_t)s->h_tgt.size();
-            for (int v = 0; v < (int)s->meta.m[d]; ++v) s->h_tgt.push_back((uint16_t)(d << 8 | v));
+            s->probe.nb_first[d] = (uint16_t)s->h_nb.size();
+            for (int k = 0; k + 1 < (int)s->meta.m[d]; ++k) s->h_nb.push_back((uint16_t)(d << 8 | k));
         }
-        for (int d = n; d <= CAO_MAX_DIMS; ++d) s->probe.dim_first[d] = (uint16_t)s->h_tgt.size();
-        s->probe.T = (uint32_t)s->h_tgt.size();
-        double e[4] = {1, 0, 0, 0};
-        for (int d = 0; d < n; ++d) for (int h = 3; h >= 1; --h) e[h] += e[h - 1] * (double)s->meta.m[d];
+        for (int d = n; d <= CAO_MAX_DIMS; ++d) s->probe.nb_first[d] = (uint16_t)s->h_nb.size();
+        s->probe.NB = (uint32_t)s->h_nb.size();
+        double e[CAO_MAX_PROBE_LEVEL + 1] = {1, 0, 0, 0, 0, 0, 0};
+        for (int d = 0; d < n; ++d) for (int h = CAO_MAX_PROBE_LEVEL; h >= 1; --h) e[h] += e[h - 1] * (double)(s->meta.m[d] - 1);
         const double scan_cost = (double)V * (5.0 * ((n + 3) / 4) + 6.0);
         int lv = 1;
-        if (e[2] * 60.0 <= scan_cost) { lv = 2; if (e[3] * 60.0 <= scan_cost) lv = 3; }
-        if (s->probe_levels_req >= 0) lv = std::min(3, std::max(0, s->probe_levels_req));
+        while (lv < CAO_MAX_PROBE_LEVEL && e[lv + 1] * 60.0 <= scan_cost) ++lv;
+        if (s->probe_levels_req >= 0) lv = std::min(CAO_MAX_PROBE_LEVEL, std::max(0, s->probe_levels_req));
         if (e[2] > 65536.0) lv = std::min(lv, 1);                      // the pair list would not fit its budget
         s->h_pairs.clear();
         if (lv >= 2)
-            for (uint32_t t1 = 0; t1 < s->probe.T; ++t1)
-                for (uint32_t t2 = s->probe.dim_first[(s->h_tgt[t1] >> 8) + 1]; t2 < s->probe.T; ++t2)
+            for (uint32_t t1 = 0; t1 < s->probe.NB; ++t1)
+                for (uint32_t t2 = s->probe.nb_first[(s->h_nb[t1] >> 8) + 1]; t2 < s->probe.NB; ++t2)
                     s->h_pairs.push_back(t1 | (t2 << 16));
         s->probe.C2 = (uint32_t)s->h_pairs.size();
         s->probe.levels = lv;
     }
-    s->off_tgt = off; off = align256(off + std::max<uint64_t>(1, s->h_tgt.size()) * 2);
+    s->off_tgt = off; off = align256(off + std::max<uint64_t>(1, s->h_nb.size()) * 2);
     s->off_pairs = off; off = align256(off + std::max<uint64_t>(1, s->h_pairs.size()) * 4);
     s->table_bytes = off;
     return CAO_OK;
@@ -425,8 +425,9 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
     uint8_t* tb = (uint8_t*)d_table;
     uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
     { int rc = launch_fill(s, tb, st); if (rc) return rc; }
-    CAO_CUDA(cudaMemcpyAsync(tb + s->off_tgt, s->h_tgt.data(), s->h_tgt.size() * 2, cudaMemcpyHostToDevice, st));
-    s->probe.tgt = (const uint16_t*)(tb + s->off_tgt);
+    if (!s->h_nb.empty())
+        CAO_CUDA(cudaMemcpyAsync(tb + s->off_tgt, s->h_nb.data(), s->h_nb.size() * 2, cudaMemcpyHostToDevice, st));
+    s->probe.nb = (const uint16_t*)(tb + s->off_tgt);
     if (!s->h_pairs.empty())
         CAO_CUDA(cudaMemcpyAsync(tb + s->off_pairs, s->h_pairs.data(), s->h_pairs.size() * 4, cudaMemcpyHostToDevice, st));
     s->probe.pairs = (const uint32_t*)(tb + s->off_pairs);

@@ -168,7 +168,7 @@ def test_small_populations_and_tiny_spaces():
                 compare(gr, orr, sp.n)
 
 
-@pytest.mark.parametrize("levels", [0, 1, 2, 3])
+@pytest.mark.parametrize("levels", [0, 1, 2, 3, 4, 5, 6])
 def test_forced_probe_levels_give_identical_runs(levels):
     """The Hamming-level probes are an exact shortcut of the scan: every setting reproduces the oracle."""
     import paper_2606_28372_b200 as cao
@@ -190,6 +190,6 @@ def test_forced_probe_levels_give_identical_runs(levels):
 def test_auto_probe_levels():
     import paper_2606_28372_b200 as cao
     sp, os_ = oracle_space(1)
-    assert gpu_space(1, os_, sp).probe_levels == 3
+    assert gpu_space(1, os_, sp).probe_levels == 6
     sp0, os0 = oracle_space(0)
     assert gpu_space(0, os0, sp0).probe_levels == 1
