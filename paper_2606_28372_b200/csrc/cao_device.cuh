@@ -30,6 +30,7 @@ struct SpaceMeta {
 // t = (dimension d, k) with k = 0 .. m_d - 2 stands for the value index v = k + (k >= c_d) != c_d of a candidate c, so
 // no probe is ever wasted on the candidate's own value.  Entries are sorted by (d, k).
 #define CAO_MAX_PROBE_LEVEL 6
+#define CAO_MAX_NB_PROBE 368            // NB above this never probes beyond level 1 (the pair list would exceed 2^16 entries)
 struct ProbeMeta {
     const uint16_t* nb;                 // NB entries: d << 8 | k
     const uint32_t* pairs;              // C2 entries: t1 | t2 << 16, dimension(t1) < dimension(t2)

@@ -142,12 +142,12 @@ struct GrpMem {
     GrpShared* gs;
     uint32_t* rank; float* f; uint32_t* idx; float* x; float* v; float* pb; float* pbf;
     uint32_t* cand; unsigned long long* key; uint32_t* scr; uint32_t* wl; uint32_t* cw; unsigned long long* skey;
-    uint32_t* bestrow; uint64_t* Lc; uint32_t* aux4;
+    uint32_t* bestrow; uint64_t* Lc; uint32_t* aux4; uint64_t* ptab;
     __device__ __forceinline__ GrpMem(uint32_t* S, const GenLayout& l)
         : gs((GrpShared*)S), rank(S + l.rank), f((float*)(S + l.f)), idx(S + l.idx), x((float*)(S + l.x)), v((float*)(S + l.v)),
           pb((float*)(S + l.pb)), pbf((float*)(S + l.pbf)), cand(S + l.cand), key((unsigned long long*)(S + l.key)),
           scr(S + l.scr), wl(S + l.wl), cw(S + l.cw), skey((unsigned long long*)(S + l.skey)), bestrow(S + l.bestrow),
-          Lc((uint64_t*)(S + l.Lc)), aux4(S + l.aux4) {}
+          Lc((uint64_t*)(S + l.Lc)), aux4(S + l.aux4), ptab((uint64_t*)(S + l.ptab)) {}
 };
 
 // O10: evaluate rank rk for run k.  Returns f; *is_new = this evaluation set the run's memo bit (L268).
@@ -442,7 +442,6 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
     if (has) {
         if (same) {
             key = S.key[i]; valid = (key >> 45) == 0;
-            if (!valid) atomicAdd(&gs->n_memo, 1u);
         } else {
             const uint32_t rk0 = valid_rank(sm.bitmap, sm.dir, L, &valid);   // operator outputs are in-domain by construction
             if (valid) key = make_key(0, 0, rk0);
@@ -452,7 +451,8 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
     if (pm.levels >= 1) {
         unsigned long long* hkey = (unsigned long long*)S.aux4;
         uint32_t* ol = S.scr;
-        if (open) { ol[atomicAdd(&gs->flag, 1u)] = i; S.Lc[i] = L; hkey[i] = ~0ull; }
+        const uint32_t pos = grp_push(open, &gs->flag);
+        if (open) { ol[pos] = i; S.Lc[i] = L; hkey[i] = ~0ull; }
         g.sync();                                                       // candidate rows, list and linear indices are visible
         const uint32_t nopen = gs->flag;
         if (nopen) {
@@ -467,15 +467,23 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             }
         }
     }
+    bool rc_hit = false;
     if (open && key == CAO_KEY_NONE) {                                  // memoised repairs of this run (L268 in spirit)
         const ulonglong2 e = rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(L)];
-        if (e.x == L) { key = e.y; atomicAdd(&gs->n_rc, 1u); }
+        if (e.x == L) { key = e.y; rc_hit = true; }
     }
     if (has && !same) S.key[i] = key;
-    if (has && key == CAO_KEY_NONE) S.wl[atomicAdd(&gs->nwl, 1u)] = i;
     {
+        const uint32_t pos = grp_push(has && key == CAO_KEY_NONE, &gs->nwl);
+        if (has && key == CAO_KEY_NONE) S.wl[pos] = i;
         const uint32_t ninv = __popc(__ballot_sync(0xFFFFFFFFu, has && !valid));
-        if ((i & 31) == 0 && ninv) atomicAdd(&gs->n_inv, ninv);
+        const uint32_t nmemo = __popc(__ballot_sync(0xFFFFFFFFu, has && same && !valid));
+        const uint32_t nrc = __popc(__ballot_sync(0xFFFFFFFFu, rc_hit));
+        if ((i & 31) == 0) {
+            if (ninv) atomicAdd(&gs->n_inv, ninv);
+            if (nmemo) atomicAdd(&gs->n_memo, nmemo);
+            if (nrc) atomicAdd(&gs->n_rc, nrc);
+        }
     }
     g.sync();
     CAO_TICK(1);
@@ -490,7 +498,7 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
                 const uint8_t* c = (const uint8_t*)S.cand + (size_t)slot * RB;
                 if (i == 0) gs->aux = ~0ull;
                 g.sync();
-                const int found = probe_levels_grp(g, sm.bitmap, tb.stride, n, pm, tb.nb, tb.pairs, c, &gs->aux);
+                const int found = probe_levels_grp(g, sm.bitmap, tb.stride, pm, tb.nb, tb.pairs, c, S.Lc[slot], S.ptab, &gs->aux);
                 if (found == 2) CAO_TICK(2); else CAO_TICK(3);
                 if (i == 0) {
                     gs->n_p2 += 1; gs->n_p3 += found != 2 && pm.levels >= 3;   // went to the Hamming-2 probe / beyond it
@@ -500,8 +508,7 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
                         const uint64_t kk = make_key((uint32_t)found, (uint32_t)(best >> 40),
                                                      valid_rank(sm.bitmap, sm.dir, best & ((1ull << 40) - 1), &dummy));
                         S.key[slot] = kk;
-                        uint64_t Lc = 0;
-                        for (int d = 0; d < n; ++d) Lc += (uint64_t)c[d] * tb.stride[d];
+                        const uint64_t Lc = S.Lc[slot];
                         rm.rcache[(uint64_t)k * CAO_RCACHE + rcache_slot(Lc)] = make_ulonglong2(Lc, kk);
                     } else {
                         S.wl[nscan] = slot;                             // nscan <= fq: compacts in place
@@ -559,8 +566,9 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             uint32_t* ol = S.scr; uint32_t* mm = S.aux4;
             if (i == 0) gs->flag = 0;
             g.sync();
+            const uint32_t pos = grp_push(mutate, &gs->flag);
             if (mutate) {
-                ol[atomicAdd(&gs->flag, 1u)] = i; S.Lc[i] = Lr;
+                ol[pos] = i; S.Lc[i] = Lr;
                 for (uint32_t w = 0; w < MW; ++w) mm[i * 4 + w] = 0;
             }
             g.sync();
@@ -667,7 +675,13 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             if (has) s_u[i] = rk;
             g.sync();
             bool acc = false;
-            if (has) {
+            if (g.G == 32) {                                            // one warp: compare through shuffles, no divergence
+                const uint32_t old = has ? S.rank[i] : 0xFFFFFFFFu;
+                bool member = false;
+                for (uint32_t j = 0; j < P; ++j) member |= __shfl_sync(0xFFFFFFFFu, old, j) == rk;
+                const uint32_t twins = __match_any_sync(0xFFFFFFFFu, has ? rk : 0xFFFFFFFFu - i);   // lanes with the same trial
+                acc = has && f <= S.f[i] && !member && (twins & ((1u << i) - 1u)) == 0;
+            } else if (has) {
                 acc = f <= S.f[i];
                 for (uint32_t j = 0; j < P && acc; ++j) if (S.rank[j] == rk) acc = false;
                 for (uint32_t j = 0; j < i && acc; ++j) if (s_u[j] == rk) acc = false;

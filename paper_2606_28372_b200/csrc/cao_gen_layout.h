@@ -4,7 +4,7 @@
 
 // Word offsets of the per-group shared-memory slice (computed on the host, cao_runs.cu: gen_layout()).
 struct GenLayout {
-    uint32_t rank, f, idx, x, v, pb, pbf, cand, key, scr, wl, cw, skey, bestrow, Lc, aux4;
+    uint32_t rank, f, idx, x, v, pb, pbf, cand, key, scr, wl, cw, skey, bestrow, Lc, aux4, ptab;
     uint32_t words;                  // words per group (multiple of 4)
     uint32_t cta_words;              // CTA-wide prefix: strides, upper coordinates, Hamming-1 neighbour list, probe lists
     uint32_t NB, nb_words;           // Hamming-1 neighbours of a point = sum (m_d - 1); words of their list

@@ -93,67 +93,70 @@ __device__ __forceinline__ void grp_min_key(const Grp& g, uint64_t v, unsigned l
     g.sync();
 }
 
-// Group-cooperative probe of ONE candidate c (n index bytes, in-domain) at Hamming levels 2 .. pm.levels, in turn.  A row
-// at Hamming distance exactly h is h neighbours (d, v != c_d) of strictly increasing dimension: the first two come from
-// the flattened pair list (spread over the threads), levels >= 4 add a depth-first walk over the middle ones, the last
-// one is a serial loop with four independent bit tests in flight.  The level minimum of (sum |v - c|, L') is exact
-// because Hamming is the primary key.  *slot must be ~0 and visible to the group on entry.  Returns the level that
-// found a valid neighbour (0 = none), group-uniform, and leaves (sad << 40 | L') in *slot.
-static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t* __restrict__ bitmap, const uint64_t* stride, int n,
+// Appends the threads with `pred` to a list: returns this thread's position (one shared-memory atomic per warp).
+__device__ __forceinline__ uint32_t grp_push(bool pred, uint32_t* counter) {
+    const uint32_t bal = __ballot_sync(0xFFFFFFFFu, pred), lane = threadIdx.x & 31;
+    uint32_t base = 0;
+    if (lane == 0 && bal) base = atomicAdd(counter, (uint32_t)__popc(bal));
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    return base + __popc(bal & ((1u << lane) - 1u));
+}
+
+// Group-cooperative probe of ONE candidate c (n index bytes, in-domain, linear index L) at Hamming levels
+// 2 .. pm.levels, in turn.  A row at Hamming distance exactly h is h neighbours (d, v != c_d) of strictly increasing
+// dimension.  Every neighbour t contributes ptab[t] = (|v - c_d| << 40) + (v - c_d) * stride_d, so the packed key
+// (sum |delta| << 40 | L') of a row is L + the sum of its neighbours' contributions (the fields cannot interfere:
+// 0 <= L' < 2^40, sum |delta| < 2^13).  The first two neighbours come from the flattened pair list (spread over the
+// threads, four independent bit tests in flight), levels >= 4 add a depth-first walk over the middle ones, the last one
+// is a serial loop with four loads in flight.  The level minimum is exact because Hamming is the primary key.  ptab:
+// pm.NB words of shared memory owned by the group.  *slot must be ~0 and visible to the group on entry.  Returns the
+// level that found a valid neighbour (0 = none), group-uniform, and leaves (sad << 40 | L') in *slot.
+static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t* __restrict__ bitmap, const uint64_t* stride,
                                                     const ProbeMeta& pm, const uint16_t* nb, const uint32_t* pairs,
-                                                    const uint8_t* c, unsigned long long* slot) {
+                                                    const uint8_t* c, uint64_t L, uint64_t* ptab, unsigned long long* slot) {
     const uint32_t NB = pm.NB, C2 = pm.C2;
-    uint64_t L = 0;
-    for (int d = 0; d < n; ++d) L += (uint64_t)c[d] * stride[d];
+    const uint64_t M40 = (1ull << 40) - 1;
+    for (uint32_t t = g.t; t < NB; t += g.G) {
+        const uint32_t e = nb[t], d = e >> 8, kq = e & 255u, cd = c[d];
+        const int dv = (int)(kq + (kq >= cd)) - (int)cd;
+        ptab[t] = ((uint64_t)(uint32_t)abs(dv) << 40) + (uint64_t)((int64_t)dv * (int64_t)stride[d]);
+    }
+    g.sync();
     for (int level = 2; level <= pm.levels; ++level) {
         uint64_t best = ~0ull;
         if (level == 2) {
             for (uint32_t q0 = 0; q0 < C2; q0 += 4 * g.G) {             // four independent bit tests per thread and pass
-                uint64_t L2[4]; uint32_t s2[4]; bool bit[4];
+                uint64_t k2[4]; bool bit[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const uint32_t q = q0 + u * g.G + g.t;
                     const uint32_t pr = pairs[q < C2 ? q : 0];
-                    const uint32_t e1 = nb[pr & 0xFFFFu], e2 = nb[pr >> 16];
-                    const uint32_t d1 = e1 >> 8, d2 = e2 >> 8, k1 = e1 & 255u, k2 = e2 & 255u, c1 = c[d1], c2 = c[d2];
-                    const int dv1 = (int)(k1 + (k1 >= c1)) - (int)c1, dv2 = (int)(k2 + (k2 >= c2)) - (int)c2;
-                    L2[u] = L + (int64_t)dv1 * (int64_t)stride[d1] + (int64_t)dv2 * (int64_t)stride[d2];
-                    s2[u] = (uint32_t)(abs(dv1) + abs(dv2));
-                    bit[u] = bit_test(bitmap, L2[u]) && q < C2;
+                    k2[u] = L + ptab[pr & 0xFFFFu] + ptab[pr >> 16];
+                    bit[u] = bit_test(bitmap, k2[u] & M40) && q < C2;
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (bit[u]) { const uint64_t k = ((uint64_t)s2[u] << 40) | L2[u]; best = k < best ? k : best; }
+                for (int u = 0; u < 4; ++u) if (bit[u]) best = k2[u] < best ? k2[u] : best;
             }
         } else {
             const int extra = level - 3;                                // middle neighbours walked depth-first (0 .. 3)
             for (uint32_t q = g.t; q < C2; q += g.G) {
                 const uint32_t pr = pairs[q];
-                const uint32_t e1 = nb[pr & 0xFFFFu], e2 = nb[pr >> 16];
-                const uint32_t d1 = e1 >> 8, d2 = e2 >> 8, k1 = e1 & 255u, k2 = e2 & 255u, c1 = c[d1], c2 = c[d2];
-                const int dv1 = (int)(k1 + (k1 >= c1)) - (int)c1, dv2 = (int)(k2 + (k2 >= c2)) - (int)c2;
-                uint64_t Lst[CAO_MAX_PROBE_LEVEL - 2]; uint32_t sst[CAO_MAX_PROBE_LEVEL - 2], tcur[CAO_MAX_PROBE_LEVEL - 2];
-                Lst[0] = L + (int64_t)dv1 * (int64_t)stride[d1] + (int64_t)dv2 * (int64_t)stride[d2];
-                sst[0] = (uint32_t)(abs(dv1) + abs(dv2));
-                tcur[0] = pm.nb_first[d2 + 1];
+                uint64_t Kst[CAO_MAX_PROBE_LEVEL - 2]; uint32_t tcur[CAO_MAX_PROBE_LEVEL - 2];
+                Kst[0] = L + ptab[pr & 0xFFFFu] + ptab[pr >> 16];
+                tcur[0] = pm.nb_first[(nb[pr >> 16] >> 8) + 1];
                 int depth = 0;
                 for (;;) {
                     if (depth == extra) {                               // innermost neighbour: serial loop, 4 loads in flight
-                        const uint64_t Lb = Lst[depth]; const uint32_t sb = sst[depth];
+                        const uint64_t Kb = Kst[depth];
                         for (uint32_t t0 = tcur[depth]; t0 < NB; t0 += 4) {
-                            uint64_t L3[4]; uint32_t s3[4]; bool bit[4];
+                            uint64_t k3[4]; bool bit[4];
 #pragma unroll
                             for (int u = 0; u < 4; ++u) {
-                                const uint32_t t = t0 + u < NB ? t0 + u : t0;
-                                const uint32_t e3 = nb[t], d3 = e3 >> 8, k3 = e3 & 255u, c3 = c[d3];
-                                const int dv3 = (int)(k3 + (k3 >= c3)) - (int)c3;
-                                L3[u] = Lb + (int64_t)dv3 * (int64_t)stride[d3];
-                                s3[u] = sb + (uint32_t)abs(dv3);
-                                bit[u] = bit_test(bitmap, L3[u]) && t0 + u < NB;
+                                k3[u] = Kb + ptab[t0 + u < NB ? t0 + u : t0];
+                                bit[u] = bit_test(bitmap, k3[u] & M40) && t0 + u < NB;
                             }
 #pragma unroll
-                            for (int u = 0; u < 4; ++u)
-                                if (bit[u]) { const uint64_t k = ((uint64_t)s3[u] << 40) | L3[u]; best = k < best ? k : best; }
+                            for (int u = 0; u < 4; ++u) if (bit[u]) best = k3[u] < best ? k3[u] : best;
                         }
                         if (depth == 0) break;
                         --depth; ++tcur[depth];
@@ -164,11 +167,9 @@ static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t*
                         --depth; ++tcur[depth];
                         continue;
                     }
-                    const uint32_t em = nb[tcur[depth]], dm = em >> 8, km = em & 255u, cm = c[dm];
-                    const int dvm = (int)(km + (km >= cm)) - (int)cm;
-                    Lst[depth + 1] = Lst[depth] + (int64_t)dvm * (int64_t)stride[dm];
-                    sst[depth + 1] = sst[depth] + (uint32_t)abs(dvm);
-                    tcur[depth + 1] = pm.nb_first[dm + 1];
+                    const uint32_t tm = tcur[depth];
+                    Kst[depth + 1] = Kst[depth] + ptab[tm];
+                    tcur[depth + 1] = pm.nb_first[(nb[tm] >> 8) + 1];
                     ++depth;
                 }
             }
@@ -191,6 +192,7 @@ __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMe
     __shared__ __align__(16) uint32_t s_cw[ROWW];
     __shared__ unsigned long long s_best;
     __shared__ uint64_t s_stride[CAO_MAX_DIMS];
+    __shared__ uint64_t s_ptab[CAO_MAX_NB_PROBE];
     const uint32_t count = *wl_count, tid = threadIdx.x;
     if (tid < (uint32_t)sm.n) s_stride[tid] = sm.stride[tid];
     const Grp g{tid, blockDim.x, 0};
@@ -200,7 +202,9 @@ __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMe
         if (tid < ROWW) s_cw[tid] = ((const uint32_t*)(cand_rows + (uint64_t)slot * (ROWW * 4)))[tid];
         if (tid == 0) s_best = ~0ull;
         __syncthreads();
-        const int found = probe_levels_grp(g, sm.bitmap, s_stride, sm.n, pm, pm.nb, pm.pairs, (const uint8_t*)s_cw, &s_best);
+        uint64_t Lc = 0;
+        for (int d = 0; d < sm.n; ++d) Lc += (uint64_t)((const uint8_t*)s_cw)[d] * s_stride[d];
+        const int found = probe_levels_grp(g, sm.bitmap, s_stride, pm, pm.nb, pm.pairs, (const uint8_t*)s_cw, Lc, s_ptab, &s_best);
         if (tid == 0) {
             const uint64_t best = s_best;
             if (found) key[slot] = make_key((uint32_t)found, (uint32_t)(best >> 40), rank_of(sm, best & ((1ull << 40) - 1)));

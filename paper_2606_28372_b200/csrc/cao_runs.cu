@@ -147,6 +147,7 @@ static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P) {
     L.scr = take(algo == CAO_GA ? 3 * P : P);
     L.wl = take(P); L.cw = take(GEN_NB * roww); L.skey = take(2 * GEN_NB); L.bestrow = take(roww);
     L.Lc = take(2 * P); L.aux4 = take(4 * P);
+    L.ptab = take(s->probe.levels >= 2 ? 2 * s->probe.NB : 0);
     L.words = off;
     L.G = (P + 31) / 32 * 32;
     L.NG = L.G <= 256 ? 256 / L.G : 1;

@@ -395,7 +395,7 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
         int lv = 1;
         while (lv < CAO_MAX_PROBE_LEVEL && e[lv + 1] * 60.0 <= scan_cost) ++lv;
         if (s->probe_levels_req >= 0) lv = std::min(CAO_MAX_PROBE_LEVEL, std::max(0, s->probe_levels_req));
-        if (e[2] > 65536.0) lv = std::min(lv, 1);                      // the pair list would not fit its budget
+        if (e[2] > 65536.0 || s->probe.NB > CAO_MAX_NB_PROBE) lv = std::min(lv, 1);   // the pair list would not fit its budget
         s->h_pairs.clear();
         if (lv >= 2)
             for (uint32_t t1 = 0; t1 < s->probe.NB; ++t1)
