@@ -158,12 +158,14 @@ int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, u
  * candidates that needed the table scan, candidates evaluated. */
 int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uint64_t* n_scanned,
                       uint64_t* n_evaluated);
-/* All sixteen 64-bit statistics words since create (synchronises `stream`): 0 n_repaired, 1 n_scanned (candidates that
- * needed the table scan), 2 n_evaluated; fused mode only: 3 candidates that went to the Hamming-2 probe, 4 ... to the
- * Hamming-3 probe, 5 invalid candidates resolved by the previous generation's memo, 6 ... by the per-run repair cache;
- * 7 reserved; 8-13 clock cycles of thread 0 of every group in operator / tail / probe-2 / probe-3 / scan / finish
- * (only in builds with -DCAO_GEN_STATS, else 0); 14-15 reserved.  L268 (memoisation) is what 5 and 6 count. */
-int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out16);
+/* All thirty-two 64-bit statistics words since create (synchronises `stream`): 0 n_repaired, 1 n_scanned (candidates
+ * that needed the table scan), 2 n_evaluated; fused mode only: 3 candidates that went to the Hamming-2 probe, 4 ...
+ * beyond it, 5 invalid candidates resolved by the previous generation's memo, 6 ... by the per-run repair cache
+ * (L268: memoisation); 7 reserved; 8-13 clock cycles of thread 0 of every group in operator / tail / probe-2 /
+ * deeper probes / scan / finish, 14-15 slowest run and most scan cycles in one run (only in builds with
+ * -DCAO_GEN_STATS, else 0); 16-24 candidates of the stepped generations by Hamming distance of their repair
+ * (16 = valid, 17 = Hamming 1, ..., 24 = eight or more; L143, L215); 25-31 reserved. */
+int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out32);
 /* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
 uint64_t cao_launch_count(void);
 
@@ -178,7 +180,14 @@ const char* cao_profile_name(int32_t cls);
 /* Device self-tests for the parity of the arithmetic primitives (O3, O5-O7): out[i] from in[i]. */
 int cao_test_philox(const uint32_t* d_ctr_key /* count x 6 */, uint32_t* d_out /* count x 4 */,
                     uint64_t count, void* stream);
+/* The same inputs through cuRAND's device function curand_Philox4x32_10: a second, independent pin of the generator. */
+int cao_test_curand_philox(const uint32_t* d_ctr_key /* count x 6 */, uint32_t* d_out /* count x 4 */,
+                           uint64_t count, void* stream);
 int cao_test_exp_neg(const float* d_z, float* d_out, uint64_t count, void* stream);
+/* Integer-issue microbenchmark (the denominator of bench.py's "alu" roofline for the repair scan):
+ * n_ctas x 256 threads, each runs `iters` x 8 independent chains of one instruction kind: 0 IMAD (mad.lo.u32),
+ * 1 LOP3, 2 VABSDIFF4 (with accumulate), 3 POPC, 4 IADD.  d_out: n_ctas * 256 words.  The caller times it. */
+int cao_test_int_peak(int32_t kind, uint32_t iters, uint32_t n_ctas, uint32_t* d_out, void* stream);
 
 const char* cao_last_error(void);
 

@@ -212,9 +212,17 @@ void enumerate(Space& s) {
 
 // O9: repair(c) = c if valid else argmin over ALL valid rows of (Hamming, sum |didx|, L).
 struct RepairKey { uint32_t ham, sad; uint64_t L; uint32_t rank; };
+// A27: a row with an index outside its domain (idx_d >= m_d) is not a point of X: it is invalid, and its repair is
+// the same argmin taken over its byte values.
+bool in_domain(const Space& s, const uint8_t* c) {
+    for (int d = 0; d < s.n; ++d) if (c[d] >= s.dom[d].size()) return false;
+    return true;
+}
 RepairKey repair(const Space& s, const uint8_t* c) {
-    uint64_t Lc = s.lin(c);
-    if (s.bit(Lc)) return RepairKey{ 0, 0, Lc, s.rank_of(Lc) };
+    if (in_domain(s, c)) {
+        uint64_t Lc = s.lin(c);
+        if (s.bit(Lc)) return RepairKey{ 0, 0, Lc, s.rank_of(Lc) };
+    }
     RepairKey best{ 0xFFFFFFFFu, 0xFFFFFFFFu, ~0ull, 0xFFFFFFFFu };
     for (uint64_t r = 0; r < s.V; ++r) {
         const uint8_t* v = &s.rows[r * s.n];
@@ -571,7 +579,7 @@ int32_t orc_space_n(const void* p) { return ((const Space*)p)->n; }
 const uint64_t* orc_space_bitmap(const void* p) { return ((const Space*)p)->bitmap.data(); }
 const uint8_t* orc_space_rows(const void* p) { return ((const Space*)p)->rows.data(); }
 const uint64_t* orc_space_Ltab(const void* p) { return ((const Space*)p)->Ltab.data(); }
-int orc_space_is_valid(const void* p, const uint8_t* idx) { const Space* s = (const Space*)p; return s->bit(s->lin(idx)); }
+int orc_space_is_valid(const void* p, const uint8_t* idx) { const Space* s = (const Space*)p; return in_domain(*s, idx) && s->bit(s->lin(idx)); }
 // Count of valid configs among L in [L0, L1) evaluated directly (no table): for sampled-range checks.
 uint64_t orc_space_count_range(const void* p, uint64_t L0, uint64_t L1) {
     const Space* s = (const Space*)p;

@@ -74,7 +74,9 @@ SIGNATURES = {
     "cao_profile_read": (C.c_int, [i32, C.POINTER(C.c_double), pu64]),
     "cao_profile_name": (C.c_char_p, [i32]),
     "cao_test_philox": (C.c_int, [vp, vp, u64, vp]),
+    "cao_test_curand_philox": (C.c_int, [vp, vp, u64, vp]),
     "cao_test_exp_neg": (C.c_int, [vp, vp, u64, vp]),
+    "cao_test_int_peak": (C.c_int, [i32, u32, u32, vp, vp]),
     "cao_last_error": (C.c_char_p, []),
 }
 
@@ -376,11 +378,13 @@ class Runs:
 
     def stats(self):
         """cao_runs_stats: the sixteen statistics words as a dict."""
-        a = (C.c_uint64 * 16)()
+        a = (C.c_uint64 * 32)()
         _check(lib().cao_runs_stats(self._h, _stream(), a))
         names = ["n_repaired", "n_scanned", "n_evaluated", "n_probe2", "n_probe3", "n_memo", "n_rcache", "r7",
                  "cyc_op", "cyc_tail", "cyc_probe2", "cyc_probe3", "cyc_scan", "cyc_finish", "cyc_max_run", "cyc_max_scan"]
-        return {k: int(v) for k, v in zip(names, a)}
+        out = {k: int(v) for k, v in zip(names, a)}
+        out["ham_hist"] = [int(a[16 + h]) for h in range(9)]
+        return out
 
     def __del__(self):
         try:
@@ -397,6 +401,14 @@ def test_philox(ctr_key: torch.Tensor) -> torch.Tensor:
     return out
 
 
+def test_curand_philox(ctr_key: torch.Tensor) -> torch.Tensor:
+    """Same as test_philox, but computed by cuRAND's curand_Philox4x32_10 device function."""
+    t = ctr_key.contiguous()
+    out = torch.empty((t.shape[0], 4), dtype=torch.int32, device=t.device)
+    _check(lib().cao_test_curand_philox(t.data_ptr(), out.data_ptr(), t.shape[0], _stream()))
+    return out
+
+
 def test_exp_neg(z: torch.Tensor) -> torch.Tensor:
     t = z.contiguous()
     out = torch.empty_like(t)
@@ -404,5 +416,24 @@ def test_exp_neg(z: torch.Tensor) -> torch.Tensor:
     return out
 
 
+INT_PEAK_KINDS = {"imad": 0, "lop3": 1, "vabsdiff4": 2, "popc": 3, "iadd": 4}
+
+
+def int_peak(kind: str, iters=4096, n_ctas=148 * 8, reps=5) -> float:
+    """Measured issue rate of one integer instruction kind in lane-operations per second (cao_test_int_peak timed
+    with CUDA events on the current stream, best of `reps`)."""
+    out = torch.empty(n_ctas * 256, dtype=torch.int32, device="cuda")
+    best = None
+    for _ in range(reps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(lib().cao_test_int_peak(INT_PEAK_KINDS[kind], iters, n_ctas, out.data_ptr(), _stream()))
+        e1.record(); e1.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    return n_ctas * 256 * iters * 8 / (best / 1e3)
+
+
 test_philox.__test__ = False
+test_curand_philox.__test__ = False
 test_exp_neg.__test__ = False

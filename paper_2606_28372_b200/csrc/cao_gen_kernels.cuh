@@ -21,6 +21,7 @@ struct GrpShared {                   // first words of every group slice
     uint32_t run, uniq, stagn, n_new, flag, nwl, bestrow_rank, gens;
     uint32_t n_inv, n_scan, n_eval, n_p2, n_p3, n_memo, n_rc, pad;   // statistics of this run in this launch
     unsigned long long cyc[6];       // CAO_GEN_STATS builds: clock cycles in operator / tail / probe-2 / probe-3 / scan / finish
+    uint32_t hist[16];               // repaired candidates by Hamming distance of the repair (0 = valid, ..., 8 = eight or more)
 };
 #ifdef CAO_GEN_STATS
 #define CAO_TICK(slot) do { if (g.t == 0) { const long long now_ = clock64(); gs->cyc[slot] += (unsigned long long)(now_ - t_mark); t_mark = now_; } } while (0)
@@ -238,6 +239,7 @@ __device__ __forceinline__ void load_state(const Grp& g, const SpaceMeta& sm, co
         gs->n_inv = 0; gs->n_scan = 0; gs->n_eval = 0; gs->gens = 0;
         gs->n_p2 = 0; gs->n_p3 = 0; gs->n_memo = 0; gs->n_rc = 0;
         for (int z = 0; z < 6; ++z) gs->cyc[z] = 0;
+        for (int z = 0; z < 16; ++z) gs->hist[z] = 0;
     }
     g.sync();
 }
@@ -271,6 +273,7 @@ __device__ __forceinline__ void store_state(const Grp& g, const SpaceMeta& sm, c
         if (gs->n_p3) atomicAdd(&rm.counters[4], (unsigned long long)gs->n_p3);
         if (gs->n_memo) atomicAdd(&rm.counters[5], (unsigned long long)gs->n_memo);
         if (gs->n_rc) atomicAdd(&rm.counters[6], (unsigned long long)gs->n_rc);
+        for (int z = 0; z < 9; ++z) if (gs->hist[z]) atomicAdd(&rm.counters[16 + z], (unsigned long long)gs->hist[z]);
 #ifdef CAO_GEN_STATS
         unsigned long long tot = 0;
         for (int z = 0; z < 6; ++z) { atomicAdd(&rm.counters[8 + z], gs->cyc[z]); tot += gs->cyc[z]; }
@@ -542,6 +545,11 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
         CAO_TICK(4);
     }
 
+    {                                                                   // statistics: Hamming distance of every repair
+        const uint32_t h = has ? min((uint32_t)(key >> 45), 8u) : 31u;
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, h);
+        if (has && (i & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&gs->hist[h], (uint32_t)__popc(peers));
+    }
     // ---- S6 + S7
     uint32_t rk = (uint32_t)key;
     const uint32_t rep = rk;

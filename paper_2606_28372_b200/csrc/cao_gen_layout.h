@@ -12,4 +12,4 @@ struct GenLayout {
     uint32_t G, NG;                  // threads per group, groups per CTA
 };
 
-#define GRP_SHARED_WORDS 32             // sizeof(GrpShared) / 4
+#define GRP_SHARED_WORDS 48             // sizeof(GrpShared) / 4

@@ -274,15 +274,24 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
 }
 
 // ---------------------------------------------------------------------------------------------
-// Standalone batched repair (cao_space_repair): probe kernel, k_scan, finish kernel.
+// Standalone batched repair (cao_space_repair): probe kernel, k_probe23, k_scan, finish kernel.  The caller's rows are
+// copied to `clean` with the padding bytes (positions >= n) zeroed, so that padding never adds to Hamming or sum |d|;
+// rows with an index outside its domain are invalid and skip the neighbour probes (A27): they go straight to the scan.
 template <int ROWW>
 __global__ void __launch_bounds__(256) k_repair_probe(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ rows_in,
-                                                      uint64_t count, int use_probe, unsigned long long* key,
+                                                      uint8_t* clean, uint64_t count, int use_probe, unsigned long long* key,
                                                       uint32_t* wl, uint32_t* wl_count, uint32_t* wl2, uint32_t* wl2_count) {
     uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
     uint32_t w[ROWW];
     load_row<ROWW>(rows_in + i * (ROWW * 4), w);
+#pragma unroll
+    for (int z = 0; z < ROWW; ++z) {
+        const int first = z * 4;
+        if (first >= sm.n) w[z] = 0;
+        else if (first + 4 > sm.n) w[z] &= 0xFFFFFFFFu >> (8 * (first + 4 - sm.n));
+    }
+    store_row<ROWW>(clean + i * (ROWW * 4), w);
     bool valid;
     bool in_dom = true;
 #pragma unroll
@@ -290,7 +299,6 @@ __global__ void __launch_bounds__(256) k_repair_probe(const __grid_constant__ Sp
         if (d < sm.n && ((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu) >= sm.m[d]) in_dom = false;
     uint64_t k = validate_probe<ROWW>(sm, w, use_probe != 0, valid);
     key[i] = k;
-    // rows with an index outside its domain skip the neighbour probes and go straight to the scan (wl2)
     if (k == CAO_KEY_NONE) { if (in_dom && wl2 != wl) worklist_push(wl, wl_count, (uint32_t)i); else worklist_push(wl2, wl2_count, (uint32_t)i); }
 }
 

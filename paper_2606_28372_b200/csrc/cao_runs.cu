@@ -1,6 +1,7 @@
 // cao_runs.cu -- host side of the repair query and of the runs half of include/cao.h (S2-S7).
 #include <algorithm>
 #include <cstring>
+#include <curand_kernel.h>
 #include "cao_runs_kernels.cuh"
 
 // Fused generation kernel, one object per algorithm (cao_gen_algo.cu).
@@ -30,24 +31,25 @@ struct cao_runs {
 };
 
 // ---------------------------------------------------------------------------------------------
+// in_domain: every candidate byte is a legal index (< m_d <= 128 when M <= 128), which the SMALL byte trick needs.
 template <int WU>
 static void launch_scan_wu(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
-                           unsigned long long* key, cudaStream_t st) {
-    if (sm.M <= 128) k_scan<WU, true><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
+                           unsigned long long* key, bool in_domain, cudaStream_t st) {
+    if (sm.M <= 128 && in_domain) k_scan<WU, true><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
     else k_scan<WU, false><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
 }
 static int launch_scan(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
-                       unsigned long long* key, cudaStream_t st) {
+                       unsigned long long* key, bool in_domain, cudaStream_t st) {
     ProfScope ps(PK_SCAN, st);
     switch ((sm.n + 3) / 4) {
-        case 1: launch_scan_wu<1>(sm, cand, wl, wl_count, key, st); break;
-        case 2: launch_scan_wu<2>(sm, cand, wl, wl_count, key, st); break;
-        case 3: launch_scan_wu<3>(sm, cand, wl, wl_count, key, st); break;
-        case 4: launch_scan_wu<4>(sm, cand, wl, wl_count, key, st); break;
-        case 5: launch_scan_wu<5>(sm, cand, wl, wl_count, key, st); break;
-        case 6: launch_scan_wu<6>(sm, cand, wl, wl_count, key, st); break;
-        case 7: launch_scan_wu<7>(sm, cand, wl, wl_count, key, st); break;
-        default: launch_scan_wu<8>(sm, cand, wl, wl_count, key, st); break;
+        case 1: launch_scan_wu<1>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        case 2: launch_scan_wu<2>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        case 3: launch_scan_wu<3>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        case 4: launch_scan_wu<4>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        case 5: launch_scan_wu<5>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        case 6: launch_scan_wu<6>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        case 7: launch_scan_wu<7>(sm, cand, wl, wl_count, key, in_domain, st); break;
+        default: launch_scan_wu<8>(sm, cand, wl, wl_count, key, in_domain, st); break;
     }
     CAO_LAUNCHED("k_scan");
     return CAO_OK;
@@ -86,12 +88,36 @@ static int launch_probe23(const cao_space* s, const SpaceMeta& sm, const uint8_t
         }                                                                            \
     } while (0)
 
+// Integer-issue peak (bench.py): 8 independent chains per thread of ONE instruction kind, nothing else in the loop.
+template <int KIND>
+__global__ void __launch_bounds__(256) k_int_peak(uint32_t* out, uint32_t iters) {
+    uint32_t a[8];
+    const uint32_t b = threadIdx.x * 2654435761u + 12345u, c = blockIdx.x * 40503u + 7u;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = b ^ (c + j * 0x9E3779B9u);
+    for (uint32_t it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            if (KIND == 0) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a[j]) : "r"(b), "r"(c));
+            if (KIND == 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[j]) : "r"(b), "r"(c));
+            if (KIND == 2) asm volatile("vabsdiff4.u32.u32.u32.add %0, %0, %1, %2;" : "+r"(a[j]) : "r"(b), "r"(c));
+            if (KIND == 3) asm volatile("popc.b32 %0, %0;" : "+r"(a[j]));
+            if (KIND == 4) asm volatile("add.u32 %0, %0, %1;" : "+r"(a[j]) : "r"(b));
+        }
+    }
+    uint32_t x = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x ^= a[j];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = x;
+}
+
 extern "C" {
 
 // ---------------------------------------------------------------------------------------------
 int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes) {
     if (!s || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_scratch_bytes: NULL argument");
-    *bytes = align256(std::max<uint64_t>(1, count) * 8) + 2 * align256(std::max<uint64_t>(1, count) * 4) + 256;
+    *bytes = align256(std::max<uint64_t>(1, count) * 8) + 2 * align256(std::max<uint64_t>(1, count) * 4) + 256 +
+             align256(std::max<uint64_t>(1, count) * (uint64_t)s->meta.rowB);
     return CAO_OK;
 }
 
@@ -112,6 +138,7 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
     uint32_t* wl2 = (uint32_t*)(sc + align256(count * 8) + align256(count * 4));
     uint32_t* wl_count = (uint32_t*)(sc + align256(count * 8) + 2 * align256(count * 4));
     uint32_t* wl2_count = wl_count + 1;
+    uint8_t* clean = sc + align256(count * 8) + 2 * align256(count * 4) + 256;      // rows with zeroed padding
     CAO_CUDA(cudaMemsetAsync(wl_count, 0, 8, st));
     const int levels = use_probe < 0 || use_probe > CAO_MAX_PROBE_LEVEL ? s->probe.levels : (s->probe.C2 == 0 ? std::min(use_probe, 1) : use_probe);
     const bool two = levels >= 2;
@@ -119,13 +146,13 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
     {   // without Hamming-2/3 probes everything unresolved goes to the scan list directly
         ProfScope ps(PK_QUERY, st);
         uint32_t* a = two ? wl : wl2; uint32_t* ac = two ? wl_count : wl2_count;
-        if (s->meta.rowB == 16) k_repair_probe<4><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, levels >= 1, key, a, ac, wl2, wl2_count);
-        else k_repair_probe<8><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, count, levels >= 1, key, a, ac, wl2, wl2_count);
+        if (s->meta.rowB == 16) k_repair_probe<4><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, clean, count, levels >= 1, key, a, ac, wl2, wl2_count);
+        else k_repair_probe<8><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, clean, count, levels >= 1, key, a, ac, wl2, wl2_count);
     }
     CAO_LAUNCHED("k_repair_probe");
     int rc = CAO_OK;
-    if (two) { rc = launch_probe23(s, s->meta, d_idx_rows, wl, wl_count, key, wl2, wl2_count, nullptr, levels, st); if (rc) return rc; }
-    rc = launch_scan(s->meta, d_idx_rows, wl2, wl2_count, key, st);
+    if (two) { rc = launch_probe23(s, s->meta, clean, wl, wl_count, key, wl2, wl2_count, nullptr, levels, st); if (rc) return rc; }
+    rc = launch_scan(s->meta, clean, wl2, wl2_count, key, false, st);
     if (rc) return rc;
     k_repair_finish<<<grid, 256, 0, st>>>(key, count, d_rank_out, d_key_out);
     CAO_LAUNCHED("k_repair_finish");
@@ -186,7 +213,7 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
     L.zero_from = off;
     L.dedup = take(R * L.dedup_words * 4);
     L.uniq = take(R * 4); L.gens_done = take(R * 4); L.stagn = take(R * 4);
-    L.wl_count = take(8); L.counters = take(16 * 8); L.ticket = take(8);
+    L.wl_count = take(8); L.counters = take(32 * 8); L.ticket = take(8);
     L.zero_bytes = off - L.zero_from;
     L.best_rank = take(R * 4); L.best_f = take(R * 4);
     L.traj = take((max_gens + 1) * R * 12);
@@ -332,7 +359,7 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
                                 &r->rm.counters[1], levels, st);
             if (rc) return rc;
         }
-        rc = launch_scan(r->sm, r->rm.cand, levels >= 2 ? r->rm.wl2 : r->rm.wl, levels >= 2 ? r->rm.wl2_count : r->rm.wl_count, r->rm.key, st);
+        rc = launch_scan(r->sm, r->rm.cand, levels >= 2 ? r->rm.wl2 : r->rm.wl, levels >= 2 ? r->rm.wl2_count : r->rm.wl_count, r->rm.key, true, st);
         if (rc) return rc;
 #define CALL_FIN(A, W) k_finish<A, W><<<r->rm.R, r->block, r->smem_fin, st>>>(r->sm, r->rm, g)
         { ProfScope ps(PK_FINISH, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_FIN); }
@@ -409,9 +436,9 @@ int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uin
     return CAO_OK;
 }
 
-int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out16) {
-    if (!r || !h_out16) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_stats: NULL argument");
-    CAO_CUDA(cudaMemcpyAsync(h_out16, r->rm.counters, 16 * 8, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out32) {
+    if (!r || !h_out32) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_stats: NULL argument");
+    CAO_CUDA(cudaMemcpyAsync(h_out32, r->rm.counters, 32 * 8, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CAO_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
     return CAO_OK;
 }
@@ -433,6 +460,35 @@ int cao_test_philox(const uint32_t* d_ctr_key, uint32_t* d_out, uint64_t count, 
     if (!d_ctr_key || !d_out) return cao_fail(CAO_E_INVALID_ARG, "cao_test_philox: NULL argument");
     k_test_philox<<<(unsigned)((count + 255) / 256), 256, 0, (cudaStream_t)stream>>>(d_ctr_key, d_out, count);
     CAO_LAUNCHED("k_test_philox");
+    return CAO_OK;
+}
+// The same counters and keys through cuRAND's own device function curand_Philox4x32_10 (an independent implementation).
+__global__ void k_test_curand_philox(const uint32_t* __restrict__ in, uint32_t* out, uint64_t count) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const uint32_t* p = in + i * 6;
+    uint4 r = curand_Philox4x32_10(make_uint4(p[0], p[1], p[2], p[3]), make_uint2(p[4], p[5]));
+    ((uint4*)out)[i] = r;
+}
+int cao_test_curand_philox(const uint32_t* d_ctr_key, uint32_t* d_out, uint64_t count, void* stream) {
+    if (count == 0) return CAO_OK;
+    if (!d_ctr_key || !d_out) return cao_fail(CAO_E_INVALID_ARG, "cao_test_curand_philox: NULL argument");
+    k_test_curand_philox<<<(unsigned)((count + 255) / 256), 256, 0, (cudaStream_t)stream>>>(d_ctr_key, d_out, count);
+    CAO_LAUNCHED("k_test_curand_philox");
+    return CAO_OK;
+}
+int cao_test_int_peak(int32_t kind, uint32_t iters, uint32_t n_ctas, uint32_t* d_out, void* stream) {
+    if (!d_out || n_ctas == 0) return cao_fail(CAO_E_INVALID_ARG, "cao_test_int_peak: NULL / empty argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (kind) {
+        case 0: k_int_peak<0><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
+        case 1: k_int_peak<1><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
+        case 2: k_int_peak<2><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
+        case 3: k_int_peak<3><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
+        case 4: k_int_peak<4><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
+        default: return cao_fail(CAO_E_INVALID_ARG, "cao_test_int_peak: kind must be 0..4");
+    }
+    CAO_LAUNCHED("k_int_peak");
     return CAO_OK;
 }
 int cao_test_exp_neg(const float* d_z, float* d_out, uint64_t count, void* stream) {

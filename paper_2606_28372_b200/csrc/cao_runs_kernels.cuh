@@ -355,6 +355,11 @@ __device__ __forceinline__ void gen_finish(const SpaceMeta& sm, const RunsMeta& 
     __syncthreads();
     const uint64_t q = (uint64_t)k * P + i;
     uint32_t rk = 0; float f = 0.0f;
+    {                                                                   // statistics: Hamming distance of every repair
+        const uint32_t h = i < P ? min((uint32_t)(rm.key[q] >> 45), 8u) : 31u;
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, h);
+        if (i < P && (i & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&rm.counters[16 + h], (unsigned long long)__popc(peers));
+    }
     if (i < P) {
         rk = (uint32_t)rm.key[q];
         rm.rep_rank[q] = rk;

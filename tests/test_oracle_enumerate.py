@@ -156,6 +156,37 @@ def test_repair_is_the_key_minimum_on_tiny_spaces(seed):
             assert ham >= 1
 
 
+@pytest.mark.parametrize("seed", range(10))
+def test_repair_of_rows_outside_the_domain(seed):
+    """A27: idx_d >= m_d is not a point of X: is-valid is false, repair is the same key minimum over the byte values
+    (numpy brute force; a worked cfg0 value: (7,0,0) -> nearest row by (Hamming, sum |d|, L))."""
+    sp = W.random_tiny_space(300 + seed)
+    s = O.OracleSpace.from_space(sp).build()
+    if s.V == 0:
+        pytest.skip("empty space")
+    rows, Ls = s.rows(), s.Ltab()
+    rng = np.random.default_rng(seed)
+    cands = np.stack([rng.integers(0, mm, 40) for mm in sp.m], axis=1).astype(np.uint8)
+    col = rng.integers(0, sp.n, 40)
+    cands[np.arange(40), col] = np.array([sp.m[c] for c in col]) + rng.integers(0, 200, 40)   # at least one index outside
+    got = s.repair(cands)
+    for i, c in enumerate(cands):
+        assert not s.is_valid(c)
+        r, ham, sad, L = numpy_repair(rows, Ls, c)
+        assert ham >= 1
+        assert (int(got["rank"][i]), int(got["ham"][i]), int(got["sad"][i]), int(got["L"][i])) == (r, ham, sad, L)
+
+
+def test_repair_outside_the_domain_worked_cfg0():
+    # cfg0: bx idx 7 does not exist (m = 5).  Rows (x,0,0) are valid for x = 1..4 (32 <= bx*1 <= 1024 needs bx >= 32):
+    # Hamming 1 each, sum |d| = 7 - x, so (4,0,0) wins with key (1, 3, L = 4*24 = 96).
+    sp, s = oracle_space(0, with_objective=False)
+    got = s.repair(np.array([[7, 0, 0]], np.uint8))
+    assert list(s.rows()[got["rank"][0]]) == [4, 0, 0]
+    assert (int(got["ham"][0]), int(got["sad"][0]), int(got["L"][0])) == (1, 3, 96)
+    assert not s.is_valid(np.array([7, 0, 0], np.uint8))
+
+
 def test_repair_worked_examples_cfg0():
     sp, s = oracle_space(0, with_objective=False)
     rows = s.rows()
