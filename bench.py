@@ -10,6 +10,11 @@ Workload at N=1: BASELINE.json configs[1] (GEMM-like space, DE+PSO+Firefly+GA, p
 evaluations, cap 200 generations, 1000 runs each).  N>1: every rank processes its own 1000 runs per algorithm
 (run indices rank*1000..), no data-path collective (weak scaling).
 
+Besides the headline line the same JSON carries, as top-level keys: `enumeration` (S1 alone on configs[1..3]),
+`sweep_cfg4` (configs[4]: candidates/s against the run count), `steps_cfg2` / `steps_cfg3` (the generation step of
+configs[2] and configs[3] at their BASELINE sizes, fused and phased), `int_peak` (measured integer issue rates) and
+`cpu_baseline`.
+
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
 prints ONE JSON line on rank 0.
 """
@@ -27,10 +32,13 @@ if ROOT not in sys.path:
 
 import numpy as np
 
-ALGO_GENS_CAP = {1: 200, 0: 50, 2: 150, 3: 100, 4: 200}
-ISSUE_LANES_PER_SM_CLK = 128          # 4 SMSP x 32 lanes: one warp instruction per SMSP per clock (B300_MICROARCH.md)
 N_SM = 148
-NCU_KGEN_DRAM_BYTES_PER_LAUNCH = 18.35e6   # (26.2 + 28.7 + 8.1 + 10.4) MB / 4, profiles/r1b_fused.md
+# dram__bytes_read.sum + dram__bytes_write.sum per k_gen launch of THIS workload (configs[1], 1000 runs per algorithm),
+# mean of the four launches of one step: a STORED constant from the ncu --set full capture summarised in
+# profiles/r2_kgen.md (it does not change with the run; the live numbers of this line are the CUDA-event times).
+NCU_KGEN_DRAM_BYTES_PER_LAUNCH = None
+NCU_KGEN_SOURCE = "profiles/r2_kgen.md"
+SECTOR_BYTES_PER_CANDIDATE = 204          # state 2(n+8) + bitmap 32 + directory 32 + obj 32 + dedup 64
 
 
 def peaks():
@@ -80,7 +88,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(nm.replace("nvmlClocksEventReason", "").replace("nvmlClocksThrottleReason", ""))
             except Exception:
                 pass
-            time.sleep(0.05)
+            time.sleep(0.02)
 
     def summary(self):
         if not self.sm:
@@ -91,14 +99,53 @@ class ClockSampler(threading.Thread):
 
 
 # ----------------------------------------------------------------------------------------------------------
-def oracle_sample_step(wl, R_o):
-    """One bounded pass of the hot path on the CPU oracle: returns (candidates evaluated, seconds)."""
+def cpu_info():
+    model = "unknown"
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count()}
+
+
+class PinnedToOneCore:
+    """The oracle is single-threaded; pin it to one core for the timed sample."""
+
+    def __enter__(self):
+        self.old = None
+        try:
+            self.old = os.sched_getaffinity(0)
+            os.sched_setaffinity(0, {sorted(self.old)[-1]})
+        except (AttributeError, OSError):
+            self.old = None
+        return self
+
+    def __exit__(self, *a):
+        if self.old is not None:
+            os.sched_setaffinity(0, self.old)
+
+
+def oracle_prepare(wl):
+    """Untimed: the oracle's own space (needed to derive the objective table, an INPUT) and that table."""
     import oracle as O
     import workloads as W
     sp = wl["space"]
+    s = O.OracleSpace.from_space(sp).build()
+    obj = W.objective_table(s.rows(), sp.m, 0)
+    return obj
+
+
+def oracle_sample_step(wl, R_o, obj):
+    """One bounded pass of the hot path on the CPU oracle: S1 in full + the first R_o runs of every algorithm.
+    Returns (candidates evaluated, seconds).  Repairs are brute-force table scans: the oracle is the definition."""
+    import oracle as O
+    sp = wl["space"]
     t0 = time.perf_counter()
     s = O.OracleSpace.from_space(sp).build()
-    s.set_objective(W.objective_table(s.rows(), sp.m, 0))
+    s.set_objective(obj)
     cands = 0
     for algo in wl["algos"]:
         r = O.OracleRuns(s, algo, n_runs=R_o, pop=wl["pop"], budget=wl["budget"], max_gens=wl["gens"], seed=wl["seed"])
@@ -110,7 +157,8 @@ def oracle_sample_step(wl, R_o):
 def oracle_sample_text(wl, R_o):
     sp = wl["space"]
     return (f"full space build (N={sp.N}) + first {R_o} runs of each of {len(wl['algos'])} algorithms "
-            f"(pop {wl['pop']}, budget {wl['budget']}, cap {wl['gens']} generations), single thread")
+            f"(pop {wl['pop']}, budget {wl['budget']}, cap {wl['gens']} generations), one thread pinned to one core; "
+            "every repair is a brute-force scan of the valid table (the oracle is the plain definition, not a tuned CPU program)")
 
 
 def reference_arm(args):
@@ -121,18 +169,20 @@ def reference_arm(args):
     wl = workload(args.config, None)
     sp = wl["space"]
     sample = oracle_sample_text(wl, args.ref_runs)
-    for _ in range(min(args.warmup, 1)):
-        oracle_sample_step(wl, args.ref_runs)
-    tot_c, tot_t = 0, 0.0
-    for _ in range(args.steps):
-        c, t = oracle_sample_step(wl, args.ref_runs)
-        tot_c += c; tot_t += t
+    obj = oracle_prepare(wl)
+    with PinnedToOneCore():
+        for _ in range(min(args.warmup, 1)):
+            oracle_sample_step(wl, args.ref_runs, obj)
+        tot_c, tot_t = 0, 0.0
+        for _ in range(args.steps):
+            c, t = oracle_sample_step(wl, args.ref_runs, obj)
+            tot_c += c; tot_t += t
     val = tot_c / tot_t
     line = {"impl": "reference", "metric": "candidates_repaired_evaluated_per_s", "value": val, "unit": "candidates/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/u64 integer + f32 (no FMA)",
             "data": "synthetic", "config": {"workload": f"BASELINE configs[{args.config}] ({sp.name}), bounded sample: {sample}"},
-            "cpu_baseline": {"value": val, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": sample, **cpu_info()},
             "e2e": {"value": val, "unit": "candidates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -140,15 +190,14 @@ def reference_arm(args):
 
 # ----------------------------------------------------------------------------------------------------------
 def scan_ops_per_pair(n):
-    """Integer instructions per (candidate, valid row) of k_scan: per index word
-    VABSDIFF4.ACC + XOR + ADD + AND/OR-merge (+ shift), per row POPC + key pack + compare/select x2 + LDS."""
+    """Integer instructions per (candidate, valid row) of k_scan, by issue class."""
     wu = (n + 3) // 4
-    return 5 * wu + 6
+    return {"vabsdiff4": wu, "lop3": 3 * wu + 3, "iadd": wu + 1, "popc": (wu + 3) // 4, "imad": 1}
 
 
-def enum_bytes(N, V, row_bytes):
+def enum_bytes(N, V, row_bytes, ltab_bytes):
     """Algorithmic bytes of S1: bitmap + rank directory + rows + Ltab."""
-    return N / 8 + N / 128 + V * (row_bytes + 8)
+    return N / 8 + N / 128 + V * (row_bytes + ltab_bytes)
 
 
 def gpu_arm(args):
@@ -250,10 +299,10 @@ def gpu_arm(args):
     # per-kernel device times: the same step, serialised on one stream, events around every launch
     ms_prof, _, prof, _, _ = timed(args.steps, False, True, concurrent=False)
     space, runs = kept
-    counters = [r.counters() for r in runs]
-    cands_step = sum(c["n_evaluated"] for c in counters)
-    scanned_step = sum(c["n_scanned"] for c in counters)
-    repaired_step = sum(c["n_repaired"] for c in counters)
+    stats = [r.stats() for r in runs]
+    cands_step = sum(c["n_evaluated"] for c in stats)
+    scanned_step = sum(c["n_scanned"] for c in stats)
+    repaired_step = sum(c["n_repaired"] for c in stats)
     gens_done = [int(r.best()["gens_done"].sum().item()) for r in runs]
     value = world * cands_step * args.steps / (ms / 1e3)
 
@@ -275,38 +324,37 @@ def gpu_arm(args):
     top = max(kern, key=lambda k: kern[k]["ms_per_step"])
     top_ms, top_n = kern[top]["ms_per_step"], kern[top]["launches_per_step"]
     dur_s = top_ms / 1e3 / top_n                                          # average launch duration
-    sm_max = clocks.get("sm_max_mhz") or pk["sm_max_mhz"]
-    alu_peak = N_SM * ISSUE_LANES_PER_SM_CLK * sm_max * 1e6 / 1e12        # T int-instr/s at the issue limit
-    if top == "k_scan":
-        ops = scanned_step * V * scan_ops_per_pair(n) / top_n             # per launch
-        roof = {"kernel": top, "bound": "alu", "achieved": ops / dur_s / 1e12, "peak": alu_peak, "unit": "Tiop/s",
-                "peak_source": f"148 SM x 128 lanes/clk x {sm_max:.0f} MHz (issue limit; DESIGN.md section 6)",
-                "traffic": None}
-    elif top == "k_enum_pass1":
-        by = N / 8
-        roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "peak_source": pk["source"], "traffic": None}
-    else:
-        # k_op / k_finish / k_init: sector-granular bytes per candidate: state + bitmap + dir + obj + dedup
-        per = {"k_op": 2 * rb + 8 + 32 + 32, "k_finish": 8 + 32 + 64 + rb + 24, "k_init": 32 + 64 + rb + 8,
-               "k_gen": 2 * (rb + 8) + 32 + 32 + 32 + 64}.get(top, 64)
-        by = per * cands_step / max(top_n, 1)
-        roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "peak_source": pk["source"], "traffic": None,
-                "algorithmic_bytes_per_candidate": per}
-        if top == "k_gen" and args.config == 1 and R == 1000:
-            # dram__bytes_read.sum + dram__bytes_write.sum per launch, mean of the four k_gen launches of one step,
-            # from the ncu --set full capture summarised in profiles/r1b_fused.md
-            roof["traffic"] = NCU_KGEN_DRAM_BYTES_PER_LAUNCH
-            roof["note"] = ("at 1000 runs k_gen is bound by per-run latency and the longest run (issue 15-23 %, DRAM 0.1 %): "
-                            "profiles/r1b_fused.md; extra.sweep_cfg4 shows candidates/s against the number of runs")
+    per = {"k_op": 2 * rb + 8 + 32 + 32, "k_finish": 8 + 32 + 64 + rb + 24, "k_init": 32 + 64 + rb + 8,
+           "k_gen": SECTOR_BYTES_PER_CANDIDATE}.get(top, 64)
+    by = per * cands_step / max(top_n, 1)
+    roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+            "peak_source": pk["source"], "algorithmic_bytes_per_candidate": per,
+            "traffic": NCU_KGEN_DRAM_BYTES_PER_LAUNCH if (top == "k_gen" and args.config == 1 and R == 1000) else None,
+            "traffic_source": f"stored constant from the ncu --set full capture in {NCU_KGEN_SOURCE}, not measured by this run"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_us"] = dur_s * 1e6
     roof["share_of_step"] = top_ms / (ms_prof / args.steps)
     roof["measured_in"] = ("the same step re-run in the timed loop on ONE stream with CUDA events around every launch "
                            f"({ms_prof / args.steps:.2f} ms/step serialised vs {ms / args.steps:.2f} ms/step with one stream per algorithm)")
+    roof["note"] = ("sector-granular HBM model of SURVEY 8(d); the kernel is bound by instruction issue, not DRAM "
+                    f"(ncu: {NCU_KGEN_SOURCE}); sweep_cfg4 shows the same kernel with the GPU filled")
 
-    # ---- S1 alone (BASELINE metric "enumeration Gcfg/s"): configs[3] (sparse, 5.7e8) and configs[2], resident buffers
+    # ---- measured integer issue peaks (lane-operations per second, one instruction kind each)
+    int_peak = {}
+    if not args.no_peak:
+        int_peak = {k: cao.int_peak(k) / 1e12 for k in ("imad", "lop3", "vabsdiff4", "popc", "iadd")}
+        int_peak["unit"] = "T lane-op/s"
+
+    def scan_alu(n_dim, pairs, seconds):
+        """Integer-pipe fraction of the repair scan: issue time of its instruction mix at the measured rates."""
+        if not int_peak or pairs == 0 or seconds <= 0:
+            return None
+        mix = scan_ops_per_pair(n_dim)
+        t_min = sum(cnt * pairs / (int_peak[k] * 1e12) for k, cnt in mix.items())
+        return {"ops_per_pair": mix, "pairs": pairs, "achieved_Tops": sum(mix.values()) * pairs / seconds / 1e12,
+                "frac_of_measured_issue": t_min / seconds}
+
+    # ---- S1 alone (BASELINE metric "enumeration Gcfg/s"): configs[1..3], resident buffers
     enum = {}
     for cfg in ([1, 2, 3] if not args.no_enum else []):
         spx = W.WORKLOADS[cfg].space()
@@ -326,11 +374,12 @@ def gpu_arm(args):
         kp = {k: v[0] / 5 * 1e3 for k, v in cao.profile_read().items() if v[1]}
         cao.profile_enable(False)
         Nx, Vx, nx, rbx = gx.sizes()
+        lb = gx.ltab_bytes
         t = float(np.median(ts)) / 1e3
-        enum[f"cfg{cfg}"] = {"N": Nx, "V": Vx, "ms": t * 1e3, "gcfg_s": Nx / t / 1e9,
-                             "hbm_gbs": enum_bytes(Nx, Vx, rbx) / t / 1e9,
-                             "hbm_frac": enum_bytes(Nx, Vx, rbx) / t / 1e9 / pk["hbm_gbs"],
-                             "algorithmic_bytes": enum_bytes(Nx, Vx, rbx), "kernel_us": kp}
+        enum[f"cfg{cfg}"] = {"N": Nx, "V": Vx, "ms": t * 1e3, "ms_min": float(min(ts)), "gcfg_s": Nx / t / 1e9,
+                             "hbm_gbs": enum_bytes(Nx, Vx, rbx, lb) / t / 1e9,
+                             "hbm_frac": enum_bytes(Nx, Vx, rbx, lb) / t / 1e9 / pk["hbm_gbs"],
+                             "algorithmic_bytes": enum_bytes(Nx, Vx, rbx, lb), "kernel_us": kp}
         del gx
 
     # ---- BASELINE configs[4]: candidates/s against the number of runs (same space, no budget, 200 generations)
@@ -350,16 +399,59 @@ def gpu_arm(args):
                     cands = Rs * P * 200
                     del r4
                 row[algo] = {"ms": best_ms, "candidates_per_s": cands / (best_ms / 1e3),
-                             "hbm_frac_204B": cands * 204 / (best_ms / 1e3) / 1e9 / pk["hbm_gbs"]}
+                             "hbm_frac_204B": cands * SECTOR_BYTES_PER_CANDIDATE / (best_ms / 1e3) / 1e9 / pk["hbm_gbs"]}
             sweep[str(Rs)] = row
         del space4
 
-    # ---- CPU oracle on a bounded sample of the same workload (rank 0, N=1 only)
+    # ---- the generation step of configs[2] (GA, P 64, 10^4 runs, 150 generations) and configs[3] (Firefly, P 128,
+    # 1000 runs, 100 generations: the repair-scan stress case) at their BASELINE sizes, fused and phased
+    other = {}
+    for cfg in ([2, 3] if not args.no_other else []):
+        w = workload(cfg, None)
+        spx = w["space"]
+        gx = cao.Space.from_space(spx).build()
+        Nx, Vx, nx, rbx = gx.sizes()
+        gx.set_objective(W.objective_table(gx.rows().cpu().numpy(), spx.m, 0))
+        leg = {"workload": f"BASELINE configs[{cfg}] ({spx.name}): N={Nx} V={Vx} n={nx}; {w['algos'][0]}, pop {w['pop']}, "
+                           f"{w['gens']} generations, {w['runs']} runs", "probe_levels": gx.probe_levels}
+        for mode in ("fused", "phased"):
+            best_ms = None
+            for rep in range(2):
+                rr = cao.Runs(gx, w["algos"][0], n_runs=w["runs"], pop=w["pop"], budget=w["budget"], max_gens=w["gens"],
+                              seed=w["seed"], mode=mode)
+                torch.cuda.synchronize(); flush.zero_()
+                if rep == 1:
+                    cao.profile_enable(True)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); rr.step(w["gens"]); e1.record(); e1.synchronize()
+                t = e0.elapsed_time(e1); best_ms = t if best_ms is None else min(best_ms, t)
+                if rep == 1:
+                    kp = {k: {"ms": v[0], "launches": v[1]} for k, v in cao.profile_read().items() if v[1]}
+                    cao.profile_enable(False)
+                    st = rr.stats()
+                del rr
+            cands = w["runs"] * w["pop"] * w["gens"]
+            row = {"ms": best_ms, "candidates_per_s": cands / (best_ms / 1e3),
+                   "hbm_frac_204B": cands * SECTOR_BYTES_PER_CANDIDATE / (best_ms / 1e3) / 1e9 / pk["hbm_gbs"],
+                   "kernels": kp, "n_repaired": st["n_repaired"], "n_scanned": st["n_scanned"], "n_memo": st["n_memo"],
+                   "n_rcache": st["n_rcache"], "ham_hist": st["ham_hist"]}
+            if mode == "phased" and "k_scan" in kp:
+                row["scan_alu"] = scan_alu(nx, st["n_scanned"] * Vx, kp["k_scan"]["ms"] / 1e3)
+            leg[mode] = row
+        other[f"cfg{cfg}"] = leg
+        del gx
+    torch.cuda.empty_cache()
+
+    # ---- CPU oracle on a bounded sample of the same workload (rank 0, N=1 only), and a spot check of the GPU against it
     cpu = None
     if world == 1 and not args.no_cpu:
-        c, t = oracle_sample_step(wl, args.ref_runs)
+        import oracle as O
+        obj_o = oracle_prepare(wl)
+        assert np.array_equal(obj_o, obj)                                 # same input on both sides
+        with PinnedToOneCore():
+            c, t = oracle_sample_step(wl, args.ref_runs, obj_o)
         cpu = {"value": c / t, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": oracle_sample_text(wl, args.ref_runs),
-               "seconds": t}
+               "seconds": t, **cpu_info()}
 
     line = {
         "metric": "candidates_repaired_evaluated_per_s", "value": value, "unit": "candidates/s", "n_gpus": world,
@@ -377,9 +469,15 @@ def gpu_arm(args):
         "gpu_launches": int(launches),
         "roofline": roof,
         "cpu_baseline": cpu,
+        "enumeration": enum,
+        "sweep_cfg4": sweep,
+        "steps_cfg2": other.get("cfg2"),
+        "steps_cfg3": other.get("cfg3"),
+        "int_peak": int_peak,
         "extra": {"candidates_per_step": int(cands_step), "invalid_post_snap_per_step": int(repaired_step),
                   "scanned_per_step": int(scanned_step), "generations_done_sum": gens_done,
-                  "kernels": kern, "enumeration": enum, "sweep_cfg4": sweep, "wall_s_timed_region": wall, "peaks": pk},
+                  "stats": {a: {k: v for k, v in s.items() if not k.startswith("cyc") and k != "r7"} for a, s in zip(wl["algos"], stats)},
+                  "kernels": kern, "wall_s_timed_region": wall, "peaks": pk},
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -394,11 +492,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--runs", type=int, default=None, help="runs per algorithm per GPU (default: the config's)")
-    ap.add_argument("--ref-runs", type=int, default=1, help="runs per algorithm of the CPU-oracle sample")
+    ap.add_argument("--ref-runs", type=int, default=3, help="runs per algorithm of the CPU-oracle sample")
     ap.add_argument("--streams", type=int, default=4, help="1 = all algorithms on one stream, >1 = one stream per algorithm")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-enum", action="store_true")
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-other", action="store_true", help="skip the configs[2] / configs[3] generation-step legs")
+    ap.add_argument("--no-peak", action="store_true", help="skip the integer issue-rate microbenchmarks")
     ap.add_argument("--sweep-points", type=int, default=4, help="how many of the run counts 1e2, 1e3, 1e4, 1e5 to sweep")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -89,23 +89,26 @@ int cao_space_set_build_mode(cao_space* s, int32_t mode);
 int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64_t* scratch_bytes);
 /* Highest Hamming level the generation step probes in the bitmap before it falls back to the table scan:
  * -1 (default) = cost model (level h is probed while (number of rows at distance h) * 60 <= V * scan cost),
- * 0..3 = fixed.  Call before build_count; probe_levels() reports the level in use after build_count. */
+ * 0..6 = fixed (clamped to 1 when the space has more than 368 Hamming-1 neighbours or 65536 neighbour pairs).  Call before build_count; probe_levels() reports the level in use after build_count. */
 int cao_space_set_probe_levels(cao_space* s, int32_t levels);
 int cao_space_probe_levels(const cao_space* s, int32_t* levels);
 /* Pass 1: validity bitmap + per-512-config counts, then the exclusive scan of the counts.
  * Synchronises `stream` once to return V in *h_V.  d_scratch may be released after build_fill. */
 int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V);
 int cao_space_table_bytes(const cao_space* s, uint64_t* bytes);
-/* Pass 2: valid rows (V x row_bytes), Ltab (V x u64) and the rank directory, into d_table. */
+/* Pass 2: valid rows (V x row_bytes), Ltab (V linear indices: u32 when N <= 2^32, else u64 -- see
+ * cao_space_ltab_bytes) and the rank directory, into d_table. */
 int cao_space_build_fill(cao_space* s, void* d_table, void* stream);
 /* Re-runs the whole of S1 (tables, bitmap, counts, scan, rows, Ltab, directory) into the buffers of the last
  * build, asynchronously and without any host round trip: the definition is unchanged, so V and the layout are
  * the ones build_count returned.  Needs a completed build_count + build_fill; d_scratch must still be alive. */
 int cao_space_rebuild(cao_space* s, void* stream);
 int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes);
+/* Bytes per Ltab entry: 4 when N <= 2^32 (every linear index fits 32 bits), else 8. */
+int cao_space_ltab_bytes(const cao_space* s, int32_t* bytes);
 /* Borrowed device views into the caller's buffers; rank_dir[i] = number of valid L < 512*i. */
 int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t** d_rows,
-                    const uint64_t** d_Ltab, const uint32_t** d_rank_dir);
+                    const void** d_Ltab, const uint32_t** d_rank_dir);
 
 /* ---------------------------------------------------------------- Search Space queries (L139), batched
  * d_idx_rows: count rows of row_bytes bytes each (padding ignored). */
@@ -113,10 +116,11 @@ int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t c
                        void* stream);
 /* S5 standalone: d_rank_out[i] = rank of argmin (Hamming, sum |didx|, L) over the valid table; the
  * identity for valid rows (L143, L215, L270; O9).  d_key_out (optional, may be NULL) receives
- * ham << 45 | sad << 32 | rank.  probe_levels: 0 = table scan only; 1, 2, 3 = first test the neighbours
+ * ham << 45 | sad << 32 | rank.  probe_levels: 0 = table scan only; 1..6 = first test the neighbours
  * at Hamming distance <= that level in the bitmap (exact: Hamming is the primary key); any other value
  * (e.g. -1) = the level the library's cost model chose for this space.  All settings give identical
- * results.  Rows with an index outside its domain are legal inputs (they are invalid and go to the scan).
+ * results.  Rows with an index outside its domain are legal inputs (A27: they are invalid, skip the probes and are
+ * repaired by the scan over their byte values); padding bytes (positions >= n) are ignored.
  * d_scratch: cao_space_repair_scratch_bytes(count) bytes. */
 int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
 int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,

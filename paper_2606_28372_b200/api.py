@@ -53,6 +53,7 @@ SIGNATURES = {
     "cao_space_build_fill": (C.c_int, [vp, vp, vp]),
     "cao_space_rebuild": (C.c_int, [vp, vp]),
     "cao_space_sizes": (C.c_int, [vp, pu64, pu64, pi32, pi32]),
+    "cao_space_ltab_bytes": (C.c_int, [vp, pi32]),
     "cao_space_views": (C.c_int, [vp, pvp, pvp, pvp, pvp]),
     "cao_space_is_valid": (C.c_int, [vp, vp, u64, vp, vp]),
     "cao_space_repair_scratch_bytes": (C.c_int, [vp, u64, pu64]),
@@ -228,9 +229,17 @@ class Space:
         N, V, n, rb = self.sizes()
         return _view(self._table, self._views()[1], V * rb, torch.uint8, (V, rb))
 
+    @property
+    def ltab_bytes(self) -> int:
+        v = i32()
+        _check(lib().cao_space_ltab_bytes(self._h, C.byref(v)))
+        return v.value
+
     def Ltab(self) -> torch.Tensor:
+        """V linear indices, ascending: int32 bit patterns of u32 when N <= 2^32, else int64."""
         N, V, n, rb = self.sizes()
-        return _view(self._table, self._views()[2], V * 8, torch.int64, (V,))
+        lb = self.ltab_bytes
+        return _view(self._table, self._views()[2], V * lb, torch.int32 if lb == 4 else torch.int64, (V,))
 
     def rank_dir(self) -> torch.Tensor:
         N, V, n, rb = self.sizes()

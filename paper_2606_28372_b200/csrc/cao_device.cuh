@@ -18,11 +18,12 @@ struct SpaceMeta {
     uint64_t magic[CAO_MAX_DIMS];       // ceil(2^64 / m_d) for m_d >= 2 (exact division of any L < 2^56)
     const uint64_t* bitmap;             // ceil(N/64) words
     const uint8_t* rows;                // V x rowB, ascending L, padding bytes zero
-    const uint64_t* Ltab;               // V
+    const void* Ltab;                   // V linear indices: u32 when N <= 2^32 (ltab32), else u64
     const uint32_t* dir;                // ceil(N/512)+1 exclusive counts
     const float* obj;                   // V
     uint32_t V;
     int32_t n, rowB, M;                 // M = max_d m_d (O6)
+    int32_t ltab32;
     uint16_t m[CAO_MAX_DIMS];
 };
 
@@ -144,6 +145,10 @@ __device__ __forceinline__ uint32_t rank_of(const SpaceMeta& sm, uint64_t L) {
         r += q1 < wi ? __popcll(v.y) : q1 == wi ? __popcll(v.y & below_mask) : 0;
     }
     return r;
+}
+
+__device__ __forceinline__ uint64_t ltab_at(const SpaceMeta& sm, uint32_t r) {
+    return sm.ltab32 ? (uint64_t)__ldg(&((const uint32_t*)sm.Ltab)[r]) : __ldg(&((const uint64_t*)sm.Ltab)[r]);
 }
 
 // Exact L / m and L % m through the precomputed reciprocal (m >= 2, L < 2^56).

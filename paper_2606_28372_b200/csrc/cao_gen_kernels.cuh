@@ -559,7 +559,7 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
         if (has) {
             uint32_t row[ROWW];
             load_row<ROWW>(sm.rows + (uint64_t)rk * RB, row);
-            Lr = __ldg(&sm.Ltab[rk]);
+            Lr = ltab_at(sm, rk);
 #pragma unroll
             for (int z = 0; z < ROWW; ++z) S.idx[i * ROWW + z] = row[z];
         }

@@ -30,11 +30,12 @@ static inline uint64_t align256(uint64_t x) { return (x + 255) & ~255ull; }
 // One constraint in the enumeration plan.
 struct ConsPlan {
     bool tabled = false;
-    std::vector<int> scope;            // parameters the program reads, ascending
+    std::vector<int> scope;            // parameters the program reads, descending
     std::vector<int> outer;            // scope digits < t (outer part)
     std::vector<uint32_t> cstride;     // mixed-radix strides of the outer scope digits (row index of the table)
     uint64_t rows = 1;                 // product of m_d over the outer scope digits
     uint64_t table_off = 0;            // u64-word offset of the table inside the tables region
+    uint64_t flag_off = 0;             // byte offset of its row flags inside the flags region
 };
 
 struct cao_space {
@@ -46,15 +47,15 @@ struct cao_space {
     // enumeration plan
     int t = 0;                         // first inner digit: digits t..n-1 form one bitmap block of B configs
     uint64_t B = 0, n_blocks = 0, nd = 0, n_words = 0;
-    uint32_t Wb = 0, nb = 0, nb_tabled = 0;           // u64 words per block mask; blocks per CTA
+    uint32_t Wb = 0, CH = 1;           // u64 words per block mask; blocks per thread of k_enum
     std::vector<ConsPlan> plan;
     std::vector<int32_t> desc;         // descriptor words uploaded to the device
-    int n_tab = 0, n_res = 0, n_rc = 0;
-    int rc_pc0[4] = {0, 0, 0, 0};
-    uint64_t off_rc[4] = {0, 0, 0, 0}, rc_bytes = 0;
+    int n_tab = 0, n_res = 0;
+    bool use_lut = false;
     // scratch layout (byte offsets)
-    uint64_t off_dom = 0, off_desc = 0, off_tables = 0, off_cnt = 0, off_part = 0, off_V = 0, scratch_bytes = 0;
-    uint64_t tables_words = 0, n_part = 0, max_table_threads = 0, max_table_ci = 1;
+    uint64_t off_dom = 0, off_desc = 0, off_tables = 0, off_flags = 0, off_lut = 0, off_cnt = 0, off_part = 0, off_V = 0,
+             off_live = 0, off_groups = 0, scratch_bytes = 0;
+    uint64_t tables_words = 0, flags_bytes = 0, n_part = 0, max_table_threads = 0, max_table_ci = 1;
     uint64_t bitmap_bytes = 0;
     void* d_scratch = nullptr;
     void* d_table = nullptr;
@@ -66,34 +67,24 @@ struct cao_space {
     std::vector<uint32_t> h_pairs;
     uint64_t off_pairs = 0;
     int probe_levels_req = -1;         // -1 = cost model
+    // the zero fill of the bitmap runs on a side stream, overlapped with the table build
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
-// Arguments of the pass-1 kernel, passed by value.
-// Residual constraint handled through value classes: blocks whose program prefix leaves the
-// same single stack value share one inner mask.
-#define CAO_HS 4096                         // hash slots = maximum number of distinct prefix values
-#define CAO_MAX_RC 4
-#define CAO_CLS_EMPTY ((long long)0x8080808080808080ll)   // below -2^62: never a saturated value
-#define CAO_CLS_FALSE 0xFFFFFFFFu
-#define CAO_CLS_OVERFLOW 0xFFFFFFFEu
-struct ResClassArgs {
-    long long* keys;                   // CAO_HS prefix values (CAO_CLS_EMPTY = free)
-    uint64_t* table;                   // CAO_HS x Wb inner masks
-    uint32_t* blk_class;               // n_blocks: hash slot of the block's prefix value
-    int32_t* overflow;                 // set if more than the table holds: the constraint falls back to phase 1b
-    int32_t pc0;                       // first token of the suffix
-};
-
+// Arguments of the pass-1 kernels, passed by value.
 struct EnumArgs {
-    uint64_t B, magicB, n_blocks, n_words;
+    uint64_t B, n_blocks;
     const int64_t* dom;                // [n][256]
     const int32_t* desc;
     const uint64_t* tables;
-    uint64_t* bitmap;
+    const uint8_t* flags;              // one byte per table row: the row has a bit set
+    uint64_t* bitmap;                  // zero-filled
     uint32_t* cnt;                     // per-512 counts (zeroed)
-    uint32_t Wb, nb;
-    int32_t t, n_tab, n_res, n_rc;     // the first n_rc residual constraints use value classes
-    ResClassArgs rc[CAO_MAX_RC];
+    uint32_t* live;                    // blocks that survive the tables (only with residual constraints)
+    uint32_t* live_count;
+    uint32_t Wb, CH;
+    int32_t t, n_tab, n_res;
 };
 
 struct cao_runs;

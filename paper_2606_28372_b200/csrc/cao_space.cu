@@ -97,7 +97,13 @@ int cao_space_create(cao_space** out) {
     *out = new cao_space();
     return CAO_OK;
 }
-void cao_space_destroy(cao_space* s) { delete s; }
+void cao_space_destroy(cao_space* s) {
+    if (!s) return;
+    if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+    if (s->ev_join) cudaEventDestroy(s->ev_join);
+    if (s->side) cudaStreamDestroy(s->side);
+    delete s;
+}
 
 int cao_space_add_param(cao_space* s, const char*, const int64_t* h_values, int32_t n_values) {
     if (!s || !h_values) return cao_fail(CAO_E_INVALID_ARG, "cao_space_add_param: NULL argument");
@@ -153,17 +159,17 @@ static int plan_space(cao_space* s) {
         if (N >= ((unsigned __int128)1 << 40)) return cao_fail(CAO_E_TOO_LARGE, "Cartesian size N >= 2^40");
     }
     M.N = (uint64_t)N;
+    M.ltab32 = M.N <= (1ull << 32) ? 1 : 0;                       // Ltab holds u32 when every L fits (SURVEY 8(a) layout)
     // inner block: smallest trailing product >= 256 (or the whole space)
     uint64_t B = 1; int t = n;
     while (t > 0 && B < 256) { --t; B *= M.m[t]; }
     s->t = t; s->B = B; s->Wb = (uint32_t)((B + 63) / 64); s->n_blocks = M.N / B;
     s->n_words = (M.N + 63) / 64; s->nd = (M.N + 511) / 512;
-    int64_t nb = (int64_t)(40960 / ((uint64_t)s->Wb * 8)) - 1;
-    s->nb = (uint32_t)std::min<int64_t>(256, std::max<int64_t>(1, nb));
-    s->nb_tabled = s->nb;
+    // blocks per thread of k_enum: one decode per thread, then an odometer; keep at least ~150 k threads
+    s->CH = (uint32_t)std::min<uint64_t>(16, std::max<uint64_t>(1, s->n_blocks / (148ull * 1024)));
     // per-constraint plan
     s->plan.assign(s->cons.size(), ConsPlan());
-    uint64_t total_words = 0;
+    uint64_t total_words = 0, total_flags = 0;
     for (size_t c = 0; c < s->cons.size(); ++c) {
         ConsPlan& p = s->plan[c];
         const auto& w = s->cons[c];
@@ -184,45 +190,16 @@ static int plan_space(cao_space* s) {
         p.rows = rows;
         uint64_t words = rows * s->Wb;
         p.tabled = s->mode == 0 && ok && words * 8 <= (8ull << 20) && (total_words + words) * 8 <= (128ull << 20);
-        if (p.tabled) { p.table_off = total_words; total_words += words; }
+        if (p.tabled) { p.table_off = total_words; total_words += words; p.flag_off = total_flags; total_flags += rows; }
     }
-    s->tables_words = total_words;
-    // descriptors: small tables first, then residual programs
+    s->tables_words = total_words; s->flags_bytes = total_flags;
+    // descriptors: small tables first (the cheapest, usually most selective tests come first), then residual programs
     std::vector<int> tab, res;
     for (size_t c = 0; c < s->cons.size(); ++c) (s->plan[c].tabled ? tab : res).push_back((int)c);
     std::stable_sort(tab.begin(), tab.end(), [&](int a, int b) { return s->plan[a].rows < s->plan[b].rows; });
     s->n_tab = (int)tab.size(); s->n_res = (int)res.size();
-    // Value classes: a residual program whose tokens before the first inner parameter leave exactly one stack
-    // value, and whose remaining tokens read inner parameters only, depends on the outer digits through that one
-    // value.  Such constraints come first in the residual list.
-    std::vector<int> cls_pc0(s->cons.size(), -1);
-    if (s->mode == 0 && (uint64_t)CAO_HS * s->Wb * 8 <= (32ull << 20)) {
-        for (int c : res) {
-            const auto& w = s->cons[c];
-            int sp = 0, pc0 = -1; bool ok = true;
-            for (size_t pc = 0; pc < w.size(); ++pc) {
-                const int op = w[pc];
-                if (op == CAO_OP_PUSH_PARAM) {
-                    const int d = w[pc + 1];
-                    if (pc0 < 0 && d >= t) { pc0 = (int)pc; if (sp != 1) ok = false; }
-                    else if (pc0 >= 0 && d < t) ok = false;               // the suffix reads an outer parameter
-                    ++pc; ++sp;
-                } else if (op == CAO_OP_PUSH_CONST) { pc += 2; ++sp; }
-                else if (op == CAO_OP_NEG || op == CAO_OP_NOT) {}
-                else --sp;
-            }
-            if (ok && pc0 > 0) cls_pc0[c] = pc0;
-        }
-        std::stable_sort(res.begin(), res.end(), [&](int a, int b) { return (cls_pc0[a] >= 0) > (cls_pc0[b] >= 0); });
-    }
-    s->n_rc = 0;
-    for (int c : res) if (cls_pc0[c] >= 0 && s->n_rc < CAO_MAX_RC) s->rc_pc0[s->n_rc++] = cls_pc0[c];
-    // residual constraints outside the classes are evaluated by one warp per block: fewer blocks per CTA keep
-    // the CTAs balanced
-    if (s->n_res > s->n_rc) s->nb = std::min<uint32_t>(s->nb, 32);
     std::vector<int32_t>& D = s->desc;
     D.assign(tab.size() + res.size() + s->cons.size(), 0);       // [tab offs][res offs][program offs of every constraint]
-    // programs first, so that the tabled descriptors can point at them
     std::vector<int32_t> prog_off(s->cons.size());
     for (size_t c = 0; c < s->cons.size(); ++c) {
         prog_off[c] = (int32_t)D.size();
@@ -234,6 +211,7 @@ static int plan_space(cao_space* s) {
         const ConsPlan& p = s->plan[tab[k]];
         D[k] = (int32_t)D.size();
         D.push_back((int32_t)(uint32_t)p.table_off); D.push_back((int32_t)(uint32_t)(p.table_off >> 32));
+        D.push_back((int32_t)(uint32_t)p.flag_off);
         D.push_back((int32_t)p.outer.size());
         for (size_t e = 0; e < p.outer.size(); ++e) { D.push_back(p.outer[e]); D.push_back((int32_t)p.cstride[e]); }
         D.push_back(prog_off[tab[k]]); D.push_back((int32_t)s->cons[tab[k]].size()); D.push_back((int32_t)p.rows);
@@ -253,17 +231,20 @@ static int plan_space(cao_space* s) {
         D.push_back((int32_t)s->cons[res[k]].size());
         D.insert(D.end(), s->cons[res[k]].begin(), s->cons[res[k]].end());
     }
+    s->use_lut = B * (uint64_t)M.rowB <= (1ull << 20);            // inner index bytes of every pattern (pass 2)
     // scratch layout
     uint64_t off = 0;
     s->off_dom = off; off = align256(off + (uint64_t)n * 256 * 8);
     s->off_desc = off; off = align256(off + D.size() * 4);
     s->off_tables = off; off = align256(off + std::max<uint64_t>(1, total_words) * 8);
-    s->off_cnt = off; off = align256(off + (s->nd + 1) * 4);
+    s->off_flags = off; off = align256(off + std::max<uint64_t>(1, total_flags));
+    s->off_lut = off; off = align256(off + (s->use_lut ? B * (uint64_t)M.rowB : 1));
     s->n_part = (s->nd + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK;
     s->off_part = off; off = align256(off + s->n_part * 4);
-    s->off_V = off; off = align256(off + 8);
-    s->rc_bytes = align256((uint64_t)CAO_HS * 8) + align256((uint64_t)CAO_HS * s->Wb * 8) + align256(s->n_blocks * 4) + 256;
-    for (int k = 0; k < s->n_rc; ++k) { s->off_rc[k] = off; off += s->rc_bytes; }
+    s->off_V = off; off = align256(off + 32);                     // V (u64), scan ticket, live count, group count
+    s->off_cnt = off; off = align256(off + (s->nd + 1) * 4);
+    s->off_live = off; off = align256(off + (s->n_res ? s->n_blocks : 1) * 4);
+    s->off_groups = off; off = align256(off + (s->nd + 1) * 4);
     s->scratch_bytes = off;
     s->bitmap_bytes = align256(s->n_words * 8);
     s->planned = true;
@@ -277,77 +258,90 @@ int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64
     return CAO_OK;
 }
 
-// S1 pass 1 on `st`: constraint tables, block masks -> bitmap + per-512 counts, exclusive scan of the counts.
+// S1 pass 1 on `st`: zero fill (side stream) || constraint tables, then block masks -> bitmap + per-512 counts,
+// residual constraints on the survivors, and the first half of the count scan (V).
 static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t st) {
-    CAO_CUDA(cudaMemsetAsync(sc + s->off_cnt, 0, (s->nd + 1) * 4, st));
+    if (!s->side) {
+        CAO_CUDA(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
+        CAO_CUDA(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
+        CAO_CUDA(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+    }
     s->meta.bitmap = (const uint64_t*)d_bitmap;
+    // fork: the zero fill of the bitmap (N/8 bytes, HBM-bound) overlaps the table build (latency-bound)
+    CAO_CUDA(cudaEventRecord(s->ev_fork, st));
+    CAO_CUDA(cudaStreamWaitEvent(s->side, s->ev_fork, 0));
+    CAO_CUDA(cudaMemsetAsync(d_bitmap, 0, s->bitmap_bytes, s->side));
+    CAO_CUDA(cudaMemsetAsync(sc + s->off_V, 0, (s->off_cnt - s->off_V) + (s->nd + 1) * 4, s->side));   // V, tickets, counts
+    CAO_CUDA(cudaEventRecord(s->ev_join, s->side));
     const int64_t* d_dom = (const int64_t*)(sc + s->off_dom);
     const int32_t* d_desc = (const int32_t*)(sc + s->off_desc);
     uint64_t* d_tables = (uint64_t*)(sc + s->off_tables);
+    uint8_t* d_flags = sc + s->off_flags;
     if (s->n_tab) {
         ProfScope ps(PK_TABLE, st);
-        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 255) / 256, 148 * 16), (unsigned)s->n_tab);
-        const size_t tsm = (size_t)std::max<uint64_t>(256, s->max_table_ci);      // <= B <= 65,280 bytes
+        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 2047) / 2048, 148 * 8), (unsigned)s->n_tab);
+        const uint32_t ci_cap = s->B <= 8192 ? (uint32_t)((s->B + 7) & ~7ull) : 0;
+        const size_t tsm = 2 * (size_t)ci_cap + (size_t)std::max<uint64_t>(256, s->max_table_ci);
         if (tsm > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_build_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
-        k_build_tables<<<grid, 256, tsm, st>>>(s->meta, d_dom, d_desc, d_tables, s->B, s->Wb, s->t);
+        k_build_tables<<<grid, 256, tsm, st>>>(s->meta, d_dom, d_desc, d_tables, d_flags, s->B, s->Wb, s->t, ci_cap);
         CAO_LAUNCHED("k_build_tables");
     }
-    EnumArgs ea{};
-    ea.n_rc = s->n_rc;
-    for (int k = 0; k < s->n_rc; ++k) {
-        uint8_t* b = sc + s->off_rc[k];
-        ResClassArgs& rc = ea.rc[k];
-        rc.keys = (long long*)b; b += align256((uint64_t)CAO_HS * 8);
-        rc.table = (uint64_t*)b; b += align256((uint64_t)CAO_HS * s->Wb * 8);
-        rc.blk_class = (uint32_t*)b; b += align256(s->n_blocks * 4);
-        rc.overflow = (int32_t*)b;
-        rc.pc0 = s->rc_pc0[k];
-        CAO_CUDA(cudaMemsetAsync(rc.keys, 0x80, (uint64_t)CAO_HS * 8, st));
-        CAO_CUDA(cudaMemsetAsync(rc.overflow, 0, 4, st));
+    if (s->use_lut) {
         ProfScope ps(PK_TABLE, st);
-        k_res_prefix<<<(unsigned)((s->n_blocks + 255) / 256), 256, 0, st>>>(s->meta, d_dom, d_desc, s->n_tab + k, rc, s->n_blocks, s->t);
-        CAO_LAUNCHED("k_res_prefix");
-        const uint64_t threads = (uint64_t)CAO_HS * s->Wb * 64;
-        k_res_class_table<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(s->meta, d_dom, d_desc, s->n_tab + k, rc, s->B, s->Wb, s->t);
-        CAO_LAUNCHED("k_res_class_table");
+        k_inner_lut<<<(unsigned)((s->B + 255) / 256), 256, 0, st>>>(s->meta, (uint32_t*)(sc + s->off_lut), s->B, s->t, s->meta.rowB / 4);
+        CAO_LAUNCHED("k_inner_lut");
     }
-    ea.B = s->B; ea.magicB = s->B > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + s->B - 1) / s->B) : 0;
-    ea.n_blocks = s->n_blocks; ea.n_words = s->n_words; ea.dom = d_dom; ea.desc = d_desc; ea.tables = d_tables;
+    CAO_CUDA(cudaStreamWaitEvent(st, s->ev_join, 0));                   // join
+    uint32_t* ctl = (uint32_t*)(sc + s->off_V);                         // [0..1] V, [2] scan ticket, [3] live count, [4] group count
+    EnumArgs ea{};
+    ea.B = s->B; ea.n_blocks = s->n_blocks; ea.dom = d_dom; ea.desc = d_desc; ea.tables = d_tables; ea.flags = d_flags;
     ea.bitmap = (uint64_t*)d_bitmap; ea.cnt = (uint32_t*)(sc + s->off_cnt);
-    ea.Wb = s->Wb; ea.nb = s->nb; ea.t = s->t; ea.n_tab = s->n_tab; ea.n_res = s->n_res;
-    size_t smem = (size_t)(s->nb + 1) * s->Wb * 8 + (size_t)CAO_MAX_DIMS * 256;
-    if (smem > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_enum_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    uint64_t grid = (s->n_blocks + s->nb - 1) / s->nb;
-    { ProfScope ps(PK_ENUM, st); k_enum_pass1<<<(unsigned)grid, 256, smem, st>>>(s->meta, ea); }
-    CAO_LAUNCHED("k_enum_pass1");
-    uint32_t* d_cnt = (uint32_t*)(sc + s->off_cnt);
-    uint32_t* d_part = (uint32_t*)(sc + s->off_part);
-    uint64_t* d_V = (uint64_t*)(sc + s->off_V);
+    ea.live = (uint32_t*)(sc + s->off_live); ea.live_count = ctl + 3;
+    ea.Wb = s->Wb; ea.CH = s->CH; ea.t = s->t; ea.n_tab = s->n_tab; ea.n_res = s->n_res;
+    {
+        const unsigned bd = 256;
+        const size_t smem = (size_t)bd * (4 * (size_t)s->n_tab + (size_t)std::max(1, s->t));
+        const uint64_t threads = (s->n_blocks + s->CH - 1) / s->CH;
+        if (smem > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_enum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ProfScope ps(PK_ENUM, st);
+        k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem, st>>>(s->meta, ea);
+        CAO_LAUNCHED("k_enum");
+    }
+    if (s->n_res) {
+        ProfScope ps(PK_ENUM, st);
+        const uint64_t warps = std::min<uint64_t>(s->n_blocks, 148ull * 64);
+        k_residual<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(s->meta, ea);
+        CAO_LAUNCHED("k_residual");
+    }
     {
         ProfScope ps(PK_CSCAN, st);
-        k_scan_reduce<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
-        CAO_LAUNCHED("k_scan_reduce");
-        k_scan_partials<<<1, 1024, 0, st>>>(d_part, s->n_part, d_V);
-        CAO_LAUNCHED("k_scan_partials");
-        k_scan_apply<<<(unsigned)s->n_part, 256, 0, st>>>(d_cnt, s->nd + 1, d_part);
-        CAO_LAUNCHED("k_scan_apply");
+        k_cnt_reduce<<<(unsigned)s->n_part, 256, 0, st>>>(ea.cnt, s->nd + 1, (uint32_t*)(sc + s->off_part), s->n_part, ctl + 2, (uint64_t*)ctl);
+        CAO_LAUNCHED("k_cnt_reduce");
     }
     return CAO_OK;
 }
 
-// S1 pass 2 on `st`: rows, Ltab, rank directory.
+// S1 pass 2 on `st`: rank directory + list of non-empty groups, then rows and Ltab.
 static int launch_fill(cao_space* s, uint8_t* tb, cudaStream_t st) {
-    uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
-    const uint32_t* cnt = (const uint32_t*)((uint8_t*)s->d_scratch + s->off_cnt);
-    // groups (512 configs) per warp pass.  One pair per warp measured fastest on dense AND sparse spaces (valid
-    // configs cluster, so a warp that skims 32 directory entries serialises the few non-empty pairs it meets).
-    const uint32_t gpw = 2u;
-    unsigned grid = (unsigned)((s->nd + 8ull * gpw - 1) / (8ull * gpw));
-    if (grid == 0) grid = 1;
+    uint8_t* sc = (uint8_t*)s->d_scratch;
+    uint8_t* rows = tb + s->off_rows; void* Ltab = tb + s->off_Ltab; uint32_t* dir = (uint32_t*)(tb + s->off_dir);
+    const uint32_t* cnt = (const uint32_t*)(sc + s->off_cnt);
+    uint32_t* ctl = (uint32_t*)(sc + s->off_V);
+    uint32_t* groups = (uint32_t*)(sc + s->off_groups);
+    CAO_CUDA(cudaMemsetAsync(ctl + 4, 0, 4, st));
+    {
+        ProfScope ps(PK_CSCAN, st);
+        k_cnt_apply<<<(unsigned)s->n_part, 256, 0, st>>>(cnt, s->nd + 1, (const uint32_t*)(sc + s->off_part), dir, groups, ctl + 4);
+        CAO_LAUNCHED("k_cnt_apply");
+    }
+    const uint32_t* lut = s->use_lut ? (const uint32_t*)(sc + s->off_lut) : nullptr;
+    const uint64_t magicB = s->B > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + s->B - 1) / s->B) : 0;
+    const unsigned grid = (unsigned)std::min<uint64_t>((s->nd + 7) / 8, 148ull * 8);   // a warp per group, grid-stride over the list
     {
         ProfScope ps(PK_FILL, st);
-        if (s->meta.rowB == 16) k_fill<4><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd, gpw);
-        else k_fill<8><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, cnt, s->nd, gpw);
+#define CALL_FILL(W, L32) k_fill<W, L32><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, groups, ctl + 4, lut, s->B, magicB, s->t)
+        if (s->meta.rowB == 16) { if (s->meta.ltab32) CALL_FILL(4, true); else CALL_FILL(4, false); }
+        else { if (s->meta.ltab32) CALL_FILL(8, true); else CALL_FILL(8, false); }
     }
     CAO_LAUNCHED("k_fill");
     return CAO_OK;
@@ -376,7 +370,7 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
     const uint64_t rowB = s->meta.rowB;
     uint64_t off = 0;
     s->off_rows = off; off = align256(off + std::max<uint64_t>(1, V) * rowB);
-    s->off_Ltab = off; off = align256(off + std::max<uint64_t>(1, V) * 8);
+    s->off_Ltab = off; off = align256(off + std::max<uint64_t>(1, V) * (s->meta.ltab32 ? 4 : 8));
     s->off_dir = off; off = align256(off + (s->nd + 1) * 4);
     // neighbour lists and the cost model that decides how many Hamming levels are probed before the scan:
     // e_h = number of index rows at Hamming distance exactly h from a point (elementary symmetric polynomial of m_d - 1)
@@ -423,7 +417,8 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
     if (!d_table || ((uintptr_t)d_table & 255)) return cao_fail(CAO_E_WORKSPACE, "cao_space_build_fill: table must be non-NULL and 256-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
     uint8_t* tb = (uint8_t*)d_table;
-    uint8_t* rows = tb + s->off_rows; uint64_t* Ltab = (uint64_t*)(tb + s->off_Ltab); uint32_t* dir = (uint32_t*)(tb + s->off_dir);
+    uint8_t* rows = tb + s->off_rows; void* Ltab = tb + s->off_Ltab; uint32_t* dir = (uint32_t*)(tb + s->off_dir);
+    s->d_table = d_table;
     { int rc = launch_fill(s, tb, st); if (rc) return rc; }
     if (!s->h_nb.empty())
         CAO_CUDA(cudaMemcpyAsync(tb + s->off_tgt, s->h_nb.data(), s->h_nb.size() * 2, cudaMemcpyHostToDevice, st));
@@ -446,6 +441,13 @@ int cao_space_rebuild(cao_space* s, void* stream) {
     return launch_fill(s, (uint8_t*)s->d_table, st);
 }
 
+int cao_space_ltab_bytes(const cao_space* s, int32_t* bytes) {
+    if (!s || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_ltab_bytes: NULL argument");
+    if (!s->planned) return cao_fail(CAO_E_STATE, "cao_space_ltab_bytes: space not planned yet");
+    *bytes = s->meta.ltab32 ? 4 : 8;
+    return CAO_OK;
+}
+
 int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes) {
     if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_sizes: NULL space");
     if (!s->planned) return cao_fail(CAO_E_STATE, "cao_space_sizes: space not planned yet");
@@ -456,7 +458,7 @@ int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, in
     return CAO_OK;
 }
 
-int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t** d_rows, const uint64_t** d_Ltab,
+int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t** d_rows, const void** d_Ltab,
                     const uint32_t** d_rank_dir) {
     if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_views: NULL space");
     if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_views: space not built");

@@ -17,7 +17,8 @@ def _gpu_space(sp, mode=0):
 
 
 def _u64(t):
-    return t.cpu().numpy().view(np.uint64)
+    a = t.cpu().numpy()
+    return a.view(np.uint32).astype(np.uint64) if a.dtype.itemsize == 4 else a.view(np.uint64)
 
 
 def _check_space(sp, os_, gs):
