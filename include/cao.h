@@ -104,6 +104,10 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream);
  * the ones build_count returned.  Needs a completed build_count + build_fill; d_scratch must still be alive. */
 int cao_space_rebuild(cao_space* s, void* stream);
 int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes);
+/* Statistics of the last build / rebuild (synchronises `stream`; d_scratch must still be alive): h_out4 = {blocks of
+ * B consecutive configs the index range is cut into, blocks that survived the tabled constraints and went on to the
+ * residual ones (0 when there is no residual constraint), non-empty 512-config groups, B}. */
+int cao_space_build_stats(const cao_space* s, void* stream, uint64_t* h_out4);
 /* Bytes per Ltab entry: 4 when N <= 2^32 (every linear index fits 32 bits), else 8. */
 int cao_space_ltab_bytes(const cao_space* s, int32_t* bytes);
 /* Borrowed device views into the caller's buffers; rank_dir[i] = number of valid L < 512*i. */
@@ -175,8 +179,9 @@ uint64_t cao_launch_count(void);
 
 /* Optional device timing per kernel class (bench.py's roofline): while enabled, every launch is bracketed by
  * CUDA events on its stream.  enable(1) clears the totals.  read() synchronises the recorded events and
- * returns the summed milliseconds and the launch count of class `cls`: 0 k_build_table, 1 k_enum_pass1,
- * 2 count scan, 3 k_fill, 4 k_init, 5 k_op, 6 k_scan, 7 k_finish, 8 queries; name() gives the kernel names. */
+ * returns the summed milliseconds and the launch count of class `cls`: 0 k_build_tables + k_inner_lut, 1 k_enum,
+ * 2 count scan, 3 k_fill, 4 k_init, 5 k_op, 6 k_scan, 7 k_finish, 8 queries, 9 k_probe23, 10 k_gen, 11 k_residual;
+ * name() gives the kernel names. */
 int cao_profile_enable(int32_t on);
 int cao_profile_read(int32_t cls, double* h_ms_total, uint64_t* h_launches);
 const char* cao_profile_name(int32_t cls);

@@ -54,6 +54,7 @@ SIGNATURES = {
     "cao_space_rebuild": (C.c_int, [vp, vp]),
     "cao_space_sizes": (C.c_int, [vp, pu64, pu64, pi32, pi32]),
     "cao_space_ltab_bytes": (C.c_int, [vp, pi32]),
+    "cao_space_build_stats": (C.c_int, [vp, vp, pu64]),
     "cao_space_views": (C.c_int, [vp, pvp, pvp, pvp, pvp]),
     "cao_space_is_valid": (C.c_int, [vp, vp, u64, vp, vp]),
     "cao_space_repair_scratch_bytes": (C.c_int, [vp, u64, pu64]),
@@ -126,7 +127,7 @@ def profile_enable(on=True):
 def profile_read():
     """{kernel class name: (total ms, launches)} since profile_enable(True)."""
     out = {}
-    for cls in range(11):
+    for cls in range(12):
         ms, n = C.c_double(), u64()
         _check(lib().cao_profile_read(cls, C.byref(ms), C.byref(n)))
         out[lib().cao_profile_name(cls).decode()] = (ms.value, n.value)
@@ -228,6 +229,11 @@ class Space:
         """(V, row_bytes) uint8, ascending L, padding zero."""
         N, V, n, rb = self.sizes()
         return _view(self._table, self._views()[1], V * rb, torch.uint8, (V, rb))
+
+    def build_stats(self):
+        a = (C.c_uint64 * 4)()
+        _check(lib().cao_space_build_stats(self._h, _stream(), a))
+        return dict(n_blocks=int(a[0]), live_blocks=int(a[1]), nonempty_groups=int(a[2]), B=int(a[3]))
 
     @property
     def ltab_bytes(self) -> int:

@@ -115,127 +115,305 @@ __global__ void __launch_bounds__(256) k_inner_lut(const __grid_constant__ Space
 }
 
 // ---------------------------------------------------------------------------------------------
-// Pass 1a.  Every thread walks CH consecutive blocks with an odometer over the outer digits (one mixed-radix decode per
-// thread, then increments).  Per block: row flags of the tabled constraints in turn (exit at the first zero), then the
-// AND of the rows word by word; non-zero words go to the zero-filled bitmap with atomicOr (a block's first and last
-// word are shared with its neighbours when B is not a multiple of 64).  Without residual constraints the popcounts of
-// the words are added to the per-512 counts here; with them the surviving blocks are listed for pass 1b instead.
-__global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
-    extern __shared__ uint32_t s_key[];                                 // [n_tab][blockDim] row index per tabled constraint
-    const uint32_t tid = threadIdx.x, bd = blockDim.x;
-    uint8_t* dig = (uint8_t*)(s_key + (size_t)a.n_tab * bd) + tid;      // [t][blockDim] outer digits of this thread's block
-    const uint64_t o0 = ((uint64_t)blockIdx.x * bd + tid) * a.CH;
-    if (o0 >= a.n_blocks) return;
-    {
-        uint64_t q = o0;
-        for (int d = a.t - 1; d >= 0; --d) {
-            const uint32_t m = sm.m[d]; uint32_t idx = 0;
-            if (m > 1) { const uint64_t q2 = div_magic(q, sm.magic[d]); idx = (uint32_t)(q - q2 * m); q = q2; }
-            dig[d * bd] = (uint8_t)idx;
-        }
+// The descriptor words (a few hundred to a few thousand) are staged in shared memory by every CTA of pass 1: the
+// kernels chase pointers through them for every block, and a chain of dependent global loads is what bounds them.
+__device__ __forceinline__ const int32_t* stage_desc(const EnumArgs& a, int32_t* s_desc) {
+    if (!a.desc_in_smem) return a.desc;
+    for (uint32_t e = threadIdx.x; e < a.desc_words; e += blockDim.x) s_desc[e] = __ldg(&a.desc[e]);
+    __syncthreads();
+    return s_desc;
+}
+// Outer digits of block o.
+__device__ __forceinline__ void decode_outer(const SpaceMeta& sm, int t, uint64_t o, uint8_t* dig, uint32_t stride) {
+    uint64_t q = o;
+    for (int d = t - 1; d >= 0; --d) {
+        const uint32_t m = sm.m[d]; uint32_t idx = 0;
+        if (m > 1) { const uint64_t q2 = div_magic(q, sm.magic[d]); idx = (uint32_t)(q - q2 * m); q = q2; }
+        dig[d * stride] = (uint8_t)idx;
     }
-    const uint32_t tail_bits = (uint32_t)(a.B - (uint64_t)(a.Wb - 1) * 64);      // 1..64 bits in the last word
-    const uint64_t tail_mask = tail_bits == 64 ? ~0ull : ((1ull << tail_bits) - 1ull);
+}
+__device__ __forceinline__ uint32_t table_key(const int32_t* ds, const uint8_t* dig, uint32_t stride) {
+    const int no = ds[TD_NO];
+    uint32_t k = 0;
+    for (int e = 0; e < no; ++e) k += (uint32_t)dig[ds[TD_OUT + 2 * e] * stride] * (uint32_t)ds[TD_OUT + 1 + 2 * e];
+    return k;
+}
+
+// Pass 1a: which blocks survive the tabled constraints?  Every thread walks CH consecutive blocks with an odometer over
+// the outer digits (one mixed-radix decode per thread, then increments).  Per block: the row flags of the tabled
+// constraints, four independent byte loads at a time, exit at the first zero.  Survivors go to the live list
+// (warp-aggregated append; the order is irrelevant).  Nothing else is touched: a dead outer prefix costs a few bytes.
+__global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
+    extern __shared__ int32_t s_enum[];
+    const uint32_t tid = threadIdx.x, bd = blockDim.x;
+    const int32_t* desc = stage_desc(a, s_enum);
+    uint8_t* dig = (uint8_t*)(s_enum + (a.desc_in_smem ? a.desc_words : 0)) + tid;      // [t][blockDim]
+    const uint64_t o0 = ((uint64_t)blockIdx.x * bd + tid) * a.CH;
+    const bool mine = o0 < a.n_blocks;
+    if (mine) decode_outer(sm, a.t, o0, dig, bd);
     for (uint32_t it = 0; it < a.CH; ++it) {
         const uint64_t o = o0 + it;
-        if (o >= a.n_blocks) break;
-        bool alive = true;
-        for (int c = 0; c < a.n_tab && alive; ++c) {
-            const int32_t* ds = a.desc + __ldg(&a.desc[c]);
-            const int no = __ldg(&ds[TD_NO]);
-            uint32_t k = 0;
-            for (int e = 0; e < no; ++e) k += (uint32_t)dig[__ldg(&ds[TD_OUT + 2 * e]) * bd] * (uint32_t)__ldg(&ds[TD_OUT + 1 + 2 * e]);
-            s_key[c * bd + tid] = k;
-            alive = __ldg(&a.flags[(uint32_t)__ldg(&ds[TD_FOFF]) + k]) != 0;
-        }
-        if (alive) {
-            const uint64_t g0 = o * a.B;                                // first global bit of the block
-            const uint32_t sh = (uint32_t)(g0 & 63);
-            uint64_t any = 0;
-            for (uint32_t j = 0; j < a.Wb; ++j) {
-                uint64_t w = j + 1 == a.Wb ? tail_mask : ~0ull;
-                for (int c = 0; c < a.n_tab && w; ++c) {
-                    const int32_t* ds = a.desc + __ldg(&a.desc[c]);
-                    const uint64_t toff = (uint32_t)__ldg(&ds[TD_TOFF]) | ((uint64_t)(uint32_t)__ldg(&ds[TD_TOFF + 1]) << 32);
-                    w &= __ldg(&a.tables[toff + (uint64_t)s_key[c * bd + tid] * a.Wb + j]);
+        bool alive = mine && o < a.n_blocks;
+        for (int c0 = 0; c0 < a.n_tab && alive; c0 += 4) {
+            uint8_t f[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                f[u] = 1;
+                if (c0 + u < a.n_tab) {
+                    const int32_t* ds = desc + desc[c0 + u];
+                    f[u] = __ldg(&a.flags[(uint32_t)ds[TD_FOFF] + table_key(ds, dig, bd)]);
                 }
-                if (!w) continue;
-                any |= w;
-                const uint64_t gw = (g0 >> 6) + j;
-                const uint64_t lo = w << sh, hi = sh ? w >> (64 - sh) : 0;
-                if (lo) { atomicOr((unsigned long long*)&a.bitmap[gw], (unsigned long long)lo); if (!a.n_res) atomicAdd(&a.cnt[gw >> 3], (uint32_t)__popcll(lo)); }
-                if (hi) { atomicOr((unsigned long long*)&a.bitmap[gw + 1], (unsigned long long)hi); if (!a.n_res) atomicAdd(&a.cnt[(gw + 1) >> 3], (uint32_t)__popcll(hi)); }
             }
-            if (any && a.n_res) a.live[atomicAdd(a.live_count, 1u)] = (uint32_t)o;    // n_blocks < 2^32 (N < 2^40, B >= 256 unless one block)
+            alive = f[0] && f[1] && f[2] && f[3];
         }
-        for (int d = a.t - 1; d >= 0; --d) {                            // odometer: next block
-            const uint32_t v = dig[d * bd] + 1u;
-            if (v < sm.m[d]) { dig[d * bd] = (uint8_t)v; break; }
-            dig[d * bd] = 0;
+        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, alive);
+        if (bal) {
+            uint32_t base = 0;
+            if ((tid & 31) == 0) base = atomicAdd(a.live_count, (uint32_t)__popc(bal));
+            base = __shfl_sync(0xFFFFFFFFu, base, 0);
+            if (alive) a.live[base + __popc(bal & ((1u << (tid & 31)) - 1u))] = (uint32_t)o;   // n_blocks < 2^32
+        }
+        if (mine) {
+            for (int d = a.t - 1; d >= 0; --d) {                        // odometer: next block
+                const uint32_t v = dig[d * bd] + 1u;
+                if (v < sm.m[d]) { dig[d * bd] = (uint8_t)v; break; }
+                dig[d * bd] = 0;
+            }
         }
     }
 }
 
-// Pass 1b: residual constraints (too wide for a table, or plain mode), one warp per surviving block.  The program
-// prefix that reads only outer digits runs once per block; the lanes share the surviving bits of each bitmap word of
-// the block (k-th-set-bit selection), clear the ones whose suffix fails (atomicAnd on this block's bits only) and add
-// the popcount of the survivors to the per-512 counts.
-__global__ void __launch_bounds__(256) k_residual(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
+// Pass 1b: one thread per (live block, word of its mask): AND of one row word per tabled constraint (independent
+// loads), non-zero words go to the zero-filled bitmap with atomicOr (a block's first and last word are shared with its
+// neighbours when B is not a multiple of 64).  Without residual constraints the popcounts are added to the per-512
+// counts here.
+__global__ void __launch_bounds__(256) k_masks(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
+    extern __shared__ int32_t s_enum[];
+    const uint32_t tid = threadIdx.x, bd = blockDim.x;
+    const int32_t* desc = stage_desc(a, s_enum);
+    uint8_t* dig = (uint8_t*)(s_enum + (a.desc_in_smem ? a.desc_words : 0)) + tid;
+    const uint32_t nlive = *a.live_count;
+    const uint64_t total = (uint64_t)nlive * a.Wb;
+    const uint32_t tail_bits = (uint32_t)(a.B - (uint64_t)(a.Wb - 1) * 64);      // 1..64 bits in the last word
+    for (uint64_t e = (uint64_t)blockIdx.x * bd + tid; e < total; e += (uint64_t)gridDim.x * bd) {
+        const uint32_t li = (uint32_t)(e / a.Wb), j = (uint32_t)(e - (uint64_t)li * a.Wb);
+        const uint64_t o = a.live[li];
+        decode_outer(sm, a.t, o, dig, bd);
+        uint64_t w = (j + 1 == a.Wb && tail_bits < 64) ? ((1ull << tail_bits) - 1ull) : ~0ull;
+        for (int c0 = 0; c0 < a.n_tab && w; c0 += 4) {
+            uint64_t r[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                r[u] = ~0ull;
+                if (c0 + u < a.n_tab) {
+                    const int32_t* ds = desc + desc[c0 + u];
+                    const uint64_t toff = (uint32_t)ds[TD_TOFF] | ((uint64_t)(uint32_t)ds[TD_TOFF + 1] << 32);
+                    r[u] = __ldg(&a.tables[toff + (uint64_t)table_key(ds, dig, bd) * a.Wb + j]);
+                }
+            }
+            w &= r[0] & r[1] & r[2] & r[3];
+        }
+        if (!w) continue;
+        const uint64_t g0 = o * a.B;                                    // first global bit of the block
+        const uint32_t sh = (uint32_t)(g0 & 63);
+        const uint64_t gw = (g0 >> 6) + j;
+        const uint64_t lo = w << sh, hi = sh ? w >> (64 - sh) : 0;
+        if (lo) { atomicOr((unsigned long long*)&a.bitmap[gw], (unsigned long long)lo); if (!a.n_res) atomicAdd(&a.cnt[gw >> 3], (uint32_t)__popcll(lo)); }
+        if (hi) { atomicOr((unsigned long long*)&a.bitmap[gw + 1], (unsigned long long)hi); if (!a.n_res) atomicAdd(&a.cnt[(gw + 1) >> 3], (uint32_t)__popcll(hi)); }
+    }
+}
+
+// Pass 1c (only with residual constraints: too wide for a table, or plain mode), over the LIVE blocks only.
+// k_res_prefix: one thread per (live block, residual constraint) runs the program prefix that reads only outer digits
+// and stores where it stopped: status 0 = the constraint is false for the whole block, 1 = true for the whole block,
+// 2 = resume at (pc, sp) with the stored stack (up to CAO_RES_STACK values), 3 = stack too deep to store (k_residual
+// re-runs the prefix).
+// Value classes: if the prefix leaves exactly ONE stack value and the rest of the program reads inner parameters only
+// (decided on the host: a.rc_of[r] >= 0), the constraint depends on the outer digits through that value alone.  The
+// value is entered into a 4096-slot open-addressing table (atomicCAS, one attempt per distinct value per warp); the
+// slot is the block's class.  k_res_class_table then resumes the program once per (class, inner pattern) and k_residual
+// ANDs the class mask into the block -- instead of interpreting the suffix for every surviving config of every block.
+// Exact: same program, same operands, same order.  More than 4096 values: overflow flag, per-config path.
+#define CAO_RES_STACK 3
+#define CAO_HS 4096
+#define CAO_CLS_EMPTY ((long long)0x8080808080808080ll)   // below -2^62: never a saturated value
+#define CAO_CLS_NONE 0xFFFFFFFFu
+struct ResPrefix { int32_t status, pc, sp; uint32_t cls; long long st[CAO_RES_STACK]; };
+__global__ void __launch_bounds__(256) k_res_prefix(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a, ResPrefix* out) {
+    extern __shared__ int32_t s_enum[];
+    const int32_t* desc = stage_desc(a, s_enum);
+    const uint32_t nlive = *a.live_count, lane = threadIdx.x & 31;
+    const uint64_t total = (uint64_t)nlive * a.n_res;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t e0 = (uint64_t)blockIdx.x * blockDim.x; e0 < total; e0 += stride) {      // whole warps iterate together
+        const uint64_t e = e0 + threadIdx.x;
+        const bool valid = e < total;
+        const uint32_t li = valid ? (uint32_t)(e / a.n_res) : 0, r = valid ? (uint32_t)(e - (uint64_t)li * a.n_res) : 0;
+        ResPrefix p;
+        p.status = 1; p.pc = 0; p.sp = 0; p.cls = CAO_CLS_NONE;
+        for (int z = 0; z < CAO_RES_STACK; ++z) p.st[z] = 0;
+        if (valid) {
+            uint8_t dig[CAO_MAX_DIMS];
+            decode_outer(sm, a.t, a.live[li], dig, 1);
+            int64_t x[CAO_MAX_DIMS];
+            for (int d = 0; d < a.t; ++d) x[d] = a.dom[d * 256 + dig[d]];
+            const int32_t* ds = desc + desc[a.n_tab + r];
+            int64_t st0[CAO_MAX_STACK];
+            int pc0 = 0, sp0 = 0;
+            const int pre = eval_core(ds + 1, ds[0], x, 0, st0, 0, a.t, &pc0, &sp0);
+            p.status = pre == 2 && sp0 > CAO_RES_STACK ? 3 : pre; p.pc = pc0; p.sp = sp0;
+            for (int z = 0; z < CAO_RES_STACK; ++z) p.st[z] = z < sp0 ? st0[z] : 0;
+        }
+        const int rc = valid ? a.rc_of[r] : -1;
+        const bool wants = rc >= 0 && p.status == 2 && !*a.rc[rc >= 0 ? rc : 0].overflow;
+        const long long key = wants ? p.st[0] : (long long)lane;        // lanes without a class never match a real key by accident:
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, (unsigned long long)key) &   // ... they also differ in `wants`
+                               __match_any_sync(0xFFFFFFFFu, wants ? rc : -1 - (int)lane);
+        uint32_t cls = CAO_CLS_NONE;
+        if (wants && lane == (uint32_t)(__ffs(peers) - 1)) {            // one insertion per distinct (constraint, value) per warp
+            long long* keys = a.rc[rc].keys;
+            uint32_t h = (uint32_t)(((uint64_t)key * 0x9E3779B97F4A7C15ull) >> 40) & (CAO_HS - 1);
+            for (int probe = 0; probe < 64; ++probe) {
+                const long long old = atomicCAS((unsigned long long*)&keys[h], (unsigned long long)CAO_CLS_EMPTY, (unsigned long long)key);
+                if (old == CAO_CLS_EMPTY || old == key) { cls = h; break; }
+                h = (h + 1) & (CAO_HS - 1);
+            }
+            if (cls == CAO_CLS_NONE) *a.rc[rc].overflow = 1;
+        }
+        cls = __shfl_sync(0xFFFFFFFFu, cls, __ffs(peers) - 1);
+        if (wants) p.cls = cls;
+        if (valid) out[e] = p;
+    }
+}
+// k_res_class_table: one thread per (class constraint, hash slot, inner pattern) resumes the program from the class key.
+__global__ void __launch_bounds__(256) k_res_class_table(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t per_row = a.Wb * 64;
+    const uint64_t per_rc = (uint64_t)CAO_HS * per_row;
+    const int rc = blockIdx.y;
+    if (gid >= per_rc) return;                                          // whole warps: the bound is a multiple of 64
+    const uint32_t slot = (uint32_t)(gid / per_row), p = (uint32_t)(gid - (uint64_t)slot * per_row);
+    const long long key = a.rc[rc].keys[slot];
+    int ok = 0;
+    if (key != CAO_CLS_EMPTY && p < a.B) {
+        const int32_t* ds = a.desc + a.desc[a.n_tab + a.rc[rc].r];
+        int64_t x[CAO_MAX_DIMS];
+        for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
+        uint32_t q = p;
+        for (int d = sm.n - 1; d >= a.t; --d) { const uint32_t m = sm.m[d]; x[d] = a.dom[d * 256 + q % m]; q /= m; }
+        int64_t st[CAO_MAX_STACK];
+        st[0] = key;
+        int u0, u1;
+        ok = eval_core(ds + 1, ds[0], x, a.rc[rc].pc0, st, 1, -1, &u0, &u1);
+    }
+    const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
+    if ((threadIdx.x & 31) == 0) ((uint32_t*)a.rc[rc].table)[gid >> 5] = word;
+}
+
+// 64 bits of a B-bit mask (Wb words) starting at bit position rel (may be negative or run past the end: zeros).
+__device__ __forceinline__ uint64_t mask_bits(const uint64_t* __restrict__ mk, int64_t rel, uint32_t Wb) {
+    uint64_t v = 0;
+    if (rel <= -64 || rel >= (int64_t)Wb * 64) return 0;
+    if (rel < 0) return __ldg(&mk[0]) << (uint32_t)(-rel);
+    const uint32_t j = (uint32_t)(rel >> 6), s = (uint32_t)(rel & 63);
+    v = __ldg(&mk[j]) >> s;
+    if (s && j + 1 < Wb) v |= __ldg(&mk[j + 1]) << (64 - s);
+    return v;
+}
+
+// k_residual: one warp per live block, one lane per bitmap word of the block.  Class constraints: AND of the class mask.
+// Other residual constraints: the set bits left in the block (a handful on sparse spaces) are numbered across the words;
+// the lanes take them 32 at a time and resume every such program from its stored prefix.  Failing bits are cleared with
+// atomicAnd (this block's bits only); the survivors are added to the per-512 counts.
+__global__ void __launch_bounds__(256) k_residual(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a,
+                                                  const ResPrefix* __restrict__ pre) {
+    extern __shared__ int32_t s_enum[];
+    const int32_t* desc = stage_desc(a, s_enum);
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t nlive = *a.live_count;
     const uint64_t wid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((uint64_t)gridDim.x * blockDim.x) >> 5;
     for (uint64_t li = wid; li < nlive; li += nwarps) {
         const uint64_t o = a.live[li];
-        int64_t x[CAO_MAX_DIMS];
-        {
-            uint64_t q = o;
-            for (int d = a.t - 1; d >= 0; --d) {
-                const uint32_t m = sm.m[d]; uint32_t idx = 0;
-                if (m > 1) { const uint64_t q2 = div_magic(q, sm.magic[d]); idx = (uint32_t)(q - q2 * m); q = q2; }
-                x[d] = a.dom[d * 256 + idx];
-            }
-        }
         const uint64_t g0 = o * a.B, g1 = g0 + a.B;                     // global bit range of the block
         const uint64_t w0 = g0 >> 6, w1 = (g1 + 63) >> 6;
-        for (uint64_t gw = w0; gw < w1; ++gw) {
-            // this block's bits inside global word gw
-            const uint64_t lo_bit = gw << 6;
-            uint64_t own = ~0ull;
-            if (lo_bit < g0) own &= ~0ull << (g0 - lo_bit);
-            if (lo_bit + 64 > g1) own &= ~0ull >> (lo_bit + 64 - g1);
-            uint64_t word = __ldcg(&a.bitmap[gw]) & own;                // written by k_enum (L2)
-            for (int r = 0; r < a.n_res && word; ++r) {
-                const int32_t* ds = a.desc + __ldg(&a.desc[a.n_tab + r]);
-                const int nw = __ldg(&ds[0]);
-                int64_t st0[CAO_MAX_STACK];
-                int pc0 = 0, sp0 = 0;
-                const int pre = eval_core(ds + 1, nw, x, 0, st0, 0, a.t, &pc0, &sp0);       // block-uniform
-                if (pre == 1) continue;                                                    // holds for the whole block
-                uint64_t kill = 0;
-                if (pre == 0) kill = word;
-                else {
-                    const uint32_t c = __popcll(word);
-                    for (uint32_t k = lane; k < c; k += 32) {
-                        const int bit = kth_set_bit64(word, k);
-                        uint64_t p = lo_bit + bit - g0;                 // pattern inside the block
+        bool dead = false, generic = false;
+        for (int r = 0; r < a.n_res; ++r) {
+            const ResPrefix& q = pre[li * a.n_res + r];
+            dead = dead || q.status == 0;
+            generic = generic || (q.status >= 2 && q.cls == CAO_CLS_NONE);
+        }
+        int64_t x[CAO_MAX_DIMS];
+        if (generic && !dead) {
+            uint8_t dig[CAO_MAX_DIMS];
+            decode_outer(sm, a.t, o, dig, 1);
+            for (int d = 0; d < a.t; ++d) x[d] = a.dom[d * 256 + dig[d]];
+        }
+        for (uint64_t wb = w0; wb < w1; wb += 32) {                     // 32 bitmap words per pass, one per lane
+            const uint64_t gw = wb + lane;
+            uint64_t own = 0;
+            if (gw < w1) {
+                own = ~0ull;
+                const uint64_t lo_bit = gw << 6;
+                if (lo_bit < g0) own &= ~0ull << (g0 - lo_bit);
+                if (lo_bit + 64 > g1) own &= ~0ull >> (lo_bit + 64 - g1);
+            }
+            const uint64_t orig = own ? (__ldcg(&a.bitmap[gw]) & own) : 0;    // written by k_masks (L2)
+            uint64_t word = dead ? 0 : orig;
+            for (int r = 0; r < a.n_res && word; ++r) {                 // class constraints: one mask word per lane
+                const ResPrefix& q = pre[li * a.n_res + r];
+                if (q.status != 2 || q.cls == CAO_CLS_NONE) continue;
+                const uint64_t* tab = a.rc[a.rc_of[r]].table + (uint64_t)q.cls * a.Wb;
+                word &= mask_bits(tab, (int64_t)(gw << 6) - (int64_t)g0, a.Wb);
+            }
+            if (generic && !dead) {
+                const uint64_t snap = word;                             // the numbering of the set bits is fixed here
+                const uint32_t pc = __popcll(word);
+                uint32_t inc = pc;
+#pragma unroll
+                for (int s = 1; s < 32; s <<= 1) { const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, s); if (lane >= (uint32_t)s) inc += v; }
+                const uint32_t tot = __shfl_sync(0xFFFFFFFFu, inc, 31), excl = inc - pc;
+                for (uint32_t k0 = 0; k0 < tot; k0 += 32) {             // the k-th set bit of the pass goes to lane k - k0
+                    const uint32_t k = k0 + lane;
+                    uint32_t src = 0;                                   // owner word = last lane whose exclusive offset is <= k
+#pragma unroll
+                    for (int step = 16; step; step >>= 1) {
+                        const uint32_t c = src + step;
+                        const uint32_t oc = __shfl_sync(0xFFFFFFFFu, excl, c & 31);
+                        if (c < 32 && oc <= k) src = c;
+                    }
+                    const uint64_t sw = __shfl_sync(0xFFFFFFFFu, snap, src);
+                    const uint32_t se = __shfl_sync(0xFFFFFFFFu, excl, src);
+                    bool fail = false; int bit = 0;
+                    if (k < tot) {
+                        bit = kth_set_bit64(sw, k - se);
+                        uint64_t p = ((wb + src) << 6) + bit - g0;      // pattern inside the block
                         for (int d = sm.n - 1; d >= a.t; --d) {
                             const uint32_t m = sm.m[d]; uint32_t idx = 0;
                             if (m > 1) { const uint64_t p2 = div_magic(p, sm.magic[d]); idx = (uint32_t)(p - p2 * m); p = p2; }
                             x[d] = a.dom[d * 256 + idx];
                         }
-                        int64_t st[CAO_MAX_STACK];
-                        for (int z = 0; z < sp0; ++z) st[z] = st0[z];
-                        int u0, u1;
-                        if (!eval_core(ds + 1, nw, x, pc0, st, sp0, -1, &u0, &u1)) kill |= 1ull << bit;
+                        for (int r = 0; r < a.n_res && !fail; ++r) {
+                            const ResPrefix& q = pre[li * a.n_res + r];
+                            if (q.status < 2 || q.cls != CAO_CLS_NONE) continue;
+                            const int32_t* ds = desc + desc[a.n_tab + r];
+                            int64_t st[CAO_MAX_STACK];
+                            int u0, u1, pc0 = 0, sp0 = 0;
+                            if (q.status == 2) { pc0 = q.pc; sp0 = q.sp; for (int z = 0; z < CAO_RES_STACK; ++z) st[z] = q.st[z]; }
+                            fail = !eval_core(ds + 1, ds[0], x, pc0, st, sp0, -1, &u0, &u1);
+                        }
                     }
-                    const uint32_t klo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)kill);
-                    const uint32_t khi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(kill >> 32));
-                    kill = ((uint64_t)khi << 32) | klo;
+                    // every lane hands its verdict to the lane that owns the word
+                    for (uint32_t l2 = 0; l2 < 32; ++l2) {
+                        const uint32_t s2 = __shfl_sync(0xFFFFFFFFu, src, l2);
+                        const int b2 = __shfl_sync(0xFFFFFFFFu, bit, l2);
+                        const bool f2 = __shfl_sync(0xFFFFFFFFu, (int)(fail && k < tot), l2) != 0;
+                        if (f2 && s2 == lane) word &= ~(1ull << b2);
+                    }
                 }
-                word &= ~kill;
-                if (kill && lane == 0) atomicAnd((unsigned long long*)&a.bitmap[gw], (unsigned long long)~kill);
             }
-            if (word && lane == 0) atomicAdd(&a.cnt[gw >> 3], (uint32_t)__popcll(word));
+            const uint64_t kill = orig & ~word;
+            if (kill) atomicAnd((unsigned long long*)&a.bitmap[gw], (unsigned long long)~kill);
+            if (word) atomicAdd(&a.cnt[gw >> 3], (uint32_t)__popcll(word));
         }
     }
 }

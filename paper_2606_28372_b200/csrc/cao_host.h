@@ -16,7 +16,7 @@ int cao_cuda_check(cudaError_t e, const char* what);
 #define CAO_LAUNCHED(what) do { ++g_cao_launches; int rc_ = cao_cuda_check(cudaGetLastError(), what); if (rc_) return rc_; } while (0)
 
 // Optional per-kernel-class device timing (cao_profile_*): CUDA events on the launching stream around each launch.
-enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_GEN, PK_N };
+enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_GEN, PK_RESID, PK_N };
 extern std::atomic<int> g_cao_prof_on;
 void cao_prof_mark(int cls, bool end, cudaStream_t st);
 struct ProfScope {
@@ -26,6 +26,15 @@ struct ProfScope {
 };
 
 static inline uint64_t align256(uint64_t x) { return (x + 255) & ~255ull; }
+
+// Value classes of a residual constraint (cao_enum_kernels.cuh, pass 1c).
+#define CAO_MAX_RC 4
+struct ResClassArgs {
+    long long* keys;                   // CAO_HS prefix values (CAO_CLS_EMPTY = free)
+    uint64_t* table;                   // CAO_HS x Wb inner masks
+    int32_t* overflow;                 // more distinct values than slots: the constraint falls back to the per-config path
+    int32_t pc0, r;                    // first token of the suffix; residual constraint number
+};
 
 // One constraint in the enumeration plan.
 struct ConsPlan {
@@ -50,11 +59,13 @@ struct cao_space {
     uint32_t Wb = 0, CH = 1;           // u64 words per block mask; blocks per thread of k_enum
     std::vector<ConsPlan> plan;
     std::vector<int32_t> desc;         // descriptor words uploaded to the device
-    int n_tab = 0, n_res = 0;
+    int n_tab = 0, n_res = 0, n_rc = 0;
+    int rc_pc0[CAO_MAX_RC] = {0, 0, 0, 0}, rc_r[CAO_MAX_RC] = {0, 0, 0, 0};
+    uint64_t off_rc[CAO_MAX_RC] = {0, 0, 0, 0}, rc_bytes = 0;
     bool use_lut = false;
     // scratch layout (byte offsets)
     uint64_t off_dom = 0, off_desc = 0, off_tables = 0, off_flags = 0, off_lut = 0, off_cnt = 0, off_part = 0, off_V = 0,
-             off_live = 0, off_groups = 0, scratch_bytes = 0;
+             off_live = 0, off_groups = 0, off_pre = 0, scratch_bytes = 0;
     uint64_t tables_words = 0, flags_bytes = 0, n_part = 0, max_table_threads = 0, max_table_ci = 1;
     uint64_t bitmap_bytes = 0;
     void* d_scratch = nullptr;
@@ -85,6 +96,10 @@ struct EnumArgs {
     uint32_t* live_count;
     uint32_t Wb, CH;
     int32_t t, n_tab, n_res;
+    uint32_t desc_words, desc_in_smem; // the descriptor words are staged in shared memory by every CTA (when they fit)
+    int32_t n_rc;                      // residual constraints with value classes
+    int8_t rc_of[32];                  // residual r -> class table (or -1); at most 32 residual constraints are looked at
+    ResClassArgs rc[CAO_MAX_RC];
 };
 
 struct cao_runs;

@@ -87,8 +87,9 @@ int cao_profile_read(int32_t cls, double* ms_total, uint64_t* launches) {
     return CAO_OK;
 }
 const char* cao_profile_name(int32_t cls) {
-    static const char* names[PK_N] = {"k_build_table", "k_enum_pass1", "k_scan_reduce+partials+apply", "k_fill", "k_init",
-                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish", "k_probe23", "k_gen"};
+    static const char* names[PK_N] = {"k_build_tables+k_inner_lut", "k_enum", "k_cnt_reduce+k_cnt_apply", "k_fill", "k_init",
+                                      "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish", "k_probe23", "k_gen",
+                                      "k_residual"};
     return cls >= 0 && cls < PK_N ? names[cls] : "";
 }
 
@@ -231,6 +232,27 @@ static int plan_space(cao_space* s) {
         D.push_back((int32_t)s->cons[res[k]].size());
         D.insert(D.end(), s->cons[res[k]].begin(), s->cons[res[k]].end());
     }
+    // Value classes: a residual program whose tokens before the first inner parameter leave exactly one stack value,
+    // and whose remaining tokens read inner parameters only, depends on the outer digits through that one value.
+    s->n_rc = 0;
+    if (s->mode == 0 && (uint64_t)CAO_HS * s->Wb * 8 <= (32ull << 20)) {
+        for (size_t k = 0; k < res.size() && k < 32 && s->n_rc < CAO_MAX_RC; ++k) {
+            const auto& w = s->cons[res[k]];
+            int sp = 0, pc0 = -1; bool ok = true;
+            for (size_t pc = 0; pc < w.size(); ++pc) {
+                const int op = w[pc];
+                if (op == CAO_OP_PUSH_PARAM) {
+                    const int d = w[pc + 1];
+                    if (pc0 < 0 && d >= t) { pc0 = (int)pc; if (sp != 1) ok = false; }
+                    else if (pc0 >= 0 && d < t) ok = false;               // the suffix reads an outer parameter
+                    ++pc; ++sp;
+                } else if (op == CAO_OP_PUSH_CONST) { pc += 2; ++sp; }
+                else if (op == CAO_OP_NEG || op == CAO_OP_NOT) {}
+                else --sp;
+            }
+            if (ok && pc0 > 0) { s->rc_pc0[s->n_rc] = pc0; s->rc_r[s->n_rc] = (int)k; ++s->n_rc; }
+        }
+    }
     s->use_lut = B * (uint64_t)M.rowB <= (1ull << 20);            // inner index bytes of every pattern (pass 2)
     // scratch layout
     uint64_t off = 0;
@@ -243,8 +265,11 @@ static int plan_space(cao_space* s) {
     s->off_part = off; off = align256(off + s->n_part * 4);
     s->off_V = off; off = align256(off + 32);                     // V (u64), scan ticket, live count, group count
     s->off_cnt = off; off = align256(off + (s->nd + 1) * 4);
-    s->off_live = off; off = align256(off + (s->n_res ? s->n_blocks : 1) * 4);
+    s->off_live = off; off = align256(off + s->n_blocks * 4);
+    s->off_pre = off; off = align256(off + (s->n_res ? s->n_blocks * (uint64_t)s->n_res * sizeof(ResPrefix) : 1));
     s->off_groups = off; off = align256(off + (s->nd + 1) * 4);
+    s->rc_bytes = align256((uint64_t)CAO_HS * 8) + align256((uint64_t)CAO_HS * s->Wb * 8) + 256;
+    for (int k = 0; k < s->n_rc; ++k) { s->off_rc[k] = off; off += s->rc_bytes; }
     s->scratch_bytes = off;
     s->bitmap_bytes = align256(s->n_words * 8);
     s->planned = true;
@@ -272,6 +297,11 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     CAO_CUDA(cudaStreamWaitEvent(s->side, s->ev_fork, 0));
     CAO_CUDA(cudaMemsetAsync(d_bitmap, 0, s->bitmap_bytes, s->side));
     CAO_CUDA(cudaMemsetAsync(sc + s->off_V, 0, (s->off_cnt - s->off_V) + (s->nd + 1) * 4, s->side));   // V, tickets, counts
+    for (int k = 0; k < s->n_rc; ++k) {                                 // class tables start empty
+        uint8_t* b = sc + s->off_rc[k];
+        CAO_CUDA(cudaMemsetAsync(b, 0x80, (uint64_t)CAO_HS * 8, s->side));
+        CAO_CUDA(cudaMemsetAsync(b + align256((uint64_t)CAO_HS * 8) + align256((uint64_t)CAO_HS * s->Wb * 8), 0, 4, s->side));
+    }
     CAO_CUDA(cudaEventRecord(s->ev_join, s->side));
     const int64_t* d_dom = (const int64_t*)(sc + s->off_dom);
     const int32_t* d_desc = (const int32_t*)(sc + s->off_desc);
@@ -298,19 +328,54 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     ea.bitmap = (uint64_t*)d_bitmap; ea.cnt = (uint32_t*)(sc + s->off_cnt);
     ea.live = (uint32_t*)(sc + s->off_live); ea.live_count = ctl + 3;
     ea.Wb = s->Wb; ea.CH = s->CH; ea.t = s->t; ea.n_tab = s->n_tab; ea.n_res = s->n_res;
+    ea.desc_words = (uint32_t)s->desc.size(); ea.desc_in_smem = s->desc.size() <= 8192;
+    ea.n_rc = s->n_rc;
+    for (int r = 0; r < 32; ++r) ea.rc_of[r] = -1;
+    for (int k = 0; k < s->n_rc; ++k) {
+        uint8_t* b = sc + s->off_rc[k];
+        ResClassArgs& rc = ea.rc[k];
+        rc.keys = (long long*)b; b += align256((uint64_t)CAO_HS * 8);
+        rc.table = (uint64_t*)b; b += align256((uint64_t)CAO_HS * s->Wb * 8);
+        rc.overflow = (int32_t*)b;
+        rc.pc0 = s->rc_pc0[k]; rc.r = s->rc_r[k];
+        ea.rc_of[s->rc_r[k]] = (int8_t)k;
+    }
+    const unsigned bd = 256;
+    const size_t smem_desc = ea.desc_in_smem ? (size_t)ea.desc_words * 4 : 0;
+    const size_t smem_dig = smem_desc + (size_t)bd * (size_t)std::max(1, s->t);
     {
-        const unsigned bd = 256;
-        const size_t smem = (size_t)bd * (4 * (size_t)s->n_tab + (size_t)std::max(1, s->t));
         const uint64_t threads = (s->n_blocks + s->CH - 1) / s->CH;
-        if (smem > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_enum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ProfScope ps(PK_ENUM, st);
-        k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem, st>>>(s->meta, ea);
+        if (smem_dig > 48 * 1024) {
+            CAO_CUDA(cudaFuncSetAttribute(k_enum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_dig));
+            CAO_CUDA(cudaFuncSetAttribute(k_masks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_dig));
+        }
+        {
+            ProfScope ps(PK_ENUM, st);
+            k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem_dig, st>>>(s->meta, ea);
+        }
         CAO_LAUNCHED("k_enum");
+        ProfScope ps(PK_PROBE, st);
+        const uint64_t items = s->n_blocks * (uint64_t)s->Wb;
+        k_masks<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 16), bd, smem_dig, st>>>(s->meta, ea);
+        CAO_LAUNCHED("k_masks");
     }
     if (s->n_res) {
-        ProfScope ps(PK_ENUM, st);
+        ResPrefix* pre = (ResPrefix*)(sc + s->off_pre);
+        const uint64_t items = s->n_blocks * (uint64_t)s->n_res;
+        {
+            ProfScope ps(PK_QUERY, st);
+            k_res_prefix<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 8), bd, smem_desc, st>>>(s->meta, ea, pre);
+        }
+        CAO_LAUNCHED("k_res_prefix");
+        if (s->n_rc) {
+            ProfScope ps(PK_QUERY, st);
+            const uint64_t threads = (uint64_t)CAO_HS * s->Wb * 64;
+            k_res_class_table<<<dim3((unsigned)((threads + 255) / 256), (unsigned)s->n_rc), 256, 0, st>>>(s->meta, ea);
+            CAO_LAUNCHED("k_res_class_table");
+        }
+        ProfScope ps(PK_RESID, st);
         const uint64_t warps = std::min<uint64_t>(s->n_blocks, 148ull * 64);
-        k_residual<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(s->meta, ea);
+        k_residual<<<(unsigned)((warps + 7) / 8), bd, smem_desc, st>>>(s->meta, ea, pre);
         CAO_LAUNCHED("k_residual");
     }
     {
@@ -439,6 +504,16 @@ int cao_space_rebuild(cao_space* s, void* stream) {
     int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st);
     if (rc) return rc;
     return launch_fill(s, (uint8_t*)s->d_table, st);
+}
+
+int cao_space_build_stats(const cao_space* s, void* stream, uint64_t* h_out4) {
+    if (!s || !h_out4) return cao_fail(CAO_E_INVALID_ARG, "cao_space_build_stats: NULL argument");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_build_stats: space not built");
+    uint32_t ctl[8] = {0};
+    CAO_CUDA(cudaMemcpyAsync(ctl, (uint8_t*)s->d_scratch + s->off_V, 32, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CAO_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    h_out4[0] = s->n_blocks; h_out4[1] = ctl[3]; h_out4[2] = ctl[4]; h_out4[3] = s->B;
+    return CAO_OK;
 }
 
 int cao_space_ltab_bytes(const cao_space* s, int32_t* bytes) {
