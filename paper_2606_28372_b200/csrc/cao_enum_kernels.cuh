@@ -148,6 +148,10 @@ __global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta 
     const uint32_t tid = threadIdx.x, bd = blockDim.x;
     const int32_t* desc = stage_desc(a, s_enum);
     uint8_t* dig = (uint8_t*)(s_enum + (a.desc_in_smem ? a.desc_words : 0)) + tid;      // [t][blockDim]
+    uint32_t* s_list = (uint32_t*)(s_enum + (a.desc_in_smem ? a.desc_words : 0)) + ((size_t)bd * max(1, a.t) + 3) / 4;   // [bd * CH]
+    __shared__ uint32_t s_n, s_base;
+    if (tid == 0) s_n = 0;
+    __syncthreads();
     const uint64_t o0 = ((uint64_t)blockIdx.x * bd + tid) * a.CH;
     const bool mine = o0 < a.n_blocks;
     if (mine) decode_outer(sm, a.t, o0, dig, bd);
@@ -167,11 +171,11 @@ __global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta 
             alive = f[0] && f[1] && f[2] && f[3];
         }
         const uint32_t bal = __ballot_sync(0xFFFFFFFFu, alive);
-        if (bal) {
+        if (bal) {                                                      // the CTA collects its survivors in shared memory
             uint32_t base = 0;
-            if ((tid & 31) == 0) base = atomicAdd(a.live_count, (uint32_t)__popc(bal));
+            if ((tid & 31) == 0) base = atomicAdd(&s_n, (uint32_t)__popc(bal));
             base = __shfl_sync(0xFFFFFFFFu, base, 0);
-            if (alive) a.live[base + __popc(bal & ((1u << (tid & 31)) - 1u))] = (uint32_t)o;   // n_blocks < 2^32
+            if (alive) s_list[base + __popc(bal & ((1u << (tid & 31)) - 1u))] = (uint32_t)o;   // n_blocks < 2^32
         }
         if (mine) {
             for (int d = a.t - 1; d >= 0; --d) {                        // odometer: next block
@@ -181,6 +185,11 @@ __global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta 
             }
         }
     }
+    __syncthreads();
+    const uint32_t n = s_n;
+    if (tid == 0 && n) s_base = atomicAdd(a.live_count, n);             // one global atomic per CTA
+    __syncthreads();
+    for (uint32_t e = tid; e < n; e += bd) a.live[s_base + e] = s_list[e];
 }
 
 // Pass 1b: one thread per (live block, word of its mask): AND of one row word per tabled constraint (independent
@@ -286,28 +295,35 @@ __global__ void __launch_bounds__(256) k_res_prefix(const __grid_constant__ Spac
     }
 }
 // k_res_class_table: one thread per (class constraint, hash slot, inner pattern) resumes the program from the class key.
+// Warps stride over (hash slot, 32 patterns) items; only the used slots (a few dozen) do any work.
 __global__ void __launch_bounds__(256) k_res_class_table(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
-    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint32_t per_row = a.Wb * 64;
-    const uint64_t per_rc = (uint64_t)CAO_HS * per_row;
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     const int rc = blockIdx.y;
-    if (gid >= per_rc) return;                                          // whole warps: the bound is a multiple of 64
-    const uint32_t slot = (uint32_t)(gid / per_row), p = (uint32_t)(gid - (uint64_t)slot * per_row);
-    const long long key = a.rc[rc].keys[slot];
-    int ok = 0;
-    if (key != CAO_CLS_EMPTY && p < a.B) {
-        const int32_t* ds = a.desc + a.desc[a.n_tab + a.rc[rc].r];
-        int64_t x[CAO_MAX_DIMS];
-        for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
-        uint32_t q = p;
-        for (int d = sm.n - 1; d >= a.t; --d) { const uint32_t m = sm.m[d]; x[d] = a.dom[d * 256 + q % m]; q /= m; }
-        int64_t st[CAO_MAX_STACK];
-        st[0] = key;
-        int u0, u1;
-        ok = eval_core(ds + 1, ds[0], x, a.rc[rc].pc0, st, 1, -1, &u0, &u1);
+    const int32_t* ds = a.desc + a.desc[a.n_tab + a.rc[rc].r];
+    const uint32_t per_row = a.Wb * 64;
+    const uint32_t chunks = per_row >> 5;                               // 32 patterns per warp item
+    for (uint32_t item = wid; item < CAO_HS * chunks; item += nwarps) {
+        const uint32_t slot = item / chunks, p0 = (item - slot * chunks) << 5;
+        const long long key = a.rc[rc].keys[slot];
+        if (key == CAO_CLS_EMPTY) continue;
+        {
+            const uint32_t p = p0 + lane;
+            int ok = 0;
+            if (p < a.B) {
+                int64_t x[CAO_MAX_DIMS];
+                for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
+                uint32_t q = p;
+                for (int d = sm.n - 1; d >= a.t; --d) { const uint32_t m = sm.m[d]; x[d] = a.dom[d * 256 + q % m]; q /= m; }
+                int64_t st[CAO_MAX_STACK];
+                st[0] = key;
+                int u0, u1;
+                ok = eval_core(ds + 1, ds[0], x, a.rc[rc].pc0, st, 1, -1, &u0, &u1);
+            }
+            const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
+            if (lane == 0) ((uint32_t*)a.rc[rc].table)[((uint64_t)slot * per_row + p0) >> 5] = word;
+        }
     }
-    const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
-    if ((threadIdx.x & 31) == 0) ((uint32_t*)a.rc[rc].table)[gid >> 5] = word;
 }
 
 // 64 bits of a B-bit mask (Wb words) starting at bit position rel (may be negative or run past the end: zeros).

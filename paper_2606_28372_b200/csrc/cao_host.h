@@ -81,6 +81,9 @@ struct cao_space {
     // the zero fill of the bitmap runs on a side stream, overlapped with the table build
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // cao_space_rebuild replays a captured CUDA graph of the whole of S1 (launch-bound on small spaces)
+    cudaGraphExec_t rebuild_exec = nullptr;
+    uint64_t rebuild_launches = 0;
 };
 
 // Arguments of the pass-1 kernels, passed by value.

@@ -100,6 +100,7 @@ int cao_space_create(cao_space** out) {
 }
 void cao_space_destroy(cao_space* s) {
     if (!s) return;
+    if (s->rebuild_exec) cudaGraphExecDestroy(s->rebuild_exec);
     if (s->ev_fork) cudaEventDestroy(s->ev_fork);
     if (s->ev_join) cudaEventDestroy(s->ev_join);
     if (s->side) cudaStreamDestroy(s->side);
@@ -342,16 +343,17 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     }
     const unsigned bd = 256;
     const size_t smem_desc = ea.desc_in_smem ? (size_t)ea.desc_words * 4 : 0;
-    const size_t smem_dig = smem_desc + (size_t)bd * (size_t)std::max(1, s->t);
+    const size_t smem_dig = smem_desc + (((size_t)bd * (size_t)std::max(1, s->t) + 3) & ~(size_t)3);
+    const size_t smem_enum = smem_dig + (size_t)bd * s->CH * 4;
     {
         const uint64_t threads = (s->n_blocks + s->CH - 1) / s->CH;
-        if (smem_dig > 48 * 1024) {
-            CAO_CUDA(cudaFuncSetAttribute(k_enum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_dig));
+        if (smem_enum > 48 * 1024) {
+            CAO_CUDA(cudaFuncSetAttribute(k_enum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_enum));
             CAO_CUDA(cudaFuncSetAttribute(k_masks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_dig));
         }
         {
             ProfScope ps(PK_ENUM, st);
-            k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem_dig, st>>>(s->meta, ea);
+            k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem_enum, st>>>(s->meta, ea);
         }
         CAO_LAUNCHED("k_enum");
         ProfScope ps(PK_PROBE, st);
@@ -369,8 +371,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         CAO_LAUNCHED("k_res_prefix");
         if (s->n_rc) {
             ProfScope ps(PK_QUERY, st);
-            const uint64_t threads = (uint64_t)CAO_HS * s->Wb * 64;
-            k_res_class_table<<<dim3((unsigned)((threads + 255) / 256), (unsigned)s->n_rc), 256, 0, st>>>(s->meta, ea);
+            k_res_class_table<<<dim3(148 * 4, (unsigned)s->n_rc), 256, 0, st>>>(s->meta, ea);
             CAO_LAUNCHED("k_res_class_table");
         }
         ProfScope ps(PK_RESID, st);
@@ -431,6 +432,7 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
     CAO_CUDA(cudaStreamSynchronize(st));
     if (V >= (1ull << 32)) return cao_fail(CAO_E_TOO_LARGE, "V >= 2^32");
     s->meta.V = (uint32_t)V; s->d_scratch = d_scratch; s->counted = true; s->filled = false;
+    if (s->rebuild_exec) { cudaGraphExecDestroy(s->rebuild_exec); s->rebuild_exec = nullptr; }     // new buffers
     *h_V = V;
     const uint64_t rowB = s->meta.rowB;
     uint64_t off = 0;
@@ -501,6 +503,30 @@ int cao_space_rebuild(cao_space* s, void* stream) {
     if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_rebuild: NULL space");
     if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_rebuild: the space must have been built once");
     cudaStream_t st = (cudaStream_t)stream;
+    // The sequence (two zero fills on the side stream, ~10 short kernels) is launch-bound on small spaces: it is captured
+    // once into a CUDA graph and replayed.  Not on the legacy default stream (capture is illegal there) and not while
+    // per-kernel profiling is on (its events must be real).
+    const bool can_graph = st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread && !g_cao_prof_on.load();
+    if (can_graph && !s->rebuild_exec) {
+        const uint64_t l0 = g_cao_launches.load();
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st);
+            if (!rc) rc = launch_fill(s, (uint8_t*)s->d_table, st);
+            cudaGraph_t graph = nullptr;
+            const cudaError_t e = cudaStreamEndCapture(st, &graph);
+            if (!rc && e == cudaSuccess && graph && cudaGraphInstantiate(&s->rebuild_exec, graph, 0) == cudaSuccess)
+                s->rebuild_launches = g_cao_launches.load() - l0;
+            else s->rebuild_exec = nullptr;
+            if (graph) cudaGraphDestroy(graph);
+            g_cao_launches.store(l0);                                   // nothing ran yet
+            cudaGetLastError();
+        }
+    }
+    if (can_graph && s->rebuild_exec) {
+        CAO_CUDA(cudaGraphLaunch(s->rebuild_exec, st));
+        g_cao_launches += s->rebuild_launches;
+        return CAO_OK;
+    }
     int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st);
     if (rc) return rc;
     return launch_fill(s, (uint8_t*)s->d_table, st);
