@@ -53,6 +53,35 @@ static __device__ __noinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_
     return c;
 }
 
+// K consecutive counter blocks (c.w, c.w + 1, ...) at once: K independent chains interleaved round by round, so a lone
+// warp is not bound by the multiply latency, and the round keys are advanced once per round for all K.
+template <int K>
+static __device__ __forceinline__ void philox4x32_10_multi(uint4 c, uint32_t k0, uint32_t k1, uint4 (&out)[K]) {
+    uint4 s[K];
+#pragma unroll
+    for (int q = 0; q < K; ++q) s[q] = make_uint4(c.x, c.y, c.z, c.w + q);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+#pragma unroll
+        for (int q = 0; q < K; ++q) {
+            const uint32_t h0 = __umulhi(0xD2511F53u, s[q].x), l0 = 0xD2511F53u * s[q].x;
+            const uint32_t h1 = __umulhi(0xCD9E8D57u, s[q].z), l1 = 0xCD9E8D57u * s[q].z;
+            s[q] = make_uint4(h1 ^ s[q].y ^ k0, l1, h0 ^ s[q].w ^ k1, l0);
+        }
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+#pragma unroll
+    for (int q = 0; q < K; ++q) out[q] = s[q];
+}
+
+struct PhiloxPair { uint4 a, b; };
+static __device__ __noinline__ PhiloxPair philox4x32_10_x2(uint4 c, uint32_t k0, uint32_t k1) {
+    uint4 o[2];
+    philox4x32_10_multi<2>(c, k0, k1, o);
+    PhiloxPair r; r.a = o[0]; r.b = o[1];
+    return r;
+}
+
 enum : uint32_t { S_INIT = 0, S_OP = 1, S_MUT = 2, S_REINIT = 3 };
 
 // Slot-addressed draws for one (seed, run, generation, individual, stream): counter =
@@ -69,6 +98,25 @@ struct Draws {
         if (b != cur) { blk = philox4x32_10(make_uint4(run, gen, ind, (stream << 24) | b), k0, k1); cur = b; }
         uint32_t s = slot & 3;
         return s == 0 ? blk.x : s == 1 ? blk.y : s == 2 ? blk.z : blk.w;
+    }
+};
+
+// The same addressing with TWO blocks per Philox call (slots 8b .. 8b+7): for the operators that walk many slots.
+struct Draws2 {
+    uint32_t k0, k1, run, gen, ind, stream, cur;
+    uint4 blk[2];
+    __device__ __forceinline__ Draws2(uint64_t seed, uint32_t run_, uint32_t gen_, uint32_t ind_, uint32_t stream_)
+        : k0((uint32_t)seed), k1((uint32_t)(seed >> 32)), run(run_), gen(gen_), ind(ind_), stream(stream_),
+          cur(0xFFFFFFFFu) {}
+    __device__ __forceinline__ uint32_t operator()(uint32_t slot) {
+        const uint32_t b = slot >> 3;
+        if (b != cur) {
+            const PhiloxPair r = philox4x32_10_x2(make_uint4(run, gen, ind, (stream << 24) | (b << 1)), k0, k1);
+            blk[0] = r.a; blk[1] = r.b; cur = b;
+        }
+        const uint4 v = (slot & 4) ? blk[1] : blk[0];
+        const uint32_t s = slot & 3;
+        return s == 0 ? v.x : s == 1 ? v.y : s == 2 ? v.z : v.w;
     }
 };
 

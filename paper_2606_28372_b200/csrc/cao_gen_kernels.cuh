@@ -164,8 +164,13 @@ __device__ __forceinline__ void fold_eval(const Grp& g, GrpShared* gs, bool has,
     const uint32_t nn = __popc(__ballot_sync(0xFFFFFFFFu, has && is_new));
     const uint64_t m = warp_min_key(has ? (((uint64_t)fbits(f) << 32) | rk) : ~0ull);
     if ((g.t & 31) == 0) {
-        if (nn) atomicAdd(&gs->n_new, nn);
-        if (m != ~0ull) atomicMin(&gs->best, (unsigned long long)m);
+        if (g.G == 32) {                                                // a single warp owns the slice: no atomics needed
+            gs->n_new += nn;
+            if (m < gs->best) gs->best = m;
+        } else {
+            if (nn) atomicAdd(&gs->n_new, nn);
+            if (m != ~0ull) atomicMin(&gs->best, (unsigned long long)m);
+        }
     }
 }
 
@@ -408,18 +413,38 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             for (int d = 0; d < RB; ++d)
                 if (d < n) { const float df = __fsub_rn(xj[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
             const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
-            const uint32_t s0 = j * (uint32_t)n;                        // noise slots j*n .. j*n+n-1, walked in order (cached blocks)
+            // the n noise draws of this j are slots j*n .. j*n+n-1: all their Philox blocks at once (independent chains),
+            // then one specialised update per alignment o = first slot & 3, so every word is a fixed register
+            const uint32_t s0 = j * (uint32_t)n, o = s0 & 3;
+            uint32_t nw[(ROWW + 1) * 4];
+            {
+                uint4 q5[ROWW + 1];
+                if (ROWW == 4) philox4x32_10_multi<ROWW + 1>(make_uint4(run, gen, i, (S_OP << 24) | (s0 >> 2)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), q5);
+                else {
+                    uint4 qa[5], qb[4];
+                    philox4x32_10_multi<5>(make_uint4(run, gen, i, (S_OP << 24) | (s0 >> 2)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), qa);
+                    philox4x32_10_multi<4>(make_uint4(run, gen, i, (S_OP << 24) | ((s0 >> 2) + 5)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), qb);
 #pragma unroll
-            for (int d = 0; d < RB; ++d) {
-                if (d < n) {
-                    const uint32_t word = dr(s0 + d);
-                    const float df = __fsub_rn(xj[d], xi[d]);
-                    float t = __fadd_rn(xi[d], __fmul_rn(beta, df));
-                    const float e = __fsub_rn(u01(word), 0.5f);
-                    t = __fadd_rn(t, __fmul_rn(rm.hp.ff_alpha, e));
-                    xi[d] = brighter ? t : xi[d];
+                    for (int z = 0; z < 5; ++z) q5[z] = qa[z];
+#pragma unroll
+                    for (int z = 0; z < 4; ++z) q5[(5 + z) % (ROWW + 1)] = qb[z];
                 }
+#pragma unroll
+                for (int z = 0; z < ROWW + 1; ++z) { nw[4 * z] = q5[z].x; nw[4 * z + 1] = q5[z].y; nw[4 * z + 2] = q5[z].z; nw[4 * z + 3] = q5[z].w; }
             }
+#define FF_UPDATE(O)                                                                         \
+            _Pragma("unroll")                                                                \
+            for (int d = 0; d < RB; ++d) {                                                   \
+                if (d < n) {                                                                 \
+                    const float df = __fsub_rn(xj[d], xi[d]);                                \
+                    float tq = __fadd_rn(xi[d], __fmul_rn(beta, df));                        \
+                    const float e = __fsub_rn(u01(nw[d + (O)]), 0.5f);                       \
+                    tq = __fadd_rn(tq, __fmul_rn(rm.hp.ff_alpha, e));                        \
+                    xi[d] = brighter ? tq : xi[d];                                           \
+                }                                                                            \
+            }
+            if (o == 0) { FF_UPDATE(0) } else if (o == 1) { FF_UPDATE(1) } else if (o == 2) { FF_UPDATE(2) } else { FF_UPDATE(3) }
+#undef FF_UPDATE
         }
         g.sync();                                                       // all start-of-generation positions are consumed
         if (has) {
@@ -454,7 +479,7 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
     if (pm.levels >= 1) {
         unsigned long long* hkey = (unsigned long long*)S.aux4;
         uint32_t* ol = S.scr;
-        const uint32_t pos = grp_push(open, &gs->flag);
+        const uint32_t pos = grp_push(open, &gs->flag, g.G == 32);
         if (open) { ol[pos] = i; S.Lc[i] = L; hkey[i] = ~0ull; }
         g.sync();                                                       // candidate rows, list and linear indices are visible
         const uint32_t nopen = gs->flag;
@@ -477,15 +502,18 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
     }
     if (has && !same) S.key[i] = key;
     {
-        const uint32_t pos = grp_push(has && key == CAO_KEY_NONE, &gs->nwl);
+        const uint32_t pos = grp_push(has && key == CAO_KEY_NONE, &gs->nwl, g.G == 32);
         if (has && key == CAO_KEY_NONE) S.wl[pos] = i;
         const uint32_t ninv = __popc(__ballot_sync(0xFFFFFFFFu, has && !valid));
         const uint32_t nmemo = __popc(__ballot_sync(0xFFFFFFFFu, has && same && !valid));
         const uint32_t nrc = __popc(__ballot_sync(0xFFFFFFFFu, rc_hit));
         if ((i & 31) == 0) {
-            if (ninv) atomicAdd(&gs->n_inv, ninv);
-            if (nmemo) atomicAdd(&gs->n_memo, nmemo);
-            if (nrc) atomicAdd(&gs->n_rc, nrc);
+            if (g.G == 32) { gs->n_inv += ninv; gs->n_memo += nmemo; gs->n_rc += nrc; }
+            else {
+                if (ninv) atomicAdd(&gs->n_inv, ninv);
+                if (nmemo) atomicAdd(&gs->n_memo, nmemo);
+                if (nrc) atomicAdd(&gs->n_rc, nrc);
+            }
         }
     }
     g.sync();
@@ -548,7 +576,10 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
     {                                                                   // statistics: Hamming distance of every repair
         const uint32_t h = has ? min((uint32_t)(key >> 45), 8u) : 31u;
         const uint32_t peers = __match_any_sync(0xFFFFFFFFu, h);
-        if (has && (i & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&gs->hist[h], (uint32_t)__popc(peers));
+        if (has && (i & 31) == (uint32_t)(__ffs(peers) - 1)) {
+            if (g.G == 32) gs->hist[h] += (uint32_t)__popc(peers);      // distinct leaders write distinct entries
+            else atomicAdd(&gs->hist[h], (uint32_t)__popc(peers));
+        }
     }
     // ---- S6 + S7
     uint32_t rk = (uint32_t)key;
@@ -574,7 +605,7 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             uint32_t* ol = S.scr; uint32_t* mm = S.aux4;
             if (i == 0) gs->flag = 0;
             g.sync();
-            const uint32_t pos = grp_push(mutate, &gs->flag);
+            const uint32_t pos = grp_push(mutate, &gs->flag, g.G == 32);
             if (mutate) {
                 ol[pos] = i; S.Lc[i] = Lr;
                 for (uint32_t w = 0; w < MW; ++w) mm[i * 4 + w] = 0;

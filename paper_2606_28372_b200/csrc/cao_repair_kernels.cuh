@@ -94,10 +94,13 @@ __device__ __forceinline__ void grp_min_key(const Grp& g, uint64_t v, unsigned l
 }
 
 // Appends the threads with `pred` to a list: returns this thread's position (one shared-memory atomic per warp).
-__device__ __forceinline__ uint32_t grp_push(bool pred, uint32_t* counter) {
+__device__ __forceinline__ uint32_t grp_push(bool pred, uint32_t* counter, bool one_warp = false) {
     const uint32_t bal = __ballot_sync(0xFFFFFFFFu, pred), lane = threadIdx.x & 31;
     uint32_t base = 0;
-    if (lane == 0 && bal) base = atomicAdd(counter, (uint32_t)__popc(bal));
+    if (lane == 0 && bal) {
+        if (one_warp) { base = *counter; *counter = base + (uint32_t)__popc(bal); }     // a single warp owns the counter
+        else base = atomicAdd(counter, (uint32_t)__popc(bal));
+    }
     base = __shfl_sync(0xFFFFFFFFu, base, 0);
     return base + __popc(bal & ((1u << lane) - 1u));
 }
