@@ -143,9 +143,13 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
                     uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens,
                     uint64_t seed, void* d_workspace, void* stream, cao_runs** out);
 void cao_runs_destroy(cao_runs* r);
-/* How cao_runs_step executes: 1 (default) = one fused persistent kernel, one CTA per run for all the requested
- * generations; 0 = phased, per generation k_op -> k_probe23 -> k_scan -> k_finish over all runs (better when
- * most candidates need the table scan).  Identical results. */
+/* How cao_runs_step executes: 1 = one fused persistent kernel (a warp group per run, population state in shared
+ * memory for all the requested generations); 0 = phased, per generation k_op -> k_probe23 -> k_scan -> k_finish over
+ * all runs (better when many candidates need the table scan).  Identical results.  The default is chosen at create:
+ * fused unless the estimated share of invalid candidates that fall through the bitmap probes to the table scan,
+ * exp(-V/N * rows within the probed Hamming levels), exceeds 1 % (configs[3]-like sparse spaces) or the population
+ * does not fit the shared memory of one SM.  cao_runs_mode reports the mode in use. */
+int cao_runs_mode(const cao_runs* r, int32_t* mode);
 int cao_runs_set_mode(cao_runs* r, int32_t mode);
 /* S3-S7, n_generations times (stops recording at max_gens).  Asynchronous. */
 int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream);

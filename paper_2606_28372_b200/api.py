@@ -64,6 +64,7 @@ SIGNATURES = {
     "cao_runs_create": (C.c_int, [vp, i32, C.POINTER(HParams), u32, u32, i32, u32, u32, u64, vp, vp, pvp]),
     "cao_runs_destroy": (None, [vp]),
     "cao_runs_set_mode": (C.c_int, [vp, i32]),
+    "cao_runs_mode": (C.c_int, [vp, pi32]),
     "cao_runs_step": (C.c_int, [vp, u32, vp]),
     "cao_runs_best": (C.c_int, [vp, vp, vp, vp, vp, vp]),
     "cao_runs_trajectory": (C.c_int, [vp, pvp, C.POINTER(u32)]),
@@ -329,6 +330,12 @@ class Runs:
         """'fused' / 1 = one persistent kernel per step call; 'phased' / 0 = per-generation kernels."""
         m = {"fused": 1, "phased": 0}.get(mode, mode)
         _check(lib().cao_runs_set_mode(self._h, int(m)))
+
+    @property
+    def mode(self) -> str:
+        v = i32()
+        _check(lib().cao_runs_mode(self._h, C.byref(v)))
+        return "fused" if v.value == 1 else "phased"
 
     def step(self, k=1):
         _check(lib().cao_runs_step(self._h, int(k), _stream()))

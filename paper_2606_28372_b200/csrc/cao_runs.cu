@@ -1,5 +1,6 @@
 // cao_runs.cu -- host side of the repair query and of the runs half of include/cao.h (S2-S7).
 #include <algorithm>
+#include <cmath>
 #include <cstring>
 #include <curand_kernel.h>
 #include "cao_runs_kernels.cuh"
@@ -282,6 +283,16 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
     r->lay = gen_layout(s, algo, (uint32_t)pop);
     r->gen_threads = r->lay.G * r->lay.NG;
     r->gen_smem = ((size_t)r->lay.cta_words + (size_t)r->lay.NG * r->lay.words) * 4;
+    {   // default execution mode: how many invalid candidates will fall through the bitmap probes to the table scan?
+        // For a uniformly random invalid point, P(no valid row within Hamming distance L) ~ exp(-density * E_L), E_L =
+        // number of rows within distance L (levels probed).  Scans by a single group are slow, so above 1 % the phased
+        // pipeline (whole-GPU k_scan per generation) is the default; cao_runs_set_mode overrides.
+        double e[CAO_MAX_PROBE_LEVEL + 1] = {1, 0, 0, 0, 0, 0, 0}, E = 0;
+        for (int d = 0; d < s->meta.n; ++d) for (int h = CAO_MAX_PROBE_LEVEL; h >= 1; --h) e[h] += e[h - 1] * (double)(s->meta.m[d] - 1);
+        for (int h = 1; h <= s->probe.levels; ++h) E += e[h];
+        const double p_scan = std::exp(-(double)s->meta.V / (double)s->meta.N * E);
+        r->mode = p_scan > 0.01 ? 0 : 1;
+    }
     if (r->gen_smem > 227 * 1024) r->mode = 0;                         // the population does not fit one SM: phased only
     const size_t P = (size_t)pop, n = (size_t)s->meta.n;
     r->smem_init = P * 4;
@@ -366,6 +377,12 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
         CAO_LAUNCHED("k_finish");
         r->gen = g;
     }
+    return CAO_OK;
+}
+
+int cao_runs_mode(const cao_runs* r, int32_t* mode) {
+    if (!r || !mode) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_mode: NULL argument");
+    *mode = r->mode;
     return CAO_OK;
 }
 

@@ -193,3 +193,12 @@ def test_auto_probe_levels():
     assert gpu_space(1, os_, sp).probe_levels == 6
     sp0, os0 = oracle_space(0)
     assert gpu_space(0, os0, sp0).probe_levels == 1
+
+
+def test_default_execution_mode():
+    """Fused unless the estimated share of candidates that reach the table scan is above 1 % (configs[3])."""
+    import paper_2606_28372_b200 as cao
+    for cfg, want in ((0, "fused"), (1, "fused"), (2, "fused"), (3, "phased")):
+        sp, os_ = oracle_space(cfg)
+        g = gpu_space(cfg, os_, sp)
+        assert cao.Runs(g, "firefly", n_runs=2, pop=8, max_gens=1).mode == want, cfg
