@@ -52,8 +52,9 @@ __global__ void __launch_bounds__(256) k_build_tables(const __grid_constant__ Sp
             s_ci[p] = (uint16_t)c;
         }
     }
-    // rows per CTA pass: at most 256 program runs (phase A), 2048 patterns (phase B, 8 per thread) and 64 rows
-    const uint32_t RPC = max(1u, min(min(Ci >= 256 ? 1u : 256u / Ci, 2048u / per_row), 64u));
+    // rows per CTA pass: at most 256 program runs (phase A, the slow part: one interpreter run per thread), 8192
+    // patterns (phase B, 32 cheap lookups per thread) and 64 rows
+    const uint32_t RPC = max(1u, min(min(Ci >= 256 ? 1u : 256u / Ci, 8192u / per_row), 64u));
     uint32_t* out32 = (uint32_t*)(tables + toff);
     for (uint32_t row0 = blockIdx.x * RPC; row0 < rows; row0 += gridDim.x * RPC) {
         const uint32_t nr = min(RPC, rows - row0);

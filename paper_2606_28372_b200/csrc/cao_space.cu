@@ -310,7 +310,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     uint8_t* d_flags = sc + s->off_flags;
     if (s->n_tab) {
         ProfScope ps(PK_TABLE, st);
-        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 2047) / 2048, 148 * 8), (unsigned)s->n_tab);
+        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 8191) / 8192, 148 * 8), (unsigned)s->n_tab);
         const uint32_t ci_cap = s->B <= 8192 ? (uint32_t)((s->B + 7) & ~7ull) : 0;
         const size_t tsm = 2 * (size_t)ci_cap + (size_t)std::max<uint64_t>(256, s->max_table_ci);
         if (tsm > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_build_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
