@@ -140,10 +140,13 @@ __device__ __forceinline__ uint32_t table_key(const int32_t* ds, const uint8_t* 
     return k;
 }
 
-// Pass 1a: which blocks survive the tabled constraints?  Every thread walks CH consecutive blocks with an odometer over
-// the outer digits (one mixed-radix decode per thread, then increments).  Per block: the row flags of the tabled
-// constraints, four independent byte loads at a time, exit at the first zero.  Survivors go to the live list
-// (warp-aggregated append; the order is irrelevant).  Nothing else is touched: a dead outer prefix costs a few bytes.
+// Pass 1a: which blocks survive the tabled constraints?  Every thread owns a CHUNK of CH consecutive blocks = all
+// combinations of the last k outer digits under one prefix of the others (CH = product of those k digits, chosen on the
+// host).  The tabled constraints are sorted: first the n_inv "chunk-invariant" ones, whose outer scope does not touch
+// the last k digits -- their row flags are tested ONCE per chunk and a failing prefix kills all CH blocks at once
+// (hierarchical pruning: on a sparse space nearly every chunk ends here, after a few byte loads) -- then the others,
+// per block, four independent byte loads at a time.  Survivors go to the live list together with their table row
+// indices (keys), first into shared memory, then with one global atomic per CTA.  Nothing else is touched.
 __global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
     extern __shared__ int32_t s_enum[];
     const uint32_t tid = threadIdx.x, bd = blockDim.x;
@@ -155,34 +158,51 @@ __global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta 
     __syncthreads();
     const uint64_t o0 = ((uint64_t)blockIdx.x * bd + tid) * a.CH;
     const bool mine = o0 < a.n_blocks;
-    if (mine) decode_outer(sm, a.t, o0, dig, bd);
-    for (uint32_t it = 0; it < a.CH; ++it) {
-        const uint64_t o = o0 + it;
-        bool alive = mine && o < a.n_blocks;
-        for (int c0 = 0; c0 < a.n_tab && alive; c0 += 4) {
+    bool chunk_alive = mine;
+    if (mine) {
+        decode_outer(sm, a.t, o0, dig, bd);
+        for (int c0 = 0; c0 < a.n_inv && chunk_alive; c0 += 4) {        // chunk-invariant constraints: once per CH blocks
             uint8_t f[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 f[u] = 1;
-                if (c0 + u < a.n_tab) {
+                if (c0 + u < a.n_inv) {
                     const int32_t* ds = desc + desc[c0 + u];
                     f[u] = __ldg(&a.flags[(uint32_t)ds[TD_FOFF] + table_key(ds, dig, bd)]);
                 }
             }
-            alive = f[0] && f[1] && f[2] && f[3];
+            chunk_alive = f[0] && f[1] && f[2] && f[3];
         }
-        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, alive);
-        if (bal) {                                                      // the CTA collects its survivors in shared memory
-            uint32_t base = 0;
-            if ((tid & 31) == 0) base = atomicAdd(&s_n, (uint32_t)__popc(bal));
-            base = __shfl_sync(0xFFFFFFFFu, base, 0);
-            if (alive) s_list[base + __popc(bal & ((1u << (tid & 31)) - 1u))] = (uint32_t)o;   // n_blocks < 2^32
-        }
-        if (mine) {
-            for (int d = a.t - 1; d >= 0; --d) {                        // odometer: next block
-                const uint32_t v = dig[d * bd] + 1u;
-                if (v < sm.m[d]) { dig[d * bd] = (uint8_t)v; break; }
-                dig[d * bd] = 0;
+    }
+    if (__syncthreads_or(chunk_alive)) {
+        for (uint32_t it = 0; it < a.CH; ++it) {
+            const uint64_t o = o0 + it;
+            bool alive = chunk_alive && o < a.n_blocks;
+            for (int c0 = a.n_inv; c0 < a.n_tab && alive; c0 += 4) {
+                uint8_t f[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    f[u] = 1;
+                    if (c0 + u < a.n_tab) {
+                        const int32_t* ds = desc + desc[c0 + u];
+                        f[u] = __ldg(&a.flags[(uint32_t)ds[TD_FOFF] + table_key(ds, dig, bd)]);
+                    }
+                }
+                alive = f[0] && f[1] && f[2] && f[3];
+            }
+            const uint32_t bal = __ballot_sync(0xFFFFFFFFu, alive);
+            if (bal) {                                                  // the CTA collects its survivors in shared memory
+                uint32_t base = 0;
+                if ((tid & 31) == 0) base = atomicAdd(&s_n, (uint32_t)__popc(bal));
+                base = __shfl_sync(0xFFFFFFFFu, base, 0);
+                if (alive) s_list[base + __popc(bal & ((1u << (tid & 31)) - 1u))] = (uint32_t)o;   // n_blocks < 2^32
+            }
+            if (chunk_alive) {
+                for (int d = a.t - 1; d >= 0; --d) {                    // odometer: next block
+                    const uint32_t v = dig[d * bd] + 1u;
+                    if (v < sm.m[d]) { dig[d * bd] = (uint8_t)v; break; }
+                    dig[d * bd] = 0;
+                }
             }
         }
     }
@@ -191,6 +211,20 @@ __global__ void __launch_bounds__(256) k_enum(const __grid_constant__ SpaceMeta 
     if (tid == 0 && n) s_base = atomicAdd(a.live_count, n);             // one global atomic per CTA
     __syncthreads();
     for (uint32_t e = tid; e < n; e += bd) a.live[s_base + e] = s_list[e];
+}
+
+// Table row indices (keys) of every live block, one thread per block (the survivors cluster in a few CTAs of k_enum, so
+// this is a separate, balanced pass): k_masks then reads keys instead of decoding the block for every mask word.
+__global__ void __launch_bounds__(256) k_keys(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
+    extern __shared__ int32_t s_enum[];
+    const uint32_t tid = threadIdx.x, bd = blockDim.x;
+    const int32_t* desc = stage_desc(a, s_enum);
+    uint8_t* dig = (uint8_t*)(s_enum + (a.desc_in_smem ? a.desc_words : 0)) + tid;
+    const uint32_t nlive = *a.live_count;
+    for (uint32_t li = blockIdx.x * bd + tid; li < nlive; li += gridDim.x * bd) {
+        decode_outer(sm, a.t, a.live[li], dig, bd);
+        for (int c = 0; c < a.n_tab; ++c) a.keys[(uint64_t)li * a.n_tab + c] = table_key(desc + desc[c], dig, bd);
+    }
 }
 
 // Pass 1b: one thread per (live block, word of its mask): AND of one row word per tabled constraint (independent
@@ -208,7 +242,7 @@ __global__ void __launch_bounds__(256) k_masks(const __grid_constant__ SpaceMeta
     for (uint64_t e = (uint64_t)blockIdx.x * bd + tid; e < total; e += (uint64_t)gridDim.x * bd) {
         const uint32_t li = (uint32_t)(e / a.Wb), j = (uint32_t)(e - (uint64_t)li * a.Wb);
         const uint64_t o = a.live[li];
-        decode_outer(sm, a.t, o, dig, bd);
+        if (!a.keys) decode_outer(sm, a.t, o, dig, bd);
         uint64_t w = (j + 1 == a.Wb && tail_bits < 64) ? ((1ull << tail_bits) - 1ull) : ~0ull;
         for (int c0 = 0; c0 < a.n_tab && w; c0 += 4) {
             uint64_t r[4];
@@ -218,7 +252,8 @@ __global__ void __launch_bounds__(256) k_masks(const __grid_constant__ SpaceMeta
                 if (c0 + u < a.n_tab) {
                     const int32_t* ds = desc + desc[c0 + u];
                     const uint64_t toff = (uint32_t)ds[TD_TOFF] | ((uint64_t)(uint32_t)ds[TD_TOFF + 1] << 32);
-                    r[u] = __ldg(&a.tables[toff + (uint64_t)table_key(ds, dig, bd) * a.Wb + j]);
+                    const uint32_t key = a.keys ? a.keys[(uint64_t)li * a.n_tab + c0 + u] : table_key(ds, dig, bd);
+                    r[u] = __ldg(&a.tables[toff + (uint64_t)key * a.Wb + j]);
                 }
             }
             w &= r[0] & r[1] & r[2] & r[3];
@@ -448,7 +483,13 @@ __global__ void __launch_bounds__(256) k_cnt_reduce(const uint32_t* __restrict__
     __shared__ uint64_t carry_s;
     uint64_t base = (uint64_t)blockIdx.x * SCAN_CHUNK + threadIdx.x * 16;
     uint32_t s = 0;
-    for (int k = 0; k < 16; ++k) if (base + k < nd) s += cnt[base + k];
+    if (base + 16 <= nd) {                                              // four independent 128-bit loads (the buffer is 256-byte aligned)
+        const uint4* q = (const uint4*)(cnt + base);
+        const uint4 a0 = q[0], a1 = q[1], a2 = q[2], a3 = q[3];
+        s = a0.x + a0.y + a0.z + a0.w + a1.x + a1.y + a1.z + a1.w + a2.x + a2.y + a2.z + a2.w + a3.x + a3.y + a3.z + a3.w;
+    } else {
+        for (int k = 0; k < 16; ++k) if (base + k < nd) s += cnt[base + k];
+    }
     for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
     if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
     __syncthreads();
@@ -484,7 +525,15 @@ __global__ void __launch_bounds__(256) k_cnt_apply(const uint32_t* __restrict__ 
     __shared__ uint32_t ws[8];
     uint64_t base = (uint64_t)blockIdx.x * SCAN_CHUNK + threadIdx.x * 16;
     uint32_t v[16], s = 0;
-    for (int k = 0; k < 16; ++k) { v[k] = (base + k < nd) ? cnt[base + k] : 0; s += v[k]; }
+    if (base + 16 <= nd) {
+        const uint4* q = (const uint4*)(cnt + base);
+        const uint4 a0 = q[0], a1 = q[1], a2 = q[2], a3 = q[3];
+        v[0] = a0.x; v[1] = a0.y; v[2] = a0.z; v[3] = a0.w; v[4] = a1.x; v[5] = a1.y; v[6] = a1.z; v[7] = a1.w;
+        v[8] = a2.x; v[9] = a2.y; v[10] = a2.z; v[11] = a2.w; v[12] = a3.x; v[13] = a3.y; v[14] = a3.z; v[15] = a3.w;
+    } else {
+        for (int k = 0; k < 16; ++k) v[k] = (base + k < nd) ? cnt[base + k] : 0;
+    }
+    for (int k = 0; k < 16; ++k) s += v[k];
     uint32_t inc = s;
     for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o); if ((threadIdx.x & 31) >= o) inc += t; }
     if ((threadIdx.x & 31) == 31) ws[threadIdx.x >> 5] = inc;

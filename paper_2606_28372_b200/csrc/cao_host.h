@@ -56,7 +56,10 @@ struct cao_space {
     // enumeration plan
     int t = 0;                         // first inner digit: digits t..n-1 form one bitmap block of B configs
     uint64_t B = 0, n_blocks = 0, nd = 0, n_words = 0;
-    uint32_t Wb = 0, CH = 1;           // u64 words per block mask; blocks per thread of k_enum
+    uint32_t Wb = 0, CH = 1;           // u64 words per block mask; blocks per thread of k_enum (product of the last outer digits)
+    int n_inv = 0, chunk_digits = 0;   // tabled constraints that do not read those digits; how many digits
+    uint64_t off_keys = 0; bool use_keys = false;
+    cudaStream_t side2 = nullptr; cudaEvent_t ev_fork2 = nullptr, ev_join2 = nullptr;   // residual prefix || masks
     std::vector<ConsPlan> plan;
     std::vector<int32_t> desc;         // descriptor words uploaded to the device
     int n_tab = 0, n_res = 0, n_rc = 0;
@@ -95,8 +98,10 @@ struct EnumArgs {
     const uint8_t* flags;              // one byte per table row: the row has a bit set
     uint64_t* bitmap;                  // zero-filled
     uint32_t* cnt;                     // per-512 counts (zeroed)
-    uint32_t* live;                    // blocks that survive the tables (only with residual constraints)
+    uint32_t* live;                    // blocks that survive the tabled constraints
     uint32_t* live_count;
+    uint32_t* keys;                    // [live][n_tab] table row index of every survivor (NULL: k_masks recomputes them)
+    int32_t n_inv;                     // the first n_inv tabled constraints do not read the last outer digits (chunk-invariant)
     uint32_t Wb, CH;
     int32_t t, n_tab, n_res;
     uint32_t desc_words, desc_in_smem; // the descriptor words are staged in shared memory by every CTA (when they fit)

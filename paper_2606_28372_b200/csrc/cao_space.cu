@@ -104,6 +104,9 @@ void cao_space_destroy(cao_space* s) {
     if (s->ev_fork) cudaEventDestroy(s->ev_fork);
     if (s->ev_join) cudaEventDestroy(s->ev_join);
     if (s->side) cudaStreamDestroy(s->side);
+    if (s->ev_fork2) cudaEventDestroy(s->ev_fork2);
+    if (s->ev_join2) cudaEventDestroy(s->ev_join2);
+    if (s->side2) cudaStreamDestroy(s->side2);
     delete s;
 }
 
@@ -167,8 +170,13 @@ static int plan_space(cao_space* s) {
     while (t > 0 && B < 256) { --t; B *= M.m[t]; }
     s->t = t; s->B = B; s->Wb = (uint32_t)((B + 63) / 64); s->n_blocks = M.N / B;
     s->n_words = (M.N + 63) / 64; s->nd = (M.N + 511) / 512;
-    // blocks per thread of k_enum: one decode per thread, then an odometer; keep at least ~150 k threads
-    s->CH = (uint32_t)std::min<uint64_t>(16, std::max<uint64_t>(1, s->n_blocks / (148ull * 1024)));
+    // chunk of k_enum = all combinations of the last k outer digits (product CH <= 32, and enough threads left)
+    s->CH = 1; s->chunk_digits = 0;
+    for (int d = t - 1; d >= 0; --d) {
+        const uint64_t c2 = (uint64_t)s->CH * M.m[d];
+        if (c2 > 32 || s->n_blocks / c2 < 148ull * 256) break;
+        s->CH = (uint32_t)c2; s->chunk_digits += 1;
+    }
     // per-constraint plan
     s->plan.assign(s->cons.size(), ConsPlan());
     uint64_t total_words = 0, total_flags = 0;
@@ -199,6 +207,11 @@ static int plan_space(cao_space* s) {
     std::vector<int> tab, res;
     for (size_t c = 0; c < s->cons.size(); ++c) (s->plan[c].tabled ? tab : res).push_back((int)c);
     std::stable_sort(tab.begin(), tab.end(), [&](int a, int b) { return s->plan[a].rows < s->plan[b].rows; });
+    // chunk-invariant constraints (no outer scope digit among the last chunk_digits) come first
+    auto invariant = [&](int c) { for (int d : s->plan[c].outer) if (d >= t - s->chunk_digits) return false; return true; };
+    std::stable_sort(tab.begin(), tab.end(), [&](int a, int b) { return invariant(a) > invariant(b); });
+    s->n_inv = 0;
+    for (int c : tab) if (invariant(c)) s->n_inv += 1;
     s->n_tab = (int)tab.size(); s->n_res = (int)res.size();
     std::vector<int32_t>& D = s->desc;
     D.assign(tab.size() + res.size() + s->cons.size(), 0);       // [tab offs][res offs][program offs of every constraint]
@@ -267,6 +280,8 @@ static int plan_space(cao_space* s) {
     s->off_V = off; off = align256(off + 32);                     // V (u64), scan ticket, live count, group count
     s->off_cnt = off; off = align256(off + (s->nd + 1) * 4);
     s->off_live = off; off = align256(off + s->n_blocks * 4);
+    s->use_keys = s->n_tab > 0 && s->n_blocks * (uint64_t)s->n_tab * 4 <= (64ull << 20);
+    s->off_keys = off; off = align256(off + (s->use_keys ? s->n_blocks * (uint64_t)s->n_tab * 4 : 1));
     s->off_pre = off; off = align256(off + (s->n_res ? s->n_blocks * (uint64_t)s->n_res * sizeof(ResPrefix) : 1));
     s->off_groups = off; off = align256(off + (s->nd + 1) * 4);
     s->rc_bytes = align256((uint64_t)CAO_HS * 8) + align256((uint64_t)CAO_HS * s->Wb * 8) + 256;
@@ -291,6 +306,9 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         CAO_CUDA(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
         CAO_CUDA(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
         CAO_CUDA(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+        CAO_CUDA(cudaStreamCreateWithFlags(&s->side2, cudaStreamNonBlocking));
+        CAO_CUDA(cudaEventCreateWithFlags(&s->ev_fork2, cudaEventDisableTiming));
+        CAO_CUDA(cudaEventCreateWithFlags(&s->ev_join2, cudaEventDisableTiming));
     }
     s->meta.bitmap = (const uint64_t*)d_bitmap;
     // fork: the zero fill of the bitmap (N/8 bytes, HBM-bound) overlaps the table build (latency-bound)
@@ -328,6 +346,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     ea.B = s->B; ea.n_blocks = s->n_blocks; ea.dom = d_dom; ea.desc = d_desc; ea.tables = d_tables; ea.flags = d_flags;
     ea.bitmap = (uint64_t*)d_bitmap; ea.cnt = (uint32_t*)(sc + s->off_cnt);
     ea.live = (uint32_t*)(sc + s->off_live); ea.live_count = ctl + 3;
+    ea.keys = s->use_keys ? (uint32_t*)(sc + s->off_keys) : nullptr; ea.n_inv = s->n_inv;
     ea.Wb = s->Wb; ea.CH = s->CH; ea.t = s->t; ea.n_tab = s->n_tab; ea.n_res = s->n_res;
     ea.desc_words = (uint32_t)s->desc.size(); ea.desc_in_smem = s->desc.size() <= 8192;
     ea.n_rc = s->n_rc;
@@ -356,6 +375,14 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
             k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem_enum, st>>>(s->meta, ea);
         }
         CAO_LAUNCHED("k_enum");
+        if (s->use_keys) {
+            k_keys<<<(unsigned)std::min<uint64_t>((s->n_blocks + bd - 1) / bd, 148ull * 4), bd, smem_dig, st>>>(s->meta, ea);
+            CAO_LAUNCHED("k_keys");
+        }
+        if (s->n_res) {                                                 // fork: the residual prefixes need the live list only
+            CAO_CUDA(cudaEventRecord(s->ev_fork2, st));
+            CAO_CUDA(cudaStreamWaitEvent(s->side2, s->ev_fork2, 0));
+        }
         ProfScope ps(PK_PROBE, st);
         const uint64_t items = s->n_blocks * (uint64_t)s->Wb;
         k_masks<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 16), bd, smem_dig, st>>>(s->meta, ea);
@@ -365,15 +392,17 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         ResPrefix* pre = (ResPrefix*)(sc + s->off_pre);
         const uint64_t items = s->n_blocks * (uint64_t)s->n_res;
         {
-            ProfScope ps(PK_QUERY, st);
-            k_res_prefix<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 8), bd, smem_desc, st>>>(s->meta, ea, pre);
+            ProfScope ps(PK_QUERY, s->side2);
+            k_res_prefix<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 8), bd, smem_desc, s->side2>>>(s->meta, ea, pre);
         }
         CAO_LAUNCHED("k_res_prefix");
         if (s->n_rc) {
-            ProfScope ps(PK_QUERY, st);
-            k_res_class_table<<<dim3(148 * 4, (unsigned)s->n_rc), 256, 0, st>>>(s->meta, ea);
+            ProfScope ps(PK_QUERY, s->side2);
+            k_res_class_table<<<dim3(148 * 4, (unsigned)s->n_rc), 256, 0, s->side2>>>(s->meta, ea);
             CAO_LAUNCHED("k_res_class_table");
         }
+        CAO_CUDA(cudaEventRecord(s->ev_join2, s->side2));
+        CAO_CUDA(cudaStreamWaitEvent(st, s->ev_join2, 0));              // join: k_residual needs the masks and the prefixes
         ProfScope ps(PK_RESID, st);
         const uint64_t warps = std::min<uint64_t>(s->n_blocks, 148ull * 64);
         k_residual<<<(unsigned)((warps + 7) / 8), bd, smem_desc, st>>>(s->meta, ea, pre);
