@@ -362,7 +362,7 @@ def gpu_arm(args):
 
     # ---- S1 alone (BASELINE metric "enumeration Gcfg/s"): configs[1..3], resident buffers
     enum = {}
-    for cfg in ([1, 2, 3] if not args.no_enum else []):
+    for cfg in ([int(c) for c in args.enum_cfgs.split(",")] if not args.no_enum else []):
         spx = W.WORKLOADS[cfg].space()
         gx = cao.Space.from_space(spx)
         gx.alloc_build(); gx.build_count(); gx.alloc_table(); gx.build_fill()
@@ -371,17 +371,19 @@ def gpu_arm(args):
         es = torch.cuda.Stream(device=dev)                                # cao_space_rebuild replays its CUDA graph on a real stream
         with torch.cuda.stream(es):
             gx.rebuild(); es.synchronize()                                # capture + first replay (untimed)
-            for _ in range(11):                                           # resident inputs, no host round trip
+            for _ in range(args.enum_reps):                               # resident inputs, no host round trip
                 flush.zero_()
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(); gx.rebuild(); e1.record(); e1.synchronize()
                 ts.append(e0.elapsed_time(e1))
-        cao.profile_enable(True)
-        for _ in range(5):
-            flush.zero_(); gx.rebuild()
-        torch.cuda.synchronize()
-        kp = {k: v[0] / 5 * 1e3 for k, v in cao.profile_read().items() if v[1]}
-        cao.profile_enable(False)
+        kp = {}
+        if not args.no_kernel_times:
+            cao.profile_enable(True)
+            for _ in range(5):
+                flush.zero_(); gx.rebuild()
+            torch.cuda.synchronize()
+            kp = {k: v[0] / 5 * 1e3 for k, v in cao.profile_read().items() if v[1]}
+            cao.profile_enable(False)
         Nx, Vx, nx, rbx = gx.sizes()
         lb = gx.ltab_bytes
         t = float(np.median(ts)) / 1e3
@@ -416,7 +418,7 @@ def gpu_arm(args):
     # ---- the generation step of configs[2] (GA, P 64, 10^4 runs, 150 generations) and configs[3] (Firefly, P 128,
     # 1000 runs, 100 generations: the repair-scan stress case) at their BASELINE sizes, fused and phased
     other = {}
-    for cfg in ([2, 3] if not args.no_other else []):
+    for cfg in ([int(c) for c in args.other_cfgs.split(",")] if not args.no_other else []):
         w = workload(cfg, None)
         spx = w["space"]
         gx = cao.Space.from_space(spx).build()
@@ -425,7 +427,7 @@ def gpu_arm(args):
         leg = {"workload": f"BASELINE configs[{cfg}] ({spx.name}): N={Nx} V={Vx} n={nx}; {w['algos'][0]}, pop {w['pop']}, "
                            f"{w['gens']} generations, {w['runs']} runs", "probe_levels": gx.probe_levels,
                "default_mode": cao.Runs(gx, w["algos"][0], n_runs=2, pop=w["pop"], max_gens=1).mode}
-        for mode in ("fused", "phased"):
+        for mode in args.other_modes.split(","):
             best_ms = None
             for rep in range(2):
                 rr = cao.Runs(gx, w["algos"][0], n_runs=w["runs"], pop=w["pop"], budget=w["budget"], max_gens=w["gens"],
@@ -511,6 +513,11 @@ def main():
     ap.add_argument("--no-other", action="store_true", help="skip the configs[2] / configs[3] generation-step legs")
     ap.add_argument("--no-peak", action="store_true", help="skip the integer issue-rate microbenchmarks")
     ap.add_argument("--sweep-points", type=int, default=4, help="how many of the run counts 1e2, 1e3, 1e4, 1e5 to sweep")
+    ap.add_argument("--enum-cfgs", default="1,2,3", help="configs of the S1 leg")
+    ap.add_argument("--enum-reps", type=int, default=11, help="timed rebuilds per config of the S1 leg")
+    ap.add_argument("--no-kernel-times", action="store_true", help="S1 leg: skip the per-kernel event timing pass")
+    ap.add_argument("--other-cfgs", default="2,3", help="configs of the generation-step legs")
+    ap.add_argument("--other-modes", default="fused,phased", help="execution modes of the generation-step legs")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_arm(args)

@@ -283,6 +283,11 @@ __device__ __forceinline__ void store_state(const Grp& g, const SpaceMeta& sm, c
         unsigned long long tot = 0;
         for (int z = 0; z < 6; ++z) { atomicAdd(&rm.counters[8 + z], gs->cyc[z]); tot += gs->cyc[z]; }
         atomicMax(&rm.counters[14], tot);                               // slowest run (cycles)
+#ifdef CAO_GEN_STATS_PRINT
+        if (tot > CAO_GEN_STATS_PRINT)
+            printf("run %u cyc %llu: op %llu tail %llu p2 %llu p3 %llu scan %llu fin %llu | inv %u p2n %u p3n %u memo %u rc %u\n", k, tot,
+                   gs->cyc[0], gs->cyc[1], gs->cyc[2], gs->cyc[3], gs->cyc[4], gs->cyc[5], gs->n_inv, gs->n_p2, gs->n_p3, gs->n_memo, gs->n_rc);
+#endif
         atomicMax(&rm.counters[15], gs->cyc[4]);                        // most scan cycles in one run
 #endif
     }

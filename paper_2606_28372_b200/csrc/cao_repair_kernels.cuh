@@ -111,7 +111,7 @@ __device__ __forceinline__ uint32_t grp_push(bool pred, uint32_t* counter, bool 
 // (sum |delta| << 40 | L') of a row is L + the sum of its neighbours' contributions (the fields cannot interfere:
 // 0 <= L' < 2^40, sum |delta| < 2^13).  The first two neighbours come from the flattened pair list (spread over the
 // threads, four independent bit tests in flight), levels >= 4 add a depth-first walk over the middle ones, the last one
-// is a serial loop with four loads in flight.  The level minimum is exact because Hamming is the primary key.  ptab:
+// is a serial loop with eight loads in flight.  The level minimum is exact because Hamming is the primary key.  ptab:
 // pm.NB words of shared memory owned by the group.  *slot must be ~0 and visible to the group on entry.  Returns the
 // level that found a valid neighbour (0 = none), group-uniform, and leaves (sad << 40 | L') in *slot.
 static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t* __restrict__ bitmap, const uint64_t* stride,
@@ -149,17 +149,17 @@ static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t*
                 tcur[0] = pm.nb_first[(nb[pr >> 16] >> 8) + 1];
                 int depth = 0;
                 for (;;) {
-                    if (depth == extra) {                               // innermost neighbour: serial loop, 4 loads in flight
+                    if (depth == extra) {                               // innermost neighbour: serial loop, 8 loads in flight
                         const uint64_t Kb = Kst[depth];
-                        for (uint32_t t0 = tcur[depth]; t0 < NB; t0 += 4) {
-                            uint64_t k3[4]; bool bit[4];
+                        for (uint32_t t0 = tcur[depth]; t0 < NB; t0 += 8) {
+                            uint64_t k3[8]; bool bit[8];
 #pragma unroll
-                            for (int u = 0; u < 4; ++u) {
+                            for (int u = 0; u < 8; ++u) {
                                 k3[u] = Kb + ptab[t0 + u < NB ? t0 + u : t0];
                                 bit[u] = bit_test(bitmap, k3[u] & M40) && t0 + u < NB;
                             }
 #pragma unroll
-                            for (int u = 0; u < 4; ++u) if (bit[u]) best = k3[u] < best ? k3[u] : best;
+                            for (int u = 0; u < 8; ++u) if (bit[u]) best = k3[u] < best ? k3[u] : best;
                         }
                         if (depth == 0) break;
                         --depth; ++tcur[depth];
