@@ -10,7 +10,7 @@ import numpy as np
 from .build import build as _build
 
 ALGOS = {"de": 0, "pso": 1, "firefly": 2, "ga": 3}
-STREAMS = {"init": 0, "op": 1, "mut": 2, "reinit": 3}
+STREAMS = {"init": 0, "op": 1, "mut": 2, "reinit": 3, "repair": 5}
 
 
 class HParams(C.Structure):
@@ -23,6 +23,22 @@ class HParams(C.Structure):
     @classmethod
     def default(cls):
         return cls(0.7, 0.6, 0.5, 3.0, 0.5, 1.0, 1.0, 0.2, 5, 3)
+
+
+class Variant(C.Structure):
+    """SURVEY 8(f) switches (oracle/cao_oracle.cc `Variant`); the default is the north_star path."""
+    _fields_ = [("aware", C.c_int32), ("repair_mode", C.c_int32), ("de_mutation", C.c_int32), ("de_crossover", C.c_int32),
+                ("ga_crossover", C.c_int32), ("init_lhs", C.c_int32), ("penalty", C.c_float), ("reserved", C.c_int32)]
+    DE_MUTATION = {"best1": 0, "rand1": 1, "currenttobest1": 2, "randtobest1": 3, "best2": 4, "rand2": 5}
+    DE_CROSSOVER = {"bin": 0, "exp": 1}
+    GA_CROSSOVER = {"single_point": 0, "two_point": 1, "uniform": 2, "disruptive_uniform": 3}
+
+    @classmethod
+    def make(cls, aware=True, repair_mode=0, de_mutation="best1", de_crossover="bin", ga_crossover="single_point",
+             init_lhs=False, penalty=1e20):
+        g = lambda table, v: table[v] if isinstance(v, str) else int(v)
+        return cls(int(bool(aware)), int(repair_mode), g(cls.DE_MUTATION, de_mutation), g(cls.DE_CROSSOVER, de_crossover),
+                   g(cls.GA_CROSSOVER, ga_crossover), int(bool(init_lhs)), float(penalty), 0)
 
 
 _lib = None
@@ -60,6 +76,16 @@ def lib():
             "orc_space_set_objective": (C.c_int, [vp, f32p]),
             "orc_runs_create": (vp, [vp, C.c_int, C.POINTER(HParams), C.c_uint32, C.c_uint32, C.c_int32,
                                      C.c_uint32, C.c_uint32, C.c_uint64]),
+            "orc_runs_create_ex": (vp, [vp, C.c_int, C.POINTER(HParams), C.POINTER(Variant), C.c_uint32, C.c_uint32, C.c_int32,
+                                        C.c_uint32, C.c_uint32, C.c_uint64]),
+            "orc_runs_n_penalised": (C.c_uint64, [vp]), "orc_runs_tap_rule": (u8p, [vp]),
+            "orc_space_neighbors": (C.c_uint64, [vp, u8p, C.c_int, u32p, C.c_uint64]),
+            "orc_space_repair_mode": (None, [vp, C.c_int, u8p, f32p, u32p, C.c_uint64, u32p, u8p]),
+            "orc_de_mutate_variant": (C.c_int, [C.c_int, C.c_float, C.c_int, C.c_int, i32p, C.c_int]),
+            "orc_lhs_rows": (None, [vp, C.c_uint64, C.c_uint32, C.c_int32, u8p]),
+            "orc_baseline": (C.c_double, [vp, C.c_uint64]),
+            "orc_baseline_budget": (C.c_uint64, [vp, C.c_double]),
+            "orc_runs_score": (C.c_double, [vp, u64p, C.c_uint32, C.POINTER(C.c_double)]),
             "orc_runs_destroy": (None, [vp]),
             "orc_runs_step": (None, [vp, C.c_uint32]),
             "orc_runs_gen": (C.c_uint32, [vp]),
@@ -101,6 +127,12 @@ def de_mutate_index(F, ibest, ia, ib, top): return int(lib().orc_de_mutate_index
 def clamp_pos(x, hi): return float(lib().orc_clamp_pos(C.c_float(x), C.c_float(hi)))
 def coord(M, k): return float(lib().orc_coord(M, k))
 def snap(M, m_d, x): return int(lib().orc_snap(M, m_d, C.c_float(x)))
+
+
+def de_mutate_variant(op, F, xi, best, donors, top):
+    r = np.zeros(5, np.int32); r[:len(donors)] = donors
+    return int(lib().orc_de_mutate_variant(Variant.DE_MUTATION[op] if isinstance(op, str) else op, C.c_float(F), xi, best,
+                                           _p(r, C.c_int32), top))
 
 
 def exp_neg_spec_many(z: np.ndarray) -> np.ndarray:
@@ -185,6 +217,38 @@ class OracleSpace:
             raise RuntimeError("set_objective before build")
         self._obj = a
 
+    # -- neighbour rules (L139-143) and the paper's repairs (L270, Alg.2, Alg.3)
+    def neighbors(self, row, rule) -> np.ndarray:
+        """Ranks of the valid neighbours of `row`; rule 0 strictly-adjacent, 1 adjacent, 2 Hamming."""
+        a = np.ascontiguousarray(row, dtype=np.uint8)
+        out = np.zeros(max(self.V, 1), np.uint32)
+        c = lib().orc_space_neighbors(self._h, _p(a, C.c_uint8), rule, _p(out, C.c_uint32), out.size)
+        return out[:c].copy()
+
+    def repair_mode(self, mode, rows, x=None, w=None):
+        """mode 'index' (L270) | 'alg2' (needs x: continuous positions) | 'alg3' (needs w: 32-bit draws) -> (rank, rule)."""
+        m = {"index": 1, "alg2": 2, "alg3": 3}[mode]
+        a = np.ascontiguousarray(rows, dtype=np.uint8).reshape(-1, self.n)
+        c = a.shape[0]
+        xx = np.ascontiguousarray(x if x is not None else np.zeros((c, self.n)), dtype=np.float32)
+        ww = np.ascontiguousarray(w if w is not None else np.zeros(c), dtype=np.uint32)
+        rank, rule = np.zeros(c, np.uint32), np.zeros(c, np.uint8)
+        lib().orc_space_repair_mode(self._h, m, _p(a, C.c_uint8), _p(xx, C.c_float), _p(ww, C.c_uint32), c,
+                                    _p(rank, C.c_uint32), _p(rule, C.c_uint8))
+        return rank, rule
+
+    def lhs_rows(self, seed, run_id, pop) -> np.ndarray:
+        out = np.zeros((pop, self.n), np.uint8)
+        lib().orc_lhs_rows(self._h, seed, run_id, pop, _p(out, C.c_uint8))
+        return out
+
+    # -- NEXT-4
+    def baseline(self, t) -> float:
+        return float(lib().orc_baseline(self._h, int(t)))
+
+    def baseline_budget(self, frac=0.95) -> int:
+        return int(lib().orc_baseline_budget(self._h, float(frac)))
+
     def __del__(self):
         try:
             lib().orc_space_destroy(self._h)
@@ -194,12 +258,13 @@ class OracleSpace:
 
 class OracleRuns:
     def __init__(self, space: OracleSpace, algo, n_runs, pop, budget=0, max_gens=0xFFFFFFFF, seed=0,
-                 first_run=0, hparams: HParams | None = None):
+                 first_run=0, hparams: HParams | None = None, variant: Variant | None = None):
         self.space, self.R, self.P, self.n = space, int(n_runs), int(pop), space.n
         self.algo = ALGOS[algo] if isinstance(algo, str) else int(algo)
         self.hp = hparams or HParams.default()
-        h = lib().orc_runs_create(space._h, self.algo, C.byref(self.hp), self.R, first_run, self.P, budget,
-                                  max_gens, seed)
+        self.variant = variant or Variant.make()
+        h = lib().orc_runs_create_ex(space._h, self.algo, C.byref(self.hp), C.byref(self.variant), self.R, first_run, self.P,
+                                     budget, max_gens, seed)
         if not h:
             raise ValueError("orc_runs_create rejected the arguments")
         self._h = C.c_void_p(h)
@@ -230,12 +295,21 @@ class OracleRuns:
         return dict(cand=g(L.orc_runs_tap_cand, (R, P, n)), valid=g(L.orc_runs_tap_valid, (R, P)),
                     rep_rank=g(L.orc_runs_tap_rep, (R, P)), eval_rank=g(L.orc_runs_tap_eval, (R, P)),
                     f=g(L.orc_runs_tap_f, (R, P)), accept=g(L.orc_runs_tap_accept, (R, P)),
-                    active=g(L.orc_runs_tap_active, (R,)))
+                    active=g(L.orc_runs_tap_active, (R,)), rule=g(L.orc_runs_tap_rule, (R, P)))
 
     @property
     def n_repaired(self): return int(lib().orc_runs_n_repaired(self._h))
     @property
     def n_evaluated(self): return int(lib().orc_runs_n_evaluated(self._h))
+    @property
+    def n_penalised(self): return int(lib().orc_runs_n_penalised(self._h))
+
+    def score(self, t):
+        """NEXT-4 (Eq.2): (score, per-sampling-point means) for the sampling points t (unique-evaluation counts)."""
+        tt = np.ascontiguousarray(t, dtype=np.uint64)
+        per = np.zeros(tt.size, np.float64)
+        sc = lib().orc_runs_score(self._h, _p(tt, C.c_uint64), tt.size, per.ctypes.data_as(C.POINTER(C.c_double)))
+        return float(sc), per
 
     def state(self):
         R, P, n = self.R, self.P, self.n
