@@ -465,6 +465,51 @@ def gpu_arm(args):
         del gx
     torch.cuda.empty_cache()
 
+    # ---- SURVEY 8(f) rows on configs[1] (1000 runs per algorithm, budget 1000 unique, cap 200 generations): the paper's
+    # own repairs (NEXT-1), the non-constraint-aware counterparts (NEXT-2), operator variants (NEXT-3), each timed like the
+    # headline step, and the performance score (NEXT-4, Eq.2) of every variant against the calculated random-search
+    # baseline -- score(aware) - score(unaware) is the quantity the paper's headline (+0.393 on its 24 spaces, L411) reports
+    nxt = {}
+    if not args.no_next:
+        spn = cao.Space.from_space(sp).build(); spn.set_objective(obj_d)
+        srt = spn.sorted_objective()
+        ts = [int(t) for t in np.linspace(P, wl["budget"] or 1000, 32)]
+        Bt = spn.baseline(srt, ts)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); srt = spn.sorted_objective(); e1.record(); e1.synchronize(); ms_sort = e0.elapsed_time(e1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); Bt = spn.baseline(srt, ts); e1.record(); e1.synchronize(); ms_base = e0.elapsed_time(e1)
+        variants = [("default", {}), ("unaware", dict(aware=False)), ("paper_repair", dict(repair_mode=1))]
+        extra = {"de": [("rand1exp", dict(de_mutation="rand1", de_crossover="exp")), ("lhs", dict(init_lhs=True))],
+                 "ga": [("uniform", dict(ga_crossover="uniform"))]}
+        for algo in wl["algos"]:
+            row = {}
+            for name, kw in variants + extra.get(algo, []):
+                best_ms = None
+                for rep in range(2):
+                    rr = cao.Runs(spn, algo, n_runs=R, pop=P, budget=wl["budget"], max_gens=G, seed=wl["seed"],
+                                  variant=cao.Variant.make(**kw) if kw else None)
+                    torch.cuda.synchronize(); flush.zero_()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(); rr.step(G); e1.record(); e1.synchronize()
+                    t = e0.elapsed_time(e1); best_ms = t if best_ms is None else min(best_ms, t)
+                    if rep == 1:
+                        st = rr.stats()
+                        sc, per = rr.score(srt, ts, Bt)
+                        row[name] = {"ms": best_ms, "mode": rr.mode, "candidates_per_s": st["n_evaluated"] / (best_ms / 1e3),
+                                     "n_repaired": st["n_repaired"], "n_scanned": st["n_scanned"], "n_penalised": st["n_penalised"],
+                                     "score": float(sc.item()), "score_at_budget": float(per[-1].item())}
+                    del rr
+            row["aware_minus_unaware_score"] = row["default"]["score"] - row["unaware"]["score"]
+            nxt[algo] = row
+        nxt["mean_aware_minus_unaware_score"] = float(np.mean([nxt[a]["aware_minus_unaware_score"] for a in wl["algos"]]))
+        nxt["score_sampling_points"] = f"32 points, {ts[0]}..{ts[-1]} unique evaluations"
+        nxt["sort_objective_ms"] = ms_sort; nxt["baseline_32_points_ms"] = ms_base
+        nxt["paper_context"] = "paper L411: +0.393 mean score gain from constraint-awareness on its 24 BAT search spaces (other hardware, other spaces)"
+        del spn
+    torch.cuda.empty_cache()
+
     # ---- CPU oracle on a bounded sample of the same workload (rank 0, N=1 only), and a spot check of the GPU against it
     cpu = None
     if world == 1 and not args.no_cpu:
@@ -497,9 +542,10 @@ def gpu_arm(args):
         "steps_cfg2": other.get("cfg2"),
         "steps_cfg3": other.get("cfg3"),
         "int_peak": int_peak,
+        "next_rows_cfg1": nxt,
         "extra": {"candidates_per_step": int(cands_step), "invalid_post_snap_per_step": int(repaired_step),
                   "scanned_per_step": int(scanned_step), "generations_done_sum": gens_done,
-                  "stats": {a: {k: v for k, v in s.items() if not k.startswith("cyc") and k != "r7"} for a, s in zip(wl["algos"], stats)},
+                  "stats": {a: {k: v for k, v in s.items() if not k.startswith("cyc") } for a, s in zip(wl["algos"], stats)},
                   "kernels": kern, "wall_s_timed_region": wall, "peaks": pk},
     }
     print(json.dumps(line), flush=True)
@@ -522,6 +568,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the configs[2] / configs[3] generation-step legs")
     ap.add_argument("--no-peak", action="store_true", help="skip the integer issue-rate microbenchmarks")
+    ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) legs (paper repairs, unaware variants, score)")
     ap.add_argument("--sweep-points", type=int, default=4, help="how many of the run counts 1e2, 1e3, 1e4, 1e5 to sweep")
     ap.add_argument("--enum-cfgs", default="1,2,3", help="configs of the S1 leg")
     ap.add_argument("--enum-reps", type=int, default=11, help="timed rebuilds per config of the S1 leg")

@@ -61,6 +61,28 @@ typedef struct {
     int32_t ga_beta_b;               /* 3: Beta(1,b) parent selection over the sorted rank (A18) */
 } cao_hparams;
 
+/* SURVEY 8(f) switches of a set of runs.  NULL / all-default = the north_star path (constraint-aware, unified repair
+ * key, DE best1bin, GA single_point, uniform initial sample).  Any non-default field selects the phased pipeline.
+ *   constraint_aware  1 (default); 0 = the paper's non-constraint-aware counterparts (L107, L272, L284): the initial
+ *                     population is random in the Cartesian space, nothing is repaired, an invalid configuration is
+ *                     not evaluated (no memo bit, no budget) and the strategy sees `penalty` instead       [NEXT-2, A33-A34]
+ *   repair_mode       0 = argmin (Hamming, sum|didx|, L) for every algorithm (north_star; A4);
+ *                     1 = the paper's own repairs: DE nearest by sum|didx| alone (L215, L270); PSO / Firefly Alg.2
+ *                     (L225-247): first non-empty of the strictly-adjacent / adjacent / Hamming neighbour sets
+ *                     (L139-143; A28), member nearest to the particle's continuous position (squared Euclidean distance,
+ *                     fp32; A30); GA Alg.3 (L298-309): a random member of that set (draw stream 5, slot 0).  Ties: smallest
+ *                     L (A5).  All three sets empty: the configuration stays invalid and is penalised     [NEXT-1]
+ *   de_mutation       0 best1 (default), 1 rand1, 2 currenttobest1, 3 randtobest1, 4 best2, 5 rand2 (L219, L272; A29)
+ *   de_crossover      0 binomial (default), 1 exponential (L272)
+ *   ga_crossover      0 single_point (default), 1 two_point, 2 uniform, 3 disruptive_uniform (L288; A31)
+ *   init_lhs          1 = DE's initial population by Latin Hypercube Sampling, repaired to valid (L223; A35)   [NEXT-3]
+ *   penalty           objective reported for an unevaluated invalid configuration, > 0 and finite (L107: 1e20)          */
+typedef struct {
+    int32_t constraint_aware, repair_mode, de_mutation, de_crossover, ga_crossover, init_lhs;
+    float penalty;
+    int32_t reserved;
+} cao_variant;
+
 /* Constraint programs: postfix (RPN) over int64, one int32 word per token (O1, A2, A3).
  * PUSH_PARAM is followed by the parameter number, PUSH_CONST by the low and the high 32 bits.
  * DIV/MOD truncate toward zero; a zero divisor makes the whole constraint false; ADD/SUB/MUL/NEG
@@ -129,6 +151,15 @@ int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t c
 int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
 int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
                      uint64_t* d_key_out, int32_t probe_levels, void* d_scratch, void* stream);
+/* NEXT-1 standalone (L139-143, L215, L270, Alg.2, Alg.3): the paper's own repairs for `count` rows.
+ * mode 1 = index distance: d_rank_out[i] = argmin (sum |didx|, L);  2 = Alg.2 with d_x: count x n fp32 continuous
+ * positions (row-major);  3 = Alg.3 with d_w: count 32-bit draws (member number floor(w K / 2^32) of the first non-empty
+ * neighbour set, ascending L).  Valid rows map to themselves.  d_rank_out[i] = 0xFFFFFFFF when every neighbour set is
+ * empty; d_rule_out (optional) receives the set used (0/1/2, 3 = none, 255 = valid row or mode 1).  Rows must be
+ * in-domain.  d_scratch: cao_space_repair_mode_scratch_bytes(count) bytes, 256-byte aligned. */
+int cao_space_repair_mode_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
+int cao_space_repair_mode(const cao_space* s, int32_t mode, const uint8_t* d_idx_rows, const float* d_x, const uint32_t* d_w,
+                          uint64_t count, uint32_t* d_rank_out, uint8_t* d_rule_out, void* d_scratch, void* stream);
 /* Objective table by rank: V floats, > 0 and finite (borrowed; L268: the evaluation is a lookup). */
 int cao_space_set_objective(cao_space* s, const float* d_obj);
 
@@ -142,6 +173,14 @@ int cao_runs_workspace_bytes(const cao_space* s, int32_t algo, int32_t pop, uint
 int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uint32_t n_runs,
                     uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens,
                     uint64_t seed, void* d_workspace, void* stream, cao_runs** out);
+/* The same with the SURVEY 8(f) switches (var == NULL: defaults = cao_runs_create).  The workspace of a non-default
+ * variant is larger: size it with cao_runs_workspace_bytes_ex.  Errors: CAO_E_INVALID_ARG for an unknown switch value,
+ * init_lhs with an algorithm other than DE or with constraint_aware = 0, a DE population smaller than donors + 1. */
+int cao_runs_workspace_bytes_ex(const cao_space* s, int32_t algo, const cao_variant* var, int32_t pop, uint32_t n_runs,
+                                uint32_t max_gens, uint64_t* bytes);
+int cao_runs_create_ex(const cao_space* s, int32_t algo, const cao_hparams* hp, const cao_variant* var, uint32_t n_runs,
+                       uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens, uint64_t seed,
+                       void* d_workspace, void* stream, cao_runs** out);
 void cao_runs_destroy(cao_runs* r);
 /* How cao_runs_step executes: 1 = one fused persistent kernel (a warp group per run, population state in shared
  * memory for all the requested generations); 0 = phased, per generation k_op -> k_probe23 -> k_scan -> k_finish over
@@ -163,6 +202,9 @@ int cao_runs_trajectory(const cao_runs* r, const void** d_traj, uint32_t* gens_r
 int cao_runs_debug_last(const cao_runs* r, const uint8_t** d_postsnap_rows, const uint8_t** d_valid,
                         const uint32_t** d_repaired_rank, const uint32_t** d_eval_rank, const float** d_f,
                         const uint8_t** d_accept, const uint8_t** d_active);
+/* NEXT-1 tap of the last stepped generation, [run][ind]: neighbour rule that repaired the candidate (0 strictly-adjacent,
+ * 1 adjacent, 2 Hamming), 3 = every set empty, 255 = not applicable (valid candidate, or another repair mode). */
+int cao_runs_debug_rule(const cao_runs* r, const uint8_t** d_rule);
 /* Raw population state, borrowed.  which: 0 idx rows [run][ind][row_bytes] u8, 1 rank [run][ind] u32,
  * 2 f [run][ind] f32, 3 x, 4 v, 5 pbest [run][dim][ind] f32 (dimension-major), 6 pbest_f [run][ind]. */
 int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, uint64_t* bytes);
@@ -178,6 +220,19 @@ int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uin
  * -DCAO_GEN_STATS, else 0); 16-24 candidates of the stepped generations by Hamming distance of their repair
  * (16 = valid, 17 = Hamming 1, ..., 24 = eight or more; L143, L215); 25-31 reserved. */
 int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out32);
+/* NEXT-4 (Eq.2; A36): performance score of a set of runs against the calculated random-search baseline
+ * B(t) = expected minimum of t draws without replacement from the V objective values (fp64).
+ *   cao_space_sort_objective: d_sorted = the objective table in ascending order (V floats; d_scratch: the next power of
+ *                             two >= V floats).
+ *   cao_space_baseline:       d_B[q] = B(d_t[q]) for S sampling points (unique-evaluation counts, clamped to 1..V).
+ *   cao_runs_score:           d_per_t[q] = mean over the runs of (B - best_r(t)) / (B - f_opt), best_r(t) = best-so-far at
+ *                             the last recorded generation whose unique-evaluation count is <= t (generation 0 if none;
+ *                             the worst objective if nothing valid was evaluated); d_score[0] = their mean over q.
+ *                             d_scratch: S * n_runs doubles.  Bit-identical to the oracle (same fp64 operation order). */
+int cao_space_sort_objective(const cao_space* s, float* d_sorted, void* d_scratch, void* stream);
+int cao_space_baseline(const cao_space* s, const float* d_sorted, const uint64_t* d_t, uint32_t S, double* d_B, void* stream);
+int cao_runs_score(const cao_runs* r, const float* d_sorted, const uint64_t* d_t, const double* d_B, uint32_t S,
+                   double* d_per_t, double* d_score, void* d_scratch, void* stream);
 /* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
 uint64_t cao_launch_count(void);
 

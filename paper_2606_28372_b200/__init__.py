@@ -5,5 +5,5 @@ It only marshals arguments: PyTorch provides device memory and streams, every st
 (enumeration, operators, snap, validity, repair, lookup, selection) runs in the library's kernels.
 There is no CPU fallback: importing :mod:`.api` objects without the built library raises.
 """
-from .api import (Space, Runs, HParams, ALGOS, CaoError, lib, launch_count, test_philox, test_exp_neg, test_curand_philox, int_peak,
+from .api import (Space, Runs, HParams, Variant, ALGOS, CaoError, lib, launch_count, test_philox, test_exp_neg, test_curand_philox, int_peak,
                   profile_enable, profile_read)  # noqa: F401

@@ -35,6 +35,23 @@ class HParams(C.Structure):
         return cls(0.7, 0.6, 0.5, 3.0, 0.5, 1.0, 1.0, 0.2, 5, 3)
 
 
+class Variant(C.Structure):
+    """cao_variant: the SURVEY 8(f) switches (include/cao.h); the default is the north_star path."""
+    _fields_ = [("constraint_aware", C.c_int32), ("repair_mode", C.c_int32), ("de_mutation", C.c_int32),
+                ("de_crossover", C.c_int32), ("ga_crossover", C.c_int32), ("init_lhs", C.c_int32), ("penalty", C.c_float),
+                ("reserved", C.c_int32)]
+    DE_MUTATION = {"best1": 0, "rand1": 1, "currenttobest1": 2, "randtobest1": 3, "best2": 4, "rand2": 5}
+    DE_CROSSOVER = {"bin": 0, "exp": 1}
+    GA_CROSSOVER = {"single_point": 0, "two_point": 1, "uniform": 2, "disruptive_uniform": 3}
+
+    @classmethod
+    def make(cls, aware=True, repair_mode=0, de_mutation="best1", de_crossover="bin", ga_crossover="single_point",
+             init_lhs=False, penalty=1e20):
+        g = lambda table, v: table[v] if isinstance(v, str) else int(v)
+        return cls(int(bool(aware)), int(repair_mode), g(cls.DE_MUTATION, de_mutation), g(cls.DE_CROSSOVER, de_crossover),
+                   g(cls.GA_CROSSOVER, ga_crossover), int(bool(init_lhs)), float(penalty), 0)
+
+
 vp, u64, u32, i32 = C.c_void_p, C.c_uint64, C.c_uint32, C.c_int32
 pu64, pi32, pvp = C.POINTER(C.c_uint64), C.POINTER(C.c_int32), C.POINTER(C.c_void_p)
 
@@ -62,6 +79,14 @@ SIGNATURES = {
     "cao_space_set_objective": (C.c_int, [vp, vp]),
     "cao_runs_workspace_bytes": (C.c_int, [vp, i32, i32, u32, u32, pu64]),
     "cao_runs_create": (C.c_int, [vp, i32, C.POINTER(HParams), u32, u32, i32, u32, u32, u64, vp, vp, pvp]),
+    "cao_runs_workspace_bytes_ex": (C.c_int, [vp, i32, C.POINTER(Variant), i32, u32, u32, pu64]),
+    "cao_runs_create_ex": (C.c_int, [vp, i32, C.POINTER(HParams), C.POINTER(Variant), u32, u32, i32, u32, u32, u64, vp, vp, pvp]),
+    "cao_runs_debug_rule": (C.c_int, [vp, pvp]),
+    "cao_space_repair_mode_scratch_bytes": (C.c_int, [vp, u64, pu64]),
+    "cao_space_repair_mode": (C.c_int, [vp, i32, vp, vp, vp, u64, vp, vp, vp, vp]),
+    "cao_space_sort_objective": (C.c_int, [vp, vp, vp, vp]),
+    "cao_space_baseline": (C.c_int, [vp, vp, vp, u32, vp, vp]),
+    "cao_runs_score": (C.c_int, [vp, vp, vp, vp, u32, vp, vp, vp, vp]),
     "cao_runs_destroy": (None, [vp]),
     "cao_runs_set_mode": (C.c_int, [vp, i32]),
     "cao_runs_mode": (C.c_int, [vp, pi32]),
@@ -292,6 +317,44 @@ class Space:
         self._last_scratch = scratch
         return rank, key
 
+    def repair_mode(self, mode, rows, x=None, w=None):
+        """NEXT-1 standalone: mode 'index' (L270) | 'alg2' (x: continuous positions) | 'alg3' (w: 32-bit draws)
+        -> (rank int32 tensor, 0xFFFFFFFF = unrepaired; rule uint8 tensor)."""
+        m = {"index": 1, "alg2": 2, "alg3": 3}[mode]
+        r = self.pack_rows(rows)
+        c = r.shape[0]
+        sb = u64()
+        _check(lib().cao_space_repair_mode_scratch_bytes(self._h, c, C.byref(sb)))
+        scratch = _dev_bytes(sb.value, self.device)
+        rank = torch.empty(c, dtype=torch.int32, device=self.device)
+        rule = torch.empty(c, dtype=torch.uint8, device=self.device)
+        xx = torch.as_tensor(np.ascontiguousarray(x, dtype=np.float32)).to(self.device).contiguous() if x is not None else None
+        ww = torch.as_tensor(np.ascontiguousarray(w, dtype=np.uint32).view(np.int32)).to(self.device).contiguous() if w is not None else None
+        _check(lib().cao_space_repair_mode(self._h, m, r.data_ptr(), xx.data_ptr() if xx is not None else None,
+                                           ww.data_ptr() if ww is not None else None, c, rank.data_ptr(), rule.data_ptr(),
+                                           scratch.data_ptr(), _stream()))
+        self._last_scratch = (scratch, xx, ww, r)
+        return rank, rule
+
+    # -- NEXT-4
+    def sorted_objective(self) -> torch.Tensor:
+        V = self.V
+        n2 = 1
+        while n2 < V:
+            n2 <<= 1
+        out = torch.empty(V, dtype=torch.float32, device=self.device)
+        scratch = _dev_bytes(n2 * 4, self.device)
+        _check(lib().cao_space_sort_objective(self._h, out.data_ptr(), scratch.data_ptr(), _stream()))
+        self._sort_scratch = scratch
+        return out
+
+    def baseline(self, sorted_obj: torch.Tensor, t) -> torch.Tensor:
+        tt = torch.as_tensor(np.ascontiguousarray(t, dtype=np.int64)).to(self.device)
+        B = torch.empty(tt.numel(), dtype=torch.float64, device=self.device)
+        _check(lib().cao_space_baseline(self._h, sorted_obj.data_ptr(), tt.data_ptr(), tt.numel(), B.data_ptr(), _stream()))
+        self._base_keep = tt
+        return B
+
     def set_objective(self, obj):
         t = obj if isinstance(obj, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(obj, dtype=np.float32))
         t = t.to(self.device, dtype=torch.float32).contiguous()
@@ -310,18 +373,20 @@ class Runs:
     """n_runs independent simulated tuning runs of one algorithm; creation executes generation 0 (S2)."""
 
     def __init__(self, space: Space, algo, n_runs, pop, budget=0, max_gens=100, seed=0, first_run=0, hparams=None,
-                 mode=None):
+                 mode=None, variant: Variant | None = None):
         self.space, self.R, self.P, self.n = space, int(n_runs), int(pop), space.n
         self.algo = ALGOS[algo] if isinstance(algo, str) else int(algo)
         self.hp = hparams or HParams.default()
+        self.variant = variant
+        vref = C.byref(variant) if variant is not None else None
         self.max_gens = int(max_gens)
         wb = u64()
-        _check(lib().cao_runs_workspace_bytes(space._h, self.algo, self.P, self.R, self.max_gens, C.byref(wb)))
+        _check(lib().cao_runs_workspace_bytes_ex(space._h, self.algo, vref, self.P, self.R, self.max_gens, C.byref(wb)))
         self.workspace_bytes = wb.value
         self._ws = _dev_bytes(wb.value, space.device)
         h = C.c_void_p()
-        _check(lib().cao_runs_create(space._h, self.algo, C.byref(self.hp), self.R, int(first_run), self.P, int(budget),
-                                     self.max_gens, int(seed), self._ws.data_ptr(), _stream(), C.byref(h)))
+        _check(lib().cao_runs_create_ex(space._h, self.algo, C.byref(self.hp), vref, self.R, int(first_run), self.P, int(budget),
+                                        self.max_gens, int(seed), self._ws.data_ptr(), _stream(), C.byref(h)))
         self._h = h
         if mode is not None:
             self.set_mode(mode)
@@ -374,6 +439,26 @@ class Runs:
                     f=v(4, R * P * 4, torch.float32, (R, P)), accept=v(5, R * P, torch.uint8, (R, P)),
                     active=v(6, R, torch.uint8, (R,)))
 
+    def rule_tap(self) -> torch.Tensor:
+        """NEXT-1: (R, P) uint8 neighbour rule of the last generation's repairs (runs with a non-default variant)."""
+        p = C.c_void_p()
+        _check(lib().cao_runs_debug_rule(self._h, C.byref(p)))
+        return _view(self._ws, p.value, self.R * self.P, torch.uint8, (self.R, self.P))
+
+    def score(self, sorted_obj: torch.Tensor, t, B: torch.Tensor | None = None):
+        """NEXT-4 (Eq.2): (score, per-sampling-point means) as device float64 tensors."""
+        dev = self.space.device
+        tt = torch.as_tensor(np.ascontiguousarray(t, dtype=np.int64)).to(dev)
+        if B is None:
+            B = self.space.baseline(sorted_obj, t)
+        per = torch.empty(tt.numel(), dtype=torch.float64, device=dev)
+        sc = torch.empty(1, dtype=torch.float64, device=dev)
+        scratch = _dev_bytes(tt.numel() * self.R * 8, dev)
+        _check(lib().cao_runs_score(self._h, sorted_obj.data_ptr(), tt.data_ptr(), B.data_ptr(), tt.numel(), per.data_ptr(),
+                                    sc.data_ptr(), scratch.data_ptr(), _stream()))
+        self._score_keep = (tt, scratch, B)
+        return sc, per
+
     def _state(self, which, dtype, shape):
         p, b = C.c_void_p(), u64()
         _check(lib().cao_runs_debug_state(self._h, which, C.byref(p), C.byref(b)))
@@ -402,7 +487,7 @@ class Runs:
         """cao_runs_stats: the sixteen statistics words as a dict."""
         a = (C.c_uint64 * 32)()
         _check(lib().cao_runs_stats(self._h, _stream(), a))
-        names = ["n_repaired", "n_scanned", "n_evaluated", "n_probe2", "n_probe3", "n_memo", "n_rcache", "r7",
+        names = ["n_repaired", "n_scanned", "n_evaluated", "n_probe2", "n_probe3", "n_memo", "n_rcache", "n_penalised",
                  "cyc_op", "cyc_tail", "cyc_probe2", "cyc_probe3", "cyc_scan", "cyc_finish", "cyc_max_run", "cyc_max_scan"]
         out = {k: int(v) for k, v in zip(names, a)}
         out["ham_hist"] = [int(a[16 + h]) for h in range(9)]

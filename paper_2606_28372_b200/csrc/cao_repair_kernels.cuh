@@ -221,7 +221,9 @@ __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMe
 
 // WU = words of a row that carry indices (ceil(n/4)); row stride in HBM = 4 or 8 words.
 // SMALL: every index < 128, so a byte of c^v is non-zero iff adding 0x7f carries into its bit 7.
-template <int WU, bool SMALL>
+// KM: key layout.  0 = north_star's (Hamming << 13 + sum|didx|) << 32 | rank; 1 = NEXT-1 index distance (L215, L270):
+// sum|didx| << 32 | rank (the Hamming count is not computed).
+template <int WU, bool SMALL, int KM = 0>
 __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
                                                   const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
                                                   unsigned long long* key) {
@@ -262,13 +264,15 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
 #pragma unroll
                 for (int k = 0; k < WU; ++k) {
                     sad = sad4_acc(c[k], v[k], sad);
-                    uint32_t x = c[k] ^ v[k];
-                    uint32_t t = SMALL ? (x + 0x7f7f7f7fu) : (((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x);
-                    if ((k & 3) == 0 && k) { ham += __popc(hb); hb = 0; }
-                    hb |= (t & 0x80808080u) >> (k & 3);
+                    if (KM == 0) {
+                        uint32_t x = c[k] ^ v[k];
+                        uint32_t t = SMALL ? (x + 0x7f7f7f7fu) : (((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x);
+                        if ((k & 3) == 0 && k) { ham += __popc(hb); hb = 0; }
+                        hb |= (t & 0x80808080u) >> (k & 3);
+                    }
                 }
                 ham += __popc(hb);
-                uint32_t k32 = (ham << 13) + sad;
+                uint32_t k32 = KM == 1 ? sad : (ham << 13) + sad;
                 if (k32 < bestk) { bestk = k32; bestr = r0 + r; }         // ascending rank: ties keep the smallest L
             }
         }

@@ -4,6 +4,7 @@
 #include <cstring>
 #include <curand_kernel.h>
 #include "cao_runs_kernels.cuh"
+#include "cao_var_kernels.cuh"
 
 // Fused generation kernel, one object per algorithm (cao_gen_algo.cu).
 struct GenLayout;
@@ -23,6 +24,7 @@ struct cao_runs {
     uint32_t gen = 0;
     unsigned block = 32;
     int mode = 1;                      // 1 = fused persistent k_gen, 0 = phased (k_op / k_probe23 / k_scan / k_finish)
+    bool var_on = false;               // a non-default cao_variant: phased pipeline only
     GenLayout lay{};                   // shared-memory slice of one group of the fused kernel
     unsigned gen_threads = 256, gen_grid = 0;
     size_t gen_smem = 0;
@@ -33,26 +35,52 @@ struct cao_runs {
 
 // ---------------------------------------------------------------------------------------------
 // in_domain: every candidate byte is a legal index (< m_d <= 128 when M <= 128), which the SMALL byte trick needs.
+// index_distance: the NEXT-1 key (sum|didx|, L) of L215 / L270 instead of north_star's (Hamming, sum|didx|, L).
 template <int WU>
 static void launch_scan_wu(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
-                           unsigned long long* key, bool in_domain, cudaStream_t st) {
-    if (sm.M <= 128 && in_domain) k_scan<WU, true><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
+                           unsigned long long* key, bool in_domain, bool index_distance, cudaStream_t st) {
+    if (index_distance) k_scan<WU, false, 1><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
+    else if (sm.M <= 128 && in_domain) k_scan<WU, true><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
     else k_scan<WU, false><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, key);
 }
-static int launch_scan(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
-                       unsigned long long* key, bool in_domain, cudaStream_t st) {
-    ProfScope ps(PK_SCAN, st);
-    switch ((sm.n + 3) / 4) {
-        case 1: launch_scan_wu<1>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        case 2: launch_scan_wu<2>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        case 3: launch_scan_wu<3>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        case 4: launch_scan_wu<4>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        case 5: launch_scan_wu<5>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        case 6: launch_scan_wu<6>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        case 7: launch_scan_wu<7>(sm, cand, wl, wl_count, key, in_domain, st); break;
-        default: launch_scan_wu<8>(sm, cand, wl, wl_count, key, in_domain, st); break;
+#define DISPATCH_WU(n_dims, CALL)                                                   \
+    switch (((n_dims) + 3) / 4) {                                                   \
+        case 1: { CALL(1); } break; case 2: { CALL(2); } break; case 3: { CALL(3); } break; case 4: { CALL(4); } break; \
+        case 5: { CALL(5); } break; case 6: { CALL(6); } break; case 7: { CALL(7); } break; default: { CALL(8); } break; \
     }
+static int launch_scan(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
+                       unsigned long long* key, bool in_domain, cudaStream_t st, bool index_distance = false) {
+    ProfScope ps(PK_SCAN, st);
+#define CALL_SCAN(W) launch_scan_wu<W>(sm, cand, wl, wl_count, key, in_domain, index_distance, st)
+    DISPATCH_WU(sm.n, CALL_SCAN);
     CAO_LAUNCHED("k_scan");
+    return CAO_OK;
+}
+// NEXT-1 neighbour-rule scan (Alg.2: kind 0, per-rule nearest member; Alg.3: kind 1, per-rule member counts).
+static int launch_scan_nb(const SpaceMeta& sm, int kind, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count,
+                          const uint8_t* present, const XAddr& xa, unsigned long long* key3, uint32_t* cnt3, cudaStream_t st) {
+    ProfScope ps(PK_SCAN, st);
+#define CALL_NB(W) if (kind == 0) k_scan_nb<W, 0><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, present, xa, key3, cnt3); \
+                   else k_scan_nb<W, 1><<<SCAN_GRID, SCAN_TC, 0, st>>>(sm, cand, wl, wl_count, present, xa, key3, cnt3)
+    DISPATCH_WU(sm.n, CALL_NB);
+    CAO_LAUNCHED("k_scan_nb");
+    return CAO_OK;
+}
+static int launch_pick_nb(const SpaceMeta& sm, const uint8_t* cand, const uint32_t* wl, const uint32_t* wl_count, const uint8_t* present,
+                          const uint32_t* cnt3, const uint32_t* w_arr, uint64_t seed, uint32_t first_run, uint32_t P, uint32_t gen,
+                          unsigned long long* key, uint8_t* rule, cudaStream_t st) {
+    ProfScope ps(PK_SCAN, st);
+#define CALL_PICK(W) k_pick_nb<W><<<148 * 4, 256, 0, st>>>(sm, cand, wl, wl_count, present, cnt3, w_arr, seed, first_run, P, gen, key, rule)
+    DISPATCH_WU(sm.n, CALL_PICK);
+    CAO_LAUNCHED("k_pick_nb");
+    return CAO_OK;
+}
+static int launch_present(const SpaceMeta& sm, uint8_t* present, cudaStream_t st) {
+    CAO_CUDA(cudaMemsetAsync(present, 0, (size_t)CAO_MAX_DIMS * 256, st));
+    const unsigned grid = (unsigned)((sm.V + 255) / 256);
+    if (sm.rowB == 16) k_present<4><<<grid, 256, 0, st>>>(sm, present);
+    else k_present<8><<<grid, 256, 0, st>>>(sm, present);
+    CAO_LAUNCHED("k_present");
     return CAO_OK;
 }
 
@@ -194,11 +222,18 @@ static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P) {
 struct RunsLayout {
     uint64_t cand, key, valid, rep_rank, eval_rank, tap_f, accept, active, idx, rank, f, x, v, pb, pbf, dedup,
         uniq, gens_done, stagn, best_rank, best_f, traj, wl, wl2, wl_count, counters, rcache, ticket, total;
+    uint64_t rule, key3, cnt3, present;   // SURVEY 8(f) variants only
     uint64_t zero_from, zero_bytes;       // region that must start as zero: dedup .. stagn
     uint32_t dedup_words;
 };
 
-static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_t R, uint64_t max_gens) {
+static const cao_variant CAO_VARIANT_DEFAULT = {1, 0, 0, 0, 0, 0, 1e20f, 0};
+static bool variant_is_default(const cao_variant& v) {
+    return v.constraint_aware == 1 && v.repair_mode == 0 && v.de_mutation == 0 && v.de_crossover == 0 && v.ga_crossover == 0 &&
+           v.init_lhs == 0;
+}
+static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_t R, uint64_t max_gens,
+                              const cao_variant& var = CAO_VARIANT_DEFAULT) {
     RunsLayout L{};
     const uint64_t RP = R * P, rowB = sm.rowB, n = sm.n;
     uint64_t off = 0;
@@ -221,6 +256,13 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
     L.wl = take(RP * 4);
     L.wl2 = take(RP * 4);
     L.rcache = take(R * CAO_RCACHE * 16);
+    if (!variant_is_default(var)) {
+        const bool paper = var.constraint_aware && var.repair_mode == 1;
+        L.rule = take(RP);
+        L.key3 = take(paper && cont ? RP * 24 : 0);
+        L.cnt3 = take(paper && algo == CAO_GA ? RP * 12 : 0);
+        L.present = take(paper ? (uint64_t)CAO_MAX_DIMS * 256 : 0);
+    }
     L.total = off;
     return L;
 }
@@ -240,29 +282,61 @@ static int check_runs_args(const cao_space* s, int32_t algo, int32_t pop, uint32
     return CAO_OK;
 }
 
-int cao_runs_workspace_bytes(const cao_space* s, int32_t algo, int32_t pop, uint32_t n_runs, uint32_t max_gens, uint64_t* bytes) {
+static int check_variant(int32_t algo, int32_t pop, const cao_variant& v) {
+    if (v.constraint_aware < 0 || v.constraint_aware > 1 || v.repair_mode < 0 || v.repair_mode > 1 || v.de_mutation < 0 ||
+        v.de_mutation > 5 || v.de_crossover < 0 || v.de_crossover > 1 || v.ga_crossover < 0 || v.ga_crossover > 3 ||
+        v.init_lhs < 0 || v.init_lhs > 1)
+        return cao_fail(CAO_E_INVALID_ARG, "runs: unknown cao_variant switch value");
+    static const int donors[6] = {2, 3, 2, 3, 4, 5};
+    if (algo == CAO_DE && pop < donors[v.de_mutation] + 1) return cao_fail(CAO_E_INVALID_ARG, "runs: DE population smaller than donors + 1");
+    if (v.init_lhs && (algo != CAO_DE || !v.constraint_aware))
+        return cao_fail(CAO_E_INVALID_ARG, "runs: init_lhs is DE's constraint-aware initial sample (L223)");
+    if (!(v.penalty > 0.0f) || !(v.penalty < 3.0e38f)) return cao_fail(CAO_E_INVALID_ARG, "runs: penalty must be > 0 and finite");
+    return CAO_OK;
+}
+
+int cao_runs_workspace_bytes_ex(const cao_space* s, int32_t algo, const cao_variant* var, int32_t pop, uint32_t n_runs,
+                                uint32_t max_gens, uint64_t* bytes) {
     if (!bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_workspace_bytes: NULL argument");
     int rc = check_runs_args(s, algo, pop, n_runs, max_gens);
     if (rc) return rc;
-    *bytes = runs_layout(s->meta, algo, (uint64_t)pop, n_runs, max_gens).total;
+    const cao_variant v = var ? *var : CAO_VARIANT_DEFAULT;
+    if ((rc = check_variant(algo, pop, v))) return rc;
+    *bytes = runs_layout(s->meta, algo, (uint64_t)pop, n_runs, max_gens, v).total;
     return CAO_OK;
+}
+int cao_runs_workspace_bytes(const cao_space* s, int32_t algo, int32_t pop, uint32_t n_runs, uint32_t max_gens, uint64_t* bytes) {
+    return cao_runs_workspace_bytes_ex(s, algo, nullptr, pop, n_runs, max_gens, bytes);
 }
 
 int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uint32_t n_runs, uint32_t first_run, int32_t pop,
                     uint32_t budget_unique, uint32_t max_gens, uint64_t seed, void* d_workspace, void* stream, cao_runs** out) {
+    return cao_runs_create_ex(s, algo, hp, nullptr, n_runs, first_run, pop, budget_unique, max_gens, seed, d_workspace, stream, out);
+}
+
+int cao_runs_create_ex(const cao_space* s, int32_t algo, const cao_hparams* hp, const cao_variant* var, uint32_t n_runs,
+                       uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens, uint64_t seed, void* d_workspace,
+                       void* stream, cao_runs** out) {
     if (!out || !hp) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_create: NULL argument");
     int rc = check_runs_args(s, algo, pop, n_runs, max_gens);
     if (rc) return rc;
+    const cao_variant vr = var ? *var : CAO_VARIANT_DEFAULT;
+    if ((rc = check_variant(algo, pop, vr))) return rc;
     if (!s->meta.obj) return cao_fail(CAO_E_STATE, "cao_runs_create: call cao_space_set_objective first");
     if (algo == CAO_GA && (hp->ga_beta_b < 1 || hp->ga_beta_b > 16 || hp->ga_mutation_chance < 1))
         return cao_fail(CAO_E_INVALID_ARG, "cao_runs_create: ga_beta_b must be 1..16 and ga_mutation_chance >= 1");
     if (!d_workspace || ((uintptr_t)d_workspace & 255)) return cao_fail(CAO_E_WORKSPACE, "cao_runs_create: workspace must be non-NULL and 256-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
-    const RunsLayout L = runs_layout(s->meta, algo, (uint64_t)pop, n_runs, max_gens);
+    const RunsLayout L = runs_layout(s->meta, algo, (uint64_t)pop, n_runs, max_gens, vr);
     uint8_t* w = (uint8_t*)d_workspace;
     cao_runs* r = new cao_runs();
     r->s = s; r->sm = s->meta;
     RunsMeta& m = r->rm;
+    m.var = vr; r->var_on = !variant_is_default(vr); m.var_on = r->var_on ? 1 : 0;
+    m.rule = nullptr; m.key3 = nullptr; m.cnt3 = nullptr; m.present = nullptr;
+    if (r->var_on) {
+        m.rule = w + L.rule; m.key3 = (unsigned long long*)(w + L.key3); m.cnt3 = (uint32_t*)(w + L.cnt3); m.present = w + L.present;
+    }
     m.R = n_runs; m.first_run = first_run; m.P = (uint32_t)pop; m.budget = budget_unique; m.max_gens = max_gens;
     m.dedup_words = L.dedup_words; m.algo = algo; m.probe_levels = s->probe.levels; m.seed = seed; m.hp = *hp;
     m.cand = w + L.cand; m.key = (unsigned long long*)(w + L.key); m.valid = w + L.valid;
@@ -294,10 +368,11 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
         r->mode = p_scan > 0.01 ? 0 : 1;
     }
     if (r->gen_smem > 227 * 1024) r->mode = 0;                         // the population does not fit one SM: phased only
+    if (r->var_on) r->mode = 0;                                         // SURVEY 8(f) variants run through the phased pipeline
     const size_t P = (size_t)pop, n = (size_t)s->meta.n;
     r->smem_init = P * 4;
-    r->smem_op = algo == CAO_GA ? P * 12 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
-    r->smem_fin = algo == CAO_DE ? P * 8 : 0;
+    r->smem_op = algo == CAO_GA ? P * 16 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
+    r->smem_fin = algo == CAO_DE ? P * 16 : 0;
     int rc2 = CAO_OK;
     do {
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.zero_from, 0, L.zero_bytes, st), "memset state"))) break;
@@ -305,6 +380,20 @@ int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uin
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.cand, 0, L.idx - L.cand, st), "memset taps"))) break;
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.key, 0xFF, RP * 8, st), "memset keys"))) break;   // no key yet
         if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.rcache, 0xFF, (uint64_t)n_runs * CAO_RCACHE * 16, st), "memset repair cache"))) break;
+        if (r->var_on) {
+            if ((rc2 = cao_cuda_check(cudaMemsetAsync(w + L.rule, 0xFF, RP, st), "memset rule tap"))) break;
+            if (vr.constraint_aware && vr.repair_mode == 1 && (rc2 = launch_present(r->sm, w + L.present, st))) break;
+        }
+        if (vr.init_lhs) {                                              // A35: LHS points -> ordinary repair pipeline -> k_init reads the ranks
+            { ProfScope ps(PK_INIT, st);
+              if (s->meta.rowB == 16) k_lhs_points<4><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm);
+              else k_lhs_points<8><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm); }
+            ++g_cao_launches;
+            if ((rc2 = cao_cuda_check(cudaGetLastError(), "k_lhs_points"))) break;
+            const int levels = s->probe.levels;
+            if (levels >= 2 && (rc2 = launch_probe23(s, r->sm, m.cand, m.wl, m.wl_count, m.key, m.wl2, m.wl2_count, nullptr, levels, st))) break;
+            if ((rc2 = launch_scan(r->sm, m.cand, levels >= 2 ? m.wl2 : m.wl, levels >= 2 ? m.wl2_count : m.wl_count, m.key, true, st))) break;
+        }
 #define CALL_INIT(A, W) \
         if (r->smem_op > 48 * 1024) cudaFuncSetAttribute(k_op<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
         k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
@@ -365,13 +454,29 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
         CAO_LAUNCHED("k_op");
         int rc = CAO_OK;
         const int levels = r->s->probe.levels;
-        if (levels >= 2) {
-            rc = launch_probe23(r->s, r->sm, r->rm.cand, r->rm.wl, r->rm.wl_count, r->rm.key, r->rm.wl2, r->rm.wl2_count,
-                                &r->rm.counters[1], levels, st);
+        const cao_variant& vr = r->rm.var;
+        if (!vr.constraint_aware) {
+            // NEXT-2: nothing is repaired (L272, L284)
+        } else if (vr.repair_mode == 1) {                               // NEXT-1: the paper's own repairs, all by table scan (wl2)
+            const RunsMeta& m = r->rm;
+            if (algo == CAO_DE) rc = launch_scan(r->sm, m.cand, m.wl2, m.wl2_count, m.key, true, st, true);
+            else if (algo == CAO_GA) {
+                rc = launch_scan_nb(r->sm, 1, m.cand, m.wl2, m.wl2_count, m.present, XAddr{nullptr, 1, 0, 0, 0}, m.key3, m.cnt3, st);
+                if (!rc) rc = launch_pick_nb(r->sm, m.cand, m.wl2, m.wl2_count, m.present, m.cnt3, nullptr, m.seed, m.first_run, m.P, g, m.key, m.rule, st);
+            } else {
+                const XAddr xa{m.x, m.P, (uint64_t)r->sm.n * m.P, m.P, 1};
+                rc = launch_scan_nb(r->sm, 0, m.cand, m.wl2, m.wl2_count, m.present, xa, m.key3, m.cnt3, st);
+            }
+            if (rc) return rc;
+        } else {
+            if (levels >= 2) {
+                rc = launch_probe23(r->s, r->sm, r->rm.cand, r->rm.wl, r->rm.wl_count, r->rm.key, r->rm.wl2, r->rm.wl2_count,
+                                    &r->rm.counters[1], levels, st);
+                if (rc) return rc;
+            }
+            rc = launch_scan(r->sm, r->rm.cand, levels >= 2 ? r->rm.wl2 : r->rm.wl, levels >= 2 ? r->rm.wl2_count : r->rm.wl_count, r->rm.key, true, st);
             if (rc) return rc;
         }
-        rc = launch_scan(r->sm, r->rm.cand, levels >= 2 ? r->rm.wl2 : r->rm.wl, levels >= 2 ? r->rm.wl2_count : r->rm.wl_count, r->rm.key, true, st);
-        if (rc) return rc;
 #define CALL_FIN(A, W) k_finish<A, W><<<r->rm.R, r->block, r->smem_fin, st>>>(r->sm, r->rm, g)
         { ProfScope ps(PK_FINISH, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_FIN); }
         CAO_LAUNCHED("k_finish");
@@ -388,6 +493,8 @@ int cao_runs_mode(const cao_runs* r, int32_t* mode) {
 
 int cao_runs_set_mode(cao_runs* r, int32_t mode) {
     if (!r || (mode != 0 && mode != 1)) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_set_mode: mode must be 0 (phased) or 1 (fused)");
+    if (mode == 1 && r->var_on)
+        return cao_fail(CAO_E_INVALID_ARG, "cao_runs_set_mode: runs with a non-default cao_variant use the phased pipeline only");
     if (mode == 1 && r->gen_smem > 227 * 1024)
         return cao_fail(CAO_E_TOO_LARGE, "cao_runs_set_mode: the population state does not fit the shared memory of one SM (fused mode)");
     r->mode = mode;
@@ -425,6 +532,13 @@ int cao_runs_debug_last(const cao_runs* r, const uint8_t** d_postsnap_rows, cons
     return CAO_OK;
 }
 
+int cao_runs_debug_rule(const cao_runs* r, const uint8_t** d_rule) {
+    if (!r || !d_rule) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_debug_rule: NULL argument");
+    if (!r->var_on) return cao_fail(CAO_E_STATE, "cao_runs_debug_rule: only runs with a non-default cao_variant record the rule");
+    *d_rule = r->rm.rule;
+    return CAO_OK;
+}
+
 int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, uint64_t* bytes) {
     if (!r || !d_ptr || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_debug_state: NULL argument");
     const int a = r->rm.algo;
@@ -457,6 +571,107 @@ int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out32) {
     if (!r || !h_out32) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_stats: NULL argument");
     CAO_CUDA(cudaMemcpyAsync(h_out32, r->rm.counters, 32 * 8, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CAO_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    return CAO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-1 standalone.  Scratch: key | key3 | cnt3 | wl | wl_count | rule | present | clean rows.
+struct ModeScratch { uint64_t key, key3, cnt3, wl, wl_count, rule, present, clean, total; };
+static ModeScratch mode_scratch(const cao_space* s, uint64_t count) {
+    ModeScratch L{};
+    const uint64_t c = std::max<uint64_t>(1, count);
+    uint64_t off = 0;
+    auto take = [&](uint64_t bytes) { uint64_t o = off; off = align256(off + bytes); return o; };
+    L.key = take(c * 8); L.key3 = take(c * 24); L.cnt3 = take(c * 12); L.wl = take(c * 4); L.wl_count = take(256);
+    L.rule = take(c); L.present = take((uint64_t)CAO_MAX_DIMS * 256); L.clean = take(c * (uint64_t)s->meta.rowB);
+    L.total = off;
+    return L;
+}
+int cao_space_repair_mode_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes) {
+    if (!s || !bytes) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_mode_scratch_bytes: NULL argument");
+    *bytes = mode_scratch(s, count).total;
+    return CAO_OK;
+}
+int cao_space_repair_mode(const cao_space* s, int32_t mode, const uint8_t* d_idx_rows, const float* d_x, const uint32_t* d_w,
+                          uint64_t count, uint32_t* d_rank_out, uint8_t* d_rule_out, void* d_scratch, void* stream) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_mode: NULL space");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_repair_mode: space not built");
+    if (mode < 1 || mode > 3) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_mode: mode must be 1 (index distance), 2 (Alg.2) or 3 (Alg.3)");
+    if (count == 0) return CAO_OK;
+    if (!d_idx_rows || !d_rank_out || (mode == 2 && !d_x) || (mode == 3 && !d_w))
+        return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_mode: NULL argument");
+    if (count >= (1ull << 32)) return cao_fail(CAO_E_TOO_LARGE, "cao_space_repair_mode: count >= 2^32");
+    if (s->meta.V == 0) return cao_fail(CAO_E_EMPTY_SPACE, "cao_space_repair_mode: the space has no valid configuration");
+    if (!d_scratch || ((uintptr_t)d_scratch & 255) || ((uintptr_t)d_idx_rows & 15))
+        return cao_fail(CAO_E_WORKSPACE, "cao_space_repair_mode: scratch must be 256-byte aligned, rows 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const ModeScratch L = mode_scratch(s, count);
+    uint8_t* sc = (uint8_t*)d_scratch;
+    unsigned long long* key = (unsigned long long*)(sc + L.key); unsigned long long* key3 = (unsigned long long*)(sc + L.key3);
+    uint32_t* cnt3 = (uint32_t*)(sc + L.cnt3); uint32_t* wl = (uint32_t*)(sc + L.wl); uint32_t* wl_count = (uint32_t*)(sc + L.wl_count);
+    uint8_t* rule = sc + L.rule; uint8_t* present = sc + L.present; uint8_t* clean = sc + L.clean;
+    CAO_CUDA(cudaMemsetAsync(wl_count, 0, 8, st));
+    int rc = launch_present(s->meta, present, st);
+    if (rc) return rc;
+    const unsigned grid = (unsigned)((count + 255) / 256);
+    {
+        ProfScope ps(PK_QUERY, st);
+        if (s->meta.rowB == 16) k_mode_probe<4><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, clean, count, key, key3, cnt3, wl, wl_count, rule);
+        else k_mode_probe<8><<<grid, 256, 0, st>>>(s->meta, d_idx_rows, clean, count, key, key3, cnt3, wl, wl_count, rule);
+    }
+    CAO_LAUNCHED("k_mode_probe");
+    if (mode == 1) rc = launch_scan(s->meta, clean, wl, wl_count, key, true, st, true);
+    else if (mode == 2) rc = launch_scan_nb(s->meta, 0, clean, wl, wl_count, present, XAddr{d_x, 1, (uint64_t)s->meta.n, 1, 0}, key3, cnt3, st);
+    else {
+        rc = launch_scan_nb(s->meta, 1, clean, wl, wl_count, present, XAddr{nullptr, 1, 0, 0, 0}, key3, cnt3, st);
+        if (!rc) rc = launch_pick_nb(s->meta, clean, wl, wl_count, present, cnt3, d_w, 0, 0, 1, 0, key, rule, st);
+    }
+    if (rc) return rc;
+    k_mode_finish<<<grid, 256, 0, st>>>(mode, key, key3, count, d_rank_out, rule, d_rule_out);
+    CAO_LAUNCHED("k_mode_finish");
+    return CAO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-4
+static uint32_t next_pow2(uint64_t v) { uint32_t p = 1; while (p < v) p <<= 1; return p; }
+int cao_space_sort_objective(const cao_space* s, float* d_sorted, void* d_scratch, void* stream) {
+    if (!s || !d_sorted || !d_scratch) return cao_fail(CAO_E_INVALID_ARG, "cao_space_sort_objective: NULL argument");
+    if (!s->filled || !s->meta.obj) return cao_fail(CAO_E_STATE, "cao_space_sort_objective: build the space and set the objective first");
+    if (s->meta.V == 0) return cao_fail(CAO_E_EMPTY_SPACE, "cao_space_sort_objective: the space has no valid configuration");
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint32_t V = s->meta.V, n2 = next_pow2(V);
+    uint32_t* buf = (uint32_t*)d_scratch;
+    const unsigned grid = (n2 + 255) / 256;
+    k_sort_load<<<grid, 256, 0, st>>>(s->meta.obj, V, buf, n2);
+    CAO_LAUNCHED("k_sort_load");
+    for (uint32_t k = 2; k <= n2; k <<= 1)
+        for (uint32_t j = k >> 1; j > 0; j >>= 1) { k_bitonic_step<<<grid, 256, 0, st>>>(buf, n2, j, k); ++g_cao_launches; }
+    CAO_CUDA(cudaGetLastError());
+    k_sort_store<<<(V + 255) / 256, 256, 0, st>>>(buf, V, d_sorted);
+    CAO_LAUNCHED("k_sort_store");
+    return CAO_OK;
+}
+int cao_space_baseline(const cao_space* s, const float* d_sorted, const uint64_t* d_t, uint32_t S, double* d_B, void* stream) {
+    if (!s || !d_sorted || !d_t || !d_B) return cao_fail(CAO_E_INVALID_ARG, "cao_space_baseline: NULL argument");
+    if (!s->filled || s->meta.V == 0) return cao_fail(CAO_E_STATE, "cao_space_baseline: space not built or empty");
+    if (S == 0) return CAO_OK;
+    k_baseline<<<(S + 31) / 32, 32, 0, (cudaStream_t)stream>>>(d_sorted, s->meta.V, d_t, S, d_B);
+    CAO_LAUNCHED("k_baseline");
+    return CAO_OK;
+}
+int cao_runs_score(const cao_runs* r, const float* d_sorted, const uint64_t* d_t, const double* d_B, uint32_t S, double* d_per_t,
+                   double* d_score, void* d_scratch, void* stream) {
+    if (!r || !d_sorted || !d_t || !d_B || !d_per_t || !d_score || !d_scratch) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_score: NULL argument");
+    if (S == 0) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_score: no sampling point");
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t items = (uint64_t)S * r->rm.R;
+    k_score_runs<<<(unsigned)((items + 255) / 256), 256, 0, st>>>(r->rm.traj, r->rm.R, r->gen, d_sorted, r->sm.V, d_t, d_B, S, (double*)d_scratch);
+    CAO_LAUNCHED("k_score_runs");
+    k_score_reduce<<<(S + 31) / 32, 32, 0, st>>>((const double*)d_scratch, r->rm.R, S, d_per_t, d_score);
+    CAO_LAUNCHED("k_score_reduce");
+    k_score_final<<<1, 1, 0, st>>>(d_per_t, S, d_score);
+    CAO_LAUNCHED("k_score_final");
     return CAO_OK;
 }
 

@@ -1,0 +1,301 @@
+// cao_var_kernels.cuh -- SURVEY 8(f) rows on the device: the paper's own neighbour rules and repairs (NEXT-1: PAPER.md
+// L139-143, L215, L270, Alg.2, Alg.3; readings A28, A30 in DESIGN.md) and the performance score
+// (NEXT-4: Eq.2; A36).  The non-constraint-aware variants (NEXT-2) and the operator variants (NEXT-3) live
+// in cao_runs_kernels.cuh next to the operators they modify.
+//
+// Strictly-adjacent neighbours are 3^n - 1 points (4.8 M at n = 14), so the neighbour sets are not probed in the bitmap:
+// they are found by the same tiled scan of the valid table as the north_star repair, with one more key layout.
+#pragma once
+#include "cao_runs_kernels.cuh"
+
+// present[d][k] = 1 iff some valid configuration has idx_d = k (A28).  Benign race: every writer stores 1.
+template <int ROWW>
+__global__ void __launch_bounds__(256) k_present(const __grid_constant__ SpaceMeta sm, uint8_t* present) {
+    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= sm.V) return;
+    uint32_t w[ROWW];
+    load_row<ROWW>(sm.rows + (uint64_t)r * (ROWW * 4), w);
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d)
+        if (d < sm.n) present[d * 256 + ((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu)] = 1;
+}
+
+// Where the continuous position of candidate `slot` lives: x(slot, d) = base[(slot / P) * blk + d * sd + (slot % P) * si].
+// Runs (state layout [run][dim][ind]): P = pop, blk = n * pop, sd = pop, si = 1.  Standalone rows: P = 1, blk = n, sd = 1.
+struct XAddr { const float* base; uint32_t P; uint64_t blk; uint32_t sd, si; };
+
+__device__ __forceinline__ uint32_t nz_bytes(uint32_t x) {              // 0x80 in every byte of x that is non-zero
+    return (((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x) & 0x80808080u;
+}
+
+// Membership of valid row v in the three neighbour sets of candidate c (L139-143): bit 0 strictly-adjacent (every
+// |delta index| <= 1), bit 1 adjacent (every index equal to c's or to the nearest present index below / above it, rows lo /
+// hi; a missing side repeats c's own index), bit 2 Hamming (exactly one parameter differs).  c is invalid, so v != c.
+template <int WU>
+__device__ __forceinline__ uint32_t nb_member(const uint32_t* c, const uint32_t* lo, const uint32_t* hi, const uint32_t* v) {
+    uint32_t far = 0, notadj = 0, ham = 0;
+#pragma unroll
+    for (int k = 0; k < WU; ++k) {
+        const uint32_t zc = nz_bytes(c[k] ^ v[k]);
+        far |= __vabsdiffu4(c[k], v[k]) & 0xFEFEFEFEu;
+        notadj |= zc & nz_bytes(lo[k] ^ v[k]) & nz_bytes(hi[k] ^ v[k]);
+        ham += __popc(zc);
+    }
+    return (far == 0 ? 1u : 0u) | (notadj == 0 ? 2u : 0u) | (ham == 1 ? 4u : 0u);
+}
+
+// lo / hi rows of candidate c from the presence table.
+template <int ROWW>
+__device__ __forceinline__ void near_rows(const SpaceMeta& sm, const uint8_t* __restrict__ present, const uint32_t (&c)[ROWW],
+                                          uint32_t (&lo)[ROWW], uint32_t (&hi)[ROWW]) {
+#pragma unroll
+    for (int z = 0; z < ROWW; ++z) { lo[z] = 0; hi[z] = 0; }
+#pragma unroll
+    for (int d = 0; d < ROWW * 4; ++d) {
+        if (d < sm.n) {
+            const int cd = (int)((c[d >> 2] >> ((d & 3) * 8)) & 0xFFu);
+            int l = cd, h = cd;
+            for (int k = cd - 1; k >= 0; --k) if (present[d * 256 + k]) { l = k; break; }
+            for (int k = cd + 1; k < (int)sm.m[d]; ++k) if (present[d * 256 + k]) { h = k; break; }
+            lo[d >> 2] |= (uint32_t)l << ((d & 3) * 8);
+            hi[d >> 2] |= (uint32_t)h << ((d & 3) * 8);
+        }
+    }
+}
+
+// Tiled scan of the valid table for the worklist candidates (same decomposition as k_scan: 128 candidates per CTA tile x
+// a chunk of the table staged through shared memory).  KIND 0 (Alg.2): per neighbour rule the minimum of
+// (squared Euclidean distance to the continuous position, fp32 bits << 32 | rank) into key3[slot][rule] (atomicMin:
+// order-free; distance >= 0, so bit patterns order like values; equal distances keep the smallest rank = smallest L).
+// KIND 1 (Alg.3): the number of members per rule into cnt3[slot][rule].
+template <int WU, int KIND>
+__global__ void __launch_bounds__(SCAN_TC) k_scan_nb(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
+                                                     const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
+                                                     const uint8_t* __restrict__ present, const XAddr xa,
+                                                     unsigned long long* key3, uint32_t* cnt3) {
+    constexpr int ROWW = WU <= 4 ? 4 : 8;
+    __shared__ uint4 tile[SCAN_TR * (ROWW / 4)];
+    __shared__ float s_coord[256];
+    const uint32_t count = *wl_count;
+    if (count == 0 || sm.V == 0) return;
+    const uint32_t tid = threadIdx.x;
+    for (uint32_t k = tid; k < 256; k += SCAN_TC) s_coord[k] = coord_M(sm.M, (int)k);     // O6: IEEE division, once
+    const uint32_t ntiles = (count + SCAN_TC - 1) / SCAN_TC;
+    const uint32_t nrt = (sm.V + SCAN_TR - 1) / SCAN_TR;
+    uint32_t nchunks = gridDim.x / ntiles; if (nchunks < 1) nchunks = 1; if (nchunks > nrt) nchunks = nrt;
+    const uint32_t tpc = (nrt + nchunks - 1) / nchunks;
+    nchunks = (nrt + tpc - 1) / tpc;
+    const uint64_t items = (uint64_t)ntiles * nchunks;
+    for (uint64_t item = blockIdx.x; item < items; item += gridDim.x) {
+        const uint32_t ct = (uint32_t)(item / nchunks), rc = (uint32_t)(item - (uint64_t)ct * nchunks);
+        const uint32_t ci = ct * SCAN_TC + tid;
+        const bool has = ci < count;
+        const uint32_t slot = has ? wl[ci] : 0;
+        uint32_t c[ROWW], lo[ROWW], hi[ROWW];
+        if (has) load_row_rw<ROWW>(cand_rows + (uint64_t)slot * (ROWW * 4), c);
+        else { for (int k = 0; k < ROWW; ++k) c[k] = 0; }
+        near_rows<ROWW>(sm, present, c, lo, hi);
+        float xr[WU * 4];
+        if (KIND == 0) {
+            const float* xp = xa.base + (uint64_t)(slot / xa.P) * xa.blk + (uint64_t)(slot % xa.P) * xa.si;
+#pragma unroll
+            for (int d = 0; d < WU * 4; ++d) xr[d] = (has && d < sm.n) ? xp[(uint64_t)d * xa.sd] : 0.0f;
+        }
+        float bestd[3] = {0.0f, 0.0f, 0.0f};
+        uint32_t bestr[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu}, cnt[3] = {0, 0, 0};
+        uint32_t rt1 = (rc + 1) * tpc; if (rt1 > nrt) rt1 = nrt;
+        for (uint32_t rt = rc * tpc; rt < rt1; ++rt) {
+            const uint32_t r0 = rt * SCAN_TR;
+            const uint32_t nr = min((uint32_t)SCAN_TR, sm.V - r0);
+            __syncthreads();
+            const uint4* src = (const uint4*)(sm.rows + (uint64_t)r0 * (ROWW * 4));
+            for (uint32_t q = tid; q < nr * (ROWW / 4); q += SCAN_TC) tile[q] = __ldg(&src[q]);
+            __syncthreads();
+#pragma unroll 2
+            for (uint32_t r = 0; r < nr; ++r) {
+                uint32_t v[ROWW];
+                { uint4 a = tile[r * (ROWW / 4)]; v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; }
+                if (ROWW == 8) { uint4 b = tile[r * 2 + 1]; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w; }
+                const uint32_t mem = nb_member<WU>(c, lo, hi, v);
+                if (mem && has) {                                       // rare: a neighbour under some rule
+                    if (KIND == 0) {
+                        float acc = 0.0f;
+#pragma unroll
+                        for (int d = 0; d < WU * 4; ++d) {
+                            if (d < sm.n) {
+                                const float df = __fsub_rn(s_coord[(v[d >> 2] >> ((d & 3) * 8)) & 0xFFu], xr[d]);
+                                acc = __fadd_rn(acc, __fmul_rn(df, df));
+                            }
+                        }
+#pragma unroll
+                        for (int q = 0; q < 3; ++q)
+                            if (((mem >> q) & 1u) && (bestr[q] == 0xFFFFFFFFu || acc < bestd[q])) { bestd[q] = acc; bestr[q] = r0 + r; }
+                    } else {
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) cnt[q] += (mem >> q) & 1u;
+                    }
+                }
+            }
+        }
+        if (has) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                if (KIND == 0) { if (bestr[q] != 0xFFFFFFFFu) atomicMin(&key3[(uint64_t)slot * 3 + q], ((unsigned long long)__float_as_uint(bestd[q]) << 32) | bestr[q]); }
+                else if (cnt[q]) atomicAdd(&cnt3[(uint64_t)slot * 3 + q], cnt[q]);
+            }
+        }
+    }
+}
+
+// Alg.3: one warp per worklist candidate.  The first non-empty rule (counts of k_scan_nb<.,1>) has K members;
+// member number below(w, K) in ascending L (= ascending rank) is found by walking the table in order, 32 rows per step
+// (ballot + prefix count).  w = w_arr[slot] (standalone) or draw(seed, first_run + slot / P, gen, slot % P, stream 5, slot 0).
+// Writes key[slot] = rank (high word 0) or leaves CAO_KEY_NONE, and the rule tap.
+template <int WU>
+__global__ void __launch_bounds__(256) k_pick_nb(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
+                                                 const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
+                                                 const uint8_t* __restrict__ present, const uint32_t* __restrict__ cnt3,
+                                                 const uint32_t* __restrict__ w_arr, uint64_t seed, uint32_t first_run, uint32_t P,
+                                                 uint32_t gen, unsigned long long* key, uint8_t* rule_out) {
+    constexpr int ROWW = WU <= 4 ? 4 : 8;
+    const uint32_t count = *wl_count, lane = threadIdx.x & 31;
+    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t ci = warp; ci < count; ci += nwarps) {
+        const uint32_t slot = wl[ci];
+        uint32_t rule = 3, K = 0;
+        for (int q = 2; q >= 0; --q) { const uint32_t e = cnt3[(uint64_t)slot * 3 + q]; if (e) { rule = (uint32_t)q; K = e; } }
+        if (rule == 3) { if (lane == 0 && rule_out) rule_out[slot] = 3; continue; }
+        uint32_t w;
+        if (w_arr) w = w_arr[slot];
+        else w = philox4x32_10(make_uint4(first_run + slot / P, gen, slot % P, 5u << 24), (uint32_t)seed, (uint32_t)(seed >> 32)).x;
+        uint32_t pick = below(w, K);
+        uint32_t c[ROWW], lo[ROWW], hi[ROWW];
+        load_row_rw<ROWW>(cand_rows + (uint64_t)slot * (ROWW * 4), c);
+        near_rows<ROWW>(sm, present, c, lo, hi);
+        uint32_t found = 0xFFFFFFFFu;
+        for (uint32_t base = 0; base < sm.V; base += 32) {
+            const uint32_t r = base + lane;
+            uint32_t v[ROWW];
+            load_row<ROWW>(sm.rows + (uint64_t)(r < sm.V ? r : base) * (ROWW * 4), v);
+            const bool mem = r < sm.V && ((nb_member<WU>(c, lo, hi, v) >> rule) & 1u);
+            const uint32_t bal = __ballot_sync(0xFFFFFFFFu, mem), n_here = (uint32_t)__popc(bal);
+            if (pick < n_here) { found = base + (uint32_t)kth_set_bit32(bal, pick); break; }
+            pick -= n_here;
+        }
+        if (lane == 0) {
+            if (found != 0xFFFFFFFFu) key[slot] = (unsigned long long)found;
+            if (rule_out) rule_out[slot] = (uint8_t)rule;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Standalone cao_space_repair_mode: rows -> clean copy, validity; invalid rows go to the worklist.
+template <int ROWW>
+__global__ void __launch_bounds__(256) k_mode_probe(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ rows_in, uint8_t* clean,
+                                                    uint64_t count, unsigned long long* key, unsigned long long* key3, uint32_t* cnt3,
+                                                    uint32_t* wl, uint32_t* wl_count, uint8_t* rule) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    uint32_t w[ROWW];
+    load_row<ROWW>(rows_in + i * (ROWW * 4), w);
+#pragma unroll
+    for (int z = 0; z < ROWW; ++z) {
+        const int first = z * 4;
+        if (first >= sm.n) w[z] = 0;
+        else if (first + 4 > sm.n) w[z] &= 0xFFFFFFFFu >> (8 * (first + 4 - sm.n));
+    }
+    store_row<ROWW>(clean + i * (ROWW * 4), w);
+    const uint64_t L = row_lin<ROWW>(sm, w);
+    const bool valid = bit_test(sm.bitmap, L);
+    key[i] = valid ? (unsigned long long)rank_of(sm, L) : CAO_KEY_NONE;
+    rule[i] = 255;
+    if (!valid) {
+        key3[i * 3] = ~0ull; key3[i * 3 + 1] = ~0ull; key3[i * 3 + 2] = ~0ull;
+        cnt3[i * 3] = 0; cnt3[i * 3 + 1] = 0; cnt3[i * 3 + 2] = 0;
+        worklist_push(wl, wl_count, (uint32_t)i);
+    }
+}
+// mode 1: rank = low word of the (sum|didx| << 32 | rank) minimum; mode 2: first rule with a member; mode 3: k_pick_nb's result.
+static __global__ void __launch_bounds__(256) k_mode_finish(int mode, const unsigned long long* __restrict__ key,
+                                                            const unsigned long long* __restrict__ key3, uint64_t count,
+                                                            uint32_t* rank_out, uint8_t* rule, uint8_t* rule_out) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    uint32_t rk = (uint32_t)key[i];
+    uint8_t ru = rule[i];
+    if (mode == 2 && key[i] == CAO_KEY_NONE) {
+        ru = 3;
+        for (int q = 2; q >= 0; --q) { const unsigned long long e = key3[i * 3 + q]; if (e != ~0ull) { ru = (uint8_t)q; rk = (uint32_t)e; } }
+    }
+    if (rank_out) rank_out[i] = rk;
+    if (rule_out) rule_out[i] = ru;
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-4.  Ascending sort of the objective table: bitonic network over the next power of two (padding = +inf bits);
+// f > 0, so fp32 bit patterns order like values.
+static __global__ void __launch_bounds__(256) k_sort_load(const float* __restrict__ obj, uint32_t V, uint32_t* buf, uint32_t n2) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n2) buf[i] = i < V ? __float_as_uint(obj[i]) : 0xFFFFFFFFu;
+}
+static __global__ void __launch_bounds__(256) k_bitonic_step(uint32_t* buf, uint32_t n2, uint32_t j, uint32_t k) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n2) return;
+    const uint32_t p = i ^ j;
+    if (p > i) {
+        const uint32_t a = buf[i], b = buf[p];
+        const bool up = (i & k) == 0;
+        if ((a > b) == up) { buf[i] = b; buf[p] = a; }
+    }
+}
+static __global__ void __launch_bounds__(256) k_sort_store(const uint32_t* __restrict__ buf, uint32_t V, float* sorted) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < V) sorted[i] = __uint_as_float(buf[i]);
+}
+// B(t) = sum_i f_(i) C(V-i, t-1) / C(V, t): one thread per sampling point runs the weight recurrence w_1 = t/V,
+// w_{i+1} = w_i (V-t-i+1) / (V-i) in the oracle's operation order (fp64, no contraction), so the values are bit-identical.
+static __global__ void __launch_bounds__(32) k_baseline(const float* __restrict__ sorted, uint64_t V, const uint64_t* __restrict__ ts,
+                                                        uint32_t S, double* B) {
+    const uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= S) return;
+    uint64_t t = ts[q];
+    if (t < 1) t = 1;
+    if (t > V) t = V;
+    double w = __ddiv_rn((double)t, (double)V), acc = 0.0;
+    for (uint64_t i = 1; i + t <= V + 1; ++i) {
+        acc = __dadd_rn(acc, __dmul_rn(w, (double)sorted[i - 1]));
+        w = __ddiv_rn(__dmul_rn(w, (double)(V - t - i + 1)), (double)(V - i));
+    }
+    B[q] = acc;
+}
+// P_t of every (sampling point, run): scratch[q * R + k].
+static __global__ void __launch_bounds__(256) k_score_runs(const uint32_t* __restrict__ traj, uint32_t R, uint32_t G,
+                                                           const float* __restrict__ sorted, uint64_t V, const uint64_t* __restrict__ ts,
+                                                           const double* __restrict__ B, uint32_t S, double* scratch) {
+    const uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (uint64_t)S * R) return;
+    const uint32_t q = (uint32_t)(e / R), k = (uint32_t)(e - (uint64_t)q * R);
+    const uint64_t t = ts[q];
+    uint32_t gsel = 0;
+    for (uint32_t g = 0; g <= G; ++g) if ((uint64_t)traj[((uint64_t)g * R + k) * 3 + 2] <= t) gsel = g;
+    const uint32_t fb = traj[((uint64_t)gsel * R + k) * 3], br = traj[((uint64_t)gsel * R + k) * 3 + 1];
+    const double best = br == 0xFFFFFFFFu ? (double)sorted[V - 1] : (double)__uint_as_float(fb);
+    const double b = B[q], opt = (double)sorted[0];
+    scratch[e] = __ddiv_rn(__dsub_rn(b, best), __dsub_rn(b, opt));
+}
+// Means in the oracle's order: over the runs (k ascending) for every sampling point, then over the sampling points.
+static __global__ void __launch_bounds__(32) k_score_reduce(const double* __restrict__ scratch, uint32_t R, uint32_t S, double* per_t,
+                                                            double* score) {
+    const uint32_t q = threadIdx.x + blockIdx.x * blockDim.x;
+    if (q < S) {
+        double acc = 0.0;
+        for (uint32_t k = 0; k < R; ++k) acc = __dadd_rn(acc, scratch[(uint64_t)q * R + k]);
+        per_t[q] = __ddiv_rn(acc, (double)R);
+    }
+}
+static __global__ void k_score_final(const double* __restrict__ per_t, uint32_t S, double* score) {
+    double tot = 0.0;
+    for (uint32_t q = 0; q < S; ++q) tot = __dadd_rn(tot, per_t[q]);
+    score[0] = S ? __ddiv_rn(tot, (double)S) : 0.0;
+}
