@@ -96,11 +96,14 @@ enum {
 };
 
 /* ---------------------------------------------------------------- define P = (X, D, C), L129-135 */
+/* An empty problem P = (X, D, C) (L129).  The handle is a host object owned by the library. */
 int cao_space_create(cao_space** out);
 void cao_space_destroy(cao_space* s);
-/* Appends a parameter with n_values (1..256) int64 values (copied).  Call order = digit order. */
+/* L131-132: appends a variable x_i with its finite domain D_i: n_values (1..256) int64 values (copied).  Call order =
+ * digit order (A1).  Errors: CAO_E_STATE after the build, CAO_E_TOO_LARGE beyond 32 parameters / 256 values. */
 int cao_space_add_param(cao_space* s, const char* name, const int64_t* h_values, int32_t n_values);
-/* Appends a constraint program (copied, validated: known opcodes, stack depth 1 at the end, <= 32). */
+/* L133: appends a constraint c_j, a predicate over a subset of the variables, as a postfix program (copied, validated:
+ * known opcodes, stack depth 1 at the end, <= 32).  Errors: CAO_E_INVALID_ARG for a malformed program. */
 int cao_space_add_constraint(cao_space* s, const int32_t* h_rpn, int32_t n_words);
 
 /* ---------------------------------------------------------------- build the space (S1; L137)
@@ -109,14 +112,16 @@ int cao_space_add_constraint(cao_space* s, const int32_t* h_rpn, int32_t n_words
  * give identical results.  Set before build_workspace_bytes. */
 int cao_space_set_build_mode(cao_space* s, int32_t mode);
 int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64_t* scratch_bytes);
-/* Highest Hamming level the generation step probes in the bitmap before it falls back to the table scan:
+/* L143 ("Hamming: all parameters identical except one"), L215: highest Hamming level the generation step probes in the bitmap before it falls back to the table scan:
  * -1 (default) = cost model (level h is probed while (number of rows at distance h) * 60 <= V * scan cost),
  * 0..6 = fixed (clamped to 1 when the space has more than 368 Hamming-1 neighbours or 65536 neighbour pairs).  Call before build_count; probe_levels() reports the level in use after build_count. */
 int cao_space_set_probe_levels(cao_space* s, int32_t levels);
 int cao_space_probe_levels(const cao_space* s, int32_t* levels);
-/* Pass 1: validity bitmap + per-512-config counts, then the exclusive scan of the counts.
+/* L137 ("determines all configurations in the search space before starting the tuning process"), O1.
+ * Pass 1: validity bitmap + per-512-config counts, then the exclusive scan of the counts.
  * Synchronises `stream` once to return V in *h_V.  d_scratch may be released after build_fill. */
 int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* stream, uint64_t* h_V);
+/* Bytes of d_table for build_fill (needs V, i.e. a completed build_count): rows + Ltab + rank directory + probe lists. */
 int cao_space_table_bytes(const cao_space* s, uint64_t* bytes);
 /* Pass 2: valid rows (V x row_bytes), Ltab (V linear indices: u32 when N <= 2^32, else u64 -- see
  * cao_space_ltab_bytes) and the rank directory, into d_table. */
@@ -125,6 +130,7 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream);
  * build, asynchronously and without any host round trip: the definition is unchanged, so V and the layout are
  * the ones build_count returned.  Needs a completed build_count + build_fill; d_scratch must still be alive. */
 int cao_space_rebuild(cao_space* s, void* stream);
+/* Table III's columns (L334-341): Cartesian size N, number of valid configurations V, dimensions n; row_bytes = 16 or 32. */
 int cao_space_sizes(const cao_space* s, uint64_t* N, uint64_t* V, int32_t* n, int32_t* row_bytes);
 /* Statistics of the last build / rebuild (synchronises `stream`; d_scratch must still be alive): h_out4 = {blocks of
  * B consecutive configs the index range is cut into, blocks that survived the tabled constraints and went on to the
@@ -137,7 +143,8 @@ int cao_space_views(const cao_space* s, const uint64_t** d_bitmap, const uint8_t
                     const void** d_Ltab, const uint32_t** d_rank_dir);
 
 /* ---------------------------------------------------------------- Search Space queries (L139), batched
- * d_idx_rows: count rows of row_bytes bytes each (padding ignored). */
+ * L139: "functionality to query whether a particular solution is valid": d_out[i] = 1 iff row i is a valid configuration
+ * (0 for a row with an index outside its domain).  d_idx_rows: count rows of row_bytes bytes each (padding ignored). */
 int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint8_t* d_out,
                        void* stream);
 /* S5 standalone: d_rank_out[i] = rank of argmin (Hamming, sum |didx|, L) over the valid table; the
@@ -160,7 +167,8 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
 int cao_space_repair_mode_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
 int cao_space_repair_mode(const cao_space* s, int32_t mode, const uint8_t* d_idx_rows, const float* d_x, const uint32_t* d_w,
                           uint64_t count, uint32_t* d_rank_out, uint8_t* d_rule_out, void* d_scratch, void* stream);
-/* Objective table by rank: V floats, > 0 and finite (borrowed; L268: the evaluation is a lookup). */
+/* Objective table by rank: V floats, > 0 and finite (borrowed).  L357: the evaluation replays pre-measured values
+ * (methodology of [29]); L268: evaluated configurations are memoised, so the evaluation is a lookup. */
 int cao_space_set_objective(cao_space* s, const float* d_obj);
 
 /* ---------------------------------------------------------------- runs (S2-S7)
@@ -168,7 +176,8 @@ int cao_space_set_objective(cao_space* s, const float* d_obj);
  * any partition of the run indices gives the same per-run results. */
 int cao_runs_workspace_bytes(const cao_space* s, int32_t algo, int32_t pop, uint32_t n_runs,
                              uint32_t max_gens, uint64_t* bytes);
-/* Creates the runs and executes generation 0 (S2; O4) on `stream`.  budget_unique: unique
+/* L139 / L282(i) ("generate a number of random samples of only valid solutions"), L125 (budget):
+ * creates the runs and executes generation 0 (S2; O4) on `stream`.  budget_unique: unique
  * evaluations per run, 0 = unlimited (L125, A20).  max_gens: generation cap = trajectory rows - 1. */
 int cao_runs_create(const cao_space* s, int32_t algo, const cao_hparams* hp, uint32_t n_runs,
                     uint32_t first_run, int32_t pop, uint32_t budget_unique, uint32_t max_gens,
@@ -190,12 +199,23 @@ void cao_runs_destroy(cao_runs* r);
  * does not fit the shared memory of one SM.  cao_runs_mode reports the mode in use. */
 int cao_runs_mode(const cao_runs* r, int32_t* mode);
 int cao_runs_set_mode(cao_runs* r, int32_t mode);
-/* S3-S7, n_generations times (stops recording at max_gens).  Asynchronous. */
+/* Fused mode only: threads per run as a multiple of the population rounded up to 32.  0 (default) = automatic: while the
+ * runs of a launch fill only part of the GPU, a run gets more lanes (Firefly: four lanes per firefly; the others: twice the
+ * threads for the cooperative neighbour probes and scans); 1, 2, 4 = fixed (4 = Firefly's four-lane operator, 16-byte
+ * rows only; a width that does not apply falls back to 1).  Identical results at every width (O3: draws are addressed,
+ * never consumed in order).  Call before the first fused cao_runs_step. */
+int cao_runs_set_fused_width(cao_runs* r, int32_t width);
+int cao_runs_fused_width(const cao_runs* r, int32_t* width);
+/* One batched generation of every run, n_generations times: operator (Alg.1 L147-213 DE; L276-282 PSO; L284 Firefly;
+ * L286-292 GA), snap (L280), validity (L139), repair (L215, L270, Alg.2-3), evaluation with memoisation (L268), selection
+ * and budget test (L125, A20).  Stops recording at max_gens.  Asynchronous. */
 int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream);
-/* Copies per-run results to DEVICE arrays of n_runs elements each (any may be NULL). */
+/* Eq.1 (L115): best configuration found so far per run (minimisation, O0), with its unique-evaluation count (L268) and the
+ * generations executed.  Copies to DEVICE arrays of n_runs elements each (any may be NULL). */
 int cao_runs_best(const cao_runs* r, float* d_best_f, uint32_t* d_best_rank, uint32_t* d_uniq,
                   uint32_t* d_gens_done, void* stream);
-/* Borrowed: trajectory [gen][run] of packed {f32 best_f, u32 best_rank, u32 uniq}, gens 0..generation. */
+/* The "performance over time" of Fig. 3-4 (L395-403) in simulated mode, time = unique evaluations.
+ * Borrowed: trajectory [gen][run] of packed {f32 best_f, u32 best_rank, u32 uniq}, gens 0..generation. */
 int cao_runs_trajectory(const cao_runs* r, const void** d_traj, uint32_t* gens_recorded);
 /* Parity taps of the last stepped generation, [run][ind]: post-snap pre-repair rows (row_bytes each),
  * validity flag, rank after repair, rank evaluated, f, accept flag, and [run] active flag. */
@@ -205,7 +225,8 @@ int cao_runs_debug_last(const cao_runs* r, const uint8_t** d_postsnap_rows, cons
 /* NEXT-1 tap of the last stepped generation, [run][ind]: neighbour rule that repaired the candidate (0 strictly-adjacent,
  * 1 adjacent, 2 Hamming), 3 = every set empty, 255 = not applicable (valid candidate, or another repair mode). */
 int cao_runs_debug_rule(const cao_runs* r, const uint8_t** d_rule);
-/* Raw population state, borrowed.  which: 0 idx rows [run][ind][row_bytes] u8, 1 rank [run][ind] u32,
+/* Raw population state, borrowed.  SURVEY 8(b) sketched one blob (`const void** d_state, uint64_t* bytes`); the arrays have
+ * different element types and only some exist per algorithm, so this call takes a selector instead.  which: 0 idx rows [run][ind][row_bytes] u8, 1 rank [run][ind] u32,
  * 2 f [run][ind] f32, 3 x, 4 v, 5 pbest [run][dim][ind] f32 (dimension-major), 6 pbest_f [run][ind]. */
 int cao_runs_debug_state(const cao_runs* r, int32_t which, const void** d_ptr, uint64_t* bytes);
 /* Counters since create (synchronises `stream`): candidates whose post-snap row was invalid,

@@ -91,6 +91,8 @@ SIGNATURES = {
     "cao_runs_set_mode": (C.c_int, [vp, i32]),
     "cao_runs_mode": (C.c_int, [vp, pi32]),
     "cao_runs_step": (C.c_int, [vp, u32, vp]),
+    "cao_runs_set_fused_width": (C.c_int, [vp, i32]),
+    "cao_runs_fused_width": (C.c_int, [vp, pi32]),
     "cao_runs_best": (C.c_int, [vp, vp, vp, vp, vp, vp]),
     "cao_runs_trajectory": (C.c_int, [vp, pvp, C.POINTER(u32)]),
     "cao_runs_debug_last": (C.c_int, [vp, pvp, pvp, pvp, pvp, pvp, pvp, pvp]),
@@ -373,7 +375,7 @@ class Runs:
     """n_runs independent simulated tuning runs of one algorithm; creation executes generation 0 (S2)."""
 
     def __init__(self, space: Space, algo, n_runs, pop, budget=0, max_gens=100, seed=0, first_run=0, hparams=None,
-                 mode=None, variant: Variant | None = None):
+                 mode=None, variant: Variant | None = None, fused_width=None):
         self.space, self.R, self.P, self.n = space, int(n_runs), int(pop), space.n
         self.algo = ALGOS[algo] if isinstance(algo, str) else int(algo)
         self.hp = hparams or HParams.default()
@@ -390,6 +392,14 @@ class Runs:
         self._h = h
         if mode is not None:
             self.set_mode(mode)
+        if fused_width is not None:
+            _check(lib().cao_runs_set_fused_width(self._h, int(fused_width)))
+
+    @property
+    def fused_width(self) -> int:
+        v = i32()
+        _check(lib().cao_runs_fused_width(self._h, C.byref(v)))
+        return v.value
 
     def set_mode(self, mode):
         """'fused' / 1 = one persistent kernel per step call; 'phased' / 0 = per-generation kernels."""

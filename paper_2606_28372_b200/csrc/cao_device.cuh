@@ -35,7 +35,8 @@ struct SpaceMeta {
 struct ProbeMeta {
     const uint16_t* nb;                 // NB entries: d << 8 | k
     const uint32_t* pairs;              // C2 entries: t1 | t2 << 16, dimension(t1) < dimension(t2)
-    uint32_t NB, C2;
+    const uint32_t* triples;            // C3 entries: t1 | t2 << 10 | t3 << 20, strictly increasing dimensions (0 entries: level 3 walks)
+    uint32_t NB, C2, C3;
     int32_t levels;                     // highest Hamming level probed in the bitmap before the table scan (0..6)
     uint16_t nb_first[CAO_MAX_DIMS + 1];    // first neighbour of dimension d; nb_first[n..] = NB
 };
@@ -132,8 +133,8 @@ __device__ __forceinline__ float exp_neg_spec(float z) {
                 c4 = 0x1.3b2ab6p-7f, c5 = -0x1.5d87fep-10f, c6 = 0x1.430912p-13f, c7 = -0x1.ffcbfcp-17f;
     float t = __fmul_rn(z, LOG2E);
     float kf = floorf(t);
-    if (!(kf < 126.0f)) return 0.0f;
-    float fr = __fsub_rn(t, kf);
+    const bool tiny = !(kf < 126.0f);                               // result 0 (also for NaN); decided by a select at the end, so
+    float fr = __fsub_rn(t, kf);                                        // the dependent chain below can overlap independent work
     float u = __fsub_rn(fr, 0.5f);
     float p = c7;
     p = __fadd_rn(__fmul_rn(p, u), c6);
@@ -144,8 +145,8 @@ __device__ __forceinline__ float exp_neg_spec(float z) {
     p = __fadd_rn(__fmul_rn(p, u), c1);
     p = __fadd_rn(__fmul_rn(p, u), c0);
     p = __fmul_rn(p, RSQRT2);
-    float scale = __uint_as_float((uint32_t)(127 - (int)kf) << 23);
-    return __fmul_rn(p, scale);
+    float scale = __uint_as_float((uint32_t)(127 - (int)(tiny ? 0.0f : kf)) << 23);
+    return tiny ? 0.0f : __fmul_rn(p, scale);
 }
 
 __device__ __forceinline__ float clamp_pos(float x, float hi) {   // NaN -> 0, -0 -> +0

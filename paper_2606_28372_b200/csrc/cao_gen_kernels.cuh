@@ -299,7 +299,7 @@ __device__ __forceinline__ void store_state(const Grp& g, const SpaceMeta& sm, c
 // issue and instruction fetch, not by memory).
 template <int ALGO, int ROWW>
 __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, const ProbeMeta& pm, const CtaTabs& tb,
-                                           const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen, bool last) {
+                                           const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen, bool last, bool wide) {
     constexpr int RB = ROWW * 4;
     const uint32_t i = g.t, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
@@ -401,6 +401,78 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
                 PUT_DIM(d, (uint32_t)kq);
             }
         }
+    } else if (ROWW == 4 && wide) {                                     // O7: Firefly, FOUR LANES PER FIREFLY (underfilled GPU)
+        // A lone warp per run is bound by the dependent chain r2 -> exp -> update of every attractor j.  Here lanes 4f..4f+3
+        // share firefly f: lane `part` owns dimensions 4 part .. 4 part + 3, computes ONE Philox block per attractor instead
+        // of five, and only the r2 sum is replicated: the 16 squared differences are gathered by shuffles and added in
+        // dimension order, so every lane holds the oracle's r2 bit for bit.  The positions are exchanged through S.x.
+        g.sync();
+        const uint32_t ff = g.t >> 2, part = g.t & 3, lane_base = (g.t & 31u) & ~3u;
+        const bool hasw = ff < P;
+        float xi4[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { const int d = (int)part * 4 + q; xi4[q] = (hasw && d < n) ? S.x[ff * n + d] : 0.0f; }
+        const float fme = hasw ? S.f[ff] : 0.0f;
+        for (uint32_t j = 0; j < P; ++j) {
+            const bool brighter = hasw && S.f[j] < fme;
+            if (!__any_sync(0xFFFFFFFFu, brighter)) continue;
+            const float* xj = S.x + (size_t)j * n;
+            float xj4[4], sq[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int d = (int)part * 4 + q;
+                xj4[q] = d < n ? xj[d] : 0.0f;
+                const float df = __fsub_rn(xj4[q], xi4[q]);
+                sq[q] = __fmul_rn(df, df);
+            }
+            // this lane's Philox block of the attractor's noise draws (slots j*n .. j*n+n-1); the next lane's block supplies
+            // the words that spill over when the first slot is not block-aligned
+            const uint32_t s0 = j * (uint32_t)n, o = s0 & 3;
+            uint4 blk = philox4x32_10(make_uint4(run, gen, ff, (S_OP << 24) | ((s0 >> 2) + part)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
+            uint32_t nx = __shfl_down_sync(0xFFFFFFFFu, blk.x, 1), ny = __shfl_down_sync(0xFFFFFFFFu, blk.y, 1),
+                     nz = __shfl_down_sync(0xFFFFFFFFu, blk.z, 1);
+            if (o + (uint32_t)n > 16u) {                                // group-uniform: the last lane needs a fifth block
+                if (part == 3) {
+                    const uint4 b5 = philox4x32_10(make_uint4(run, gen, ff, (S_OP << 24) | ((s0 >> 2) + 4)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
+                    nx = b5.x; ny = b5.y; nz = b5.z;
+                }
+            }
+            float r2 = 0.0f;                                            // sum over d = 0 .. 15 in order (padding adds +0)
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) r2 = __fadd_rn(r2, __shfl_sync(0xFFFFFFFFu, sq[q], lane_base + pp));
+            const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
+            uint32_t w4[4];
+            if (o == 0) { w4[0] = blk.x; w4[1] = blk.y; w4[2] = blk.z; w4[3] = blk.w; }
+            else if (o == 1) { w4[0] = blk.y; w4[1] = blk.z; w4[2] = blk.w; w4[3] = nx; }
+            else if (o == 2) { w4[0] = blk.z; w4[1] = blk.w; w4[2] = nx; w4[3] = ny; }
+            else { w4[0] = blk.w; w4[1] = nx; w4[2] = ny; w4[3] = nz; }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int d = (int)part * 4 + q;
+                const float df = __fsub_rn(xj4[q], xi4[q]);
+                float tq = __fadd_rn(xi4[q], __fmul_rn(beta, df));
+                const float e = __fsub_rn(u01(w4[q]), 0.5f);
+                tq = __fadd_rn(tq, __fmul_rn(rm.hp.ff_alpha, e));
+                xi4[q] = (brighter && d < n) ? tq : xi4[q];
+            }
+        }
+        g.sync();                                                       // all start-of-generation positions are consumed
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int d = (int)part * 4 + q;
+            if (hasw && d < n) S.x[ff * n + d] = clamp_pos(xi4[q], tb.hi[d]);
+        }
+        g.sync();
+        if (has) {
+            const float fM = (float)(sm.M - 1);
+            for (int d = 0; d < n; ++d) {
+                int kq = __float2int_rn(__fmul_rn(S.x[i * n + d], fM));
+                kq = min(max(kq, 0), (int)sm.m[d] - 1);
+                PUT_DIM(d, (uint32_t)kq);
+            }
+        }
     } else {                                                            // O7: Firefly (Yang's rule, synchronous)
         g.sync();
         float xi[RB];
@@ -413,11 +485,6 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             const bool brighter = has && S.f[j] < fi;                   // only brighter (cheaper) fireflies attract
             if (!__any_sync(0xFFFFFFFFu, brighter)) continue;           // warp-uniform: draws are addressed by slot, skipping is free
             const float* xj = S.x + (size_t)j * n;
-            float r2 = 0.0f;
-#pragma unroll
-            for (int d = 0; d < RB; ++d)
-                if (d < n) { const float df = __fsub_rn(xj[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
-            const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
             // the n noise draws of this j are slots j*n .. j*n+n-1: all their Philox blocks at once (independent chains),
             // then one specialised update per alignment o = first slot & 3, so every word is a fixed register
             const uint32_t s0 = j * (uint32_t)n, o = s0 & 3;
@@ -437,19 +504,47 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
 #pragma unroll
                 for (int z = 0; z < ROWW + 1; ++z) { nw[4 * z] = q5[z].x; nw[4 * z + 1] = q5[z].y; nw[4 * z + 2] = q5[z].z; nw[4 * z + 3] = q5[z].w; }
             }
-#define FF_UPDATE(O)                                                                         \
-            _Pragma("unroll")                                                                \
-            for (int d = 0; d < RB; ++d) {                                                   \
-                if (d < n) {                                                                 \
-                    const float df = __fsub_rn(xj[d], xi[d]);                                \
+            if (ROWW == 4) {
+                // Narrow rows: all 16 dimension slots are computed unconditionally (straight-line code, xi in registers).  A
+                // padding slot d >= n holds xj = xi = +0: it adds +0 to r2 (exact) and its update is discarded by the select.
+                float xjv[RB];
+#pragma unroll
+                for (int d = 0; d < RB; ++d) xjv[d] = d < n ? xj[d] : 0.0f;
+                float r2 = 0.0f;
+#pragma unroll
+                for (int d = 0; d < RB; ++d) { const float df = __fsub_rn(xjv[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
+                const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
+#define FF_UPDATE_FLAT(O)                                                                    \
+                _Pragma("unroll")                                                            \
+                for (int d = 0; d < RB; ++d) {                                               \
+                    const float df = __fsub_rn(xjv[d], xi[d]);                               \
                     float tq = __fadd_rn(xi[d], __fmul_rn(beta, df));                        \
                     const float e = __fsub_rn(u01(nw[d + (O)]), 0.5f);                       \
                     tq = __fadd_rn(tq, __fmul_rn(rm.hp.ff_alpha, e));                        \
-                    xi[d] = brighter ? tq : xi[d];                                           \
-                }                                                                            \
-            }
-            if (o == 0) { FF_UPDATE(0) } else if (o == 1) { FF_UPDATE(1) } else if (o == 2) { FF_UPDATE(2) } else { FF_UPDATE(3) }
+                    xi[d] = (brighter && d < n) ? tq : xi[d];                                \
+                }
+                if (o == 0) { FF_UPDATE_FLAT(0) } else if (o == 1) { FF_UPDATE_FLAT(1) } else if (o == 2) { FF_UPDATE_FLAT(2) } else { FF_UPDATE_FLAT(3) }
+#undef FF_UPDATE_FLAT
+            } else {
+                float r2 = 0.0f;
+#pragma unroll
+                for (int d = 0; d < RB; ++d)
+                    if (d < n) { const float df = __fsub_rn(xj[d], xi[d]); r2 = __fadd_rn(r2, __fmul_rn(df, df)); }
+                const float beta = __fmul_rn(rm.hp.ff_B0, exp_neg_spec(__fmul_rn(rm.hp.ff_gamma, r2)));
+#define FF_UPDATE(O)                                                                         \
+                _Pragma("unroll")                                                            \
+                for (int d = 0; d < RB; ++d) {                                               \
+                    if (d < n) {                                                             \
+                        const float df = __fsub_rn(xj[d], xi[d]);                            \
+                        float tq = __fadd_rn(xi[d], __fmul_rn(beta, df));                    \
+                        const float e = __fsub_rn(u01(nw[d + (O)]), 0.5f);                   \
+                        tq = __fadd_rn(tq, __fmul_rn(rm.hp.ff_alpha, e));                    \
+                        xi[d] = brighter ? tq : xi[d];                                       \
+                    }                                                                        \
+                }
+                if (o == 0) { FF_UPDATE(0) } else if (o == 1) { FF_UPDATE(1) } else if (o == 2) { FF_UPDATE(2) } else { FF_UPDATE(3) }
 #undef FF_UPDATE
+            }
         }
         g.sync();                                                       // all start-of-generation positions are consumed
         if (has) {
@@ -822,7 +917,7 @@ k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm
         for (; gen <= g_last; ++gen) {
             const bool active = rm.budget == 0 || gs->uniq < rm.budget;  // O10 (gen <= max_gens is enforced by the host)
             if (!active) break;
-            generation<ALGO, ROWW>(g, sm, pm, tb, rm, S, k, gen, gen == g_last);
+            generation<ALGO, ROWW>(g, sm, pm, tb, rm, S, k, gen, gen == g_last, lay.wide != 0);
         }
         // a run that reached its budget stays frozen: its trajectory row repeats (O10)
         for (uint32_t q = gen + g.t; q <= g_last; q += g.G) {

@@ -9,7 +9,8 @@ struct GenLayout {
     uint32_t cta_words;              // CTA-wide prefix: strides, upper coordinates, Hamming-1 neighbour list, probe lists
     uint32_t NB, nb_words;           // Hamming-1 neighbours of a point = sum (m_d - 1); words of their list
     uint32_t probe_in_smem;          // the target / pair lists of the Hamming-2/3 probe are copied to shared memory
-    uint32_t G, NG;                  // threads per group, groups per CTA
+    uint32_t G, NG;                  // threads per group (a multiple of roundup32(P): groups are widened while the GPU is underfilled), groups per CTA
+    uint32_t wide;                   // Firefly: four adjacent lanes share one firefly (G = 4 * roundup32(P))
 };
 
 #define GRP_SHARED_WORDS 48             // sizeof(GrpShared) / 4

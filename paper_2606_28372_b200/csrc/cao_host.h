@@ -78,8 +78,8 @@ struct cao_space {
     // Hamming-level probes (S5)
     ProbeMeta probe{};
     std::vector<uint16_t> h_nb;
-    std::vector<uint32_t> h_pairs;
-    uint64_t off_pairs = 0;
+    std::vector<uint32_t> h_pairs, h_triples;
+    uint64_t off_pairs = 0, off_triples = 0;
     int probe_levels_req = -1;         // -1 = cost model
     // the zero fill of the bitmap runs on a side stream, overlapped with the table build
     cudaStream_t side = nullptr;

@@ -140,6 +140,21 @@ static __device__ __noinline__ int probe_levels_grp(const Grp g, const uint64_t*
 #pragma unroll
                 for (int u = 0; u < 4; ++u) if (bit[u]) best = k2[u] < best ? k2[u] : best;
             }
+        } else if (level == 3 && pm.C3) {
+            const uint32_t C3 = pm.C3;                                  // flat triple list: eight independent bit tests per thread and pass
+            const uint32_t* __restrict__ tri = pm.triples;
+            for (uint32_t q0 = 0; q0 < C3; q0 += 8 * g.G) {
+                uint64_t k3[8]; bool bit[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const uint32_t q = q0 + u * g.G + g.t;
+                    const uint32_t tr = __ldg(&tri[q < C3 ? q : 0]);
+                    k3[u] = L + ptab[tr & 1023u] + ptab[(tr >> 10) & 1023u] + ptab[tr >> 20];
+                    bit[u] = bit_test(bitmap, k3[u] & M40) && q < C3;
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) if (bit[u]) best = k3[u] < best ? k3[u] : best;
+            }
         } else {
             const int extra = level - 3;                                // middle neighbours walked depth-first (0 .. 3)
             for (uint32_t q = g.t; q < C2; q += g.G) {

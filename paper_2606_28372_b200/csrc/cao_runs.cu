@@ -189,7 +189,11 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
 }
 
 // Shared-memory slice of one group of the fused kernel (cao_gen_kernels.cuh): word offsets.
-static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P) {
+// width: 0 = automatic, 1 / 2 / 4 = threads per group as a multiple of roundup32(P).  Automatic: while the runs of this
+// launch fill only part of the GPU's resident thread slots (148 SMs x 3 CTAs x 256 threads), a run gets more lanes --
+// Firefly four per firefly (its operator is a dependent chain per attractor), the others two (their cooperative phases:
+// neighbour probes, scans, GA mutation, stride over the group).  Results do not depend on the width.
+static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P, uint32_t R, int width) {
     GenLayout L{};
     const uint32_t n = (uint32_t)s->meta.n, roww = (uint32_t)s->meta.rowB / 4;
     uint32_t off = GRP_SHARED_WORDS;
@@ -205,7 +209,16 @@ static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P) {
     L.Lc = take(2 * P); L.aux4 = take(4 * P);
     L.ptab = take(s->probe.levels >= 2 ? 2 * s->probe.NB : 0);
     L.words = off;
-    L.G = (P + 31) / 32 * 32;
+    const uint32_t G0 = (P + 31) / 32 * 32;
+    const double slots = 148.0 * 3 * 256;
+    uint32_t f = 1;
+    if (width == 0) {
+        if (algo == CAO_FIREFLY) { if (roww == 4 && G0 * 4 <= 256 && (double)R * G0 * 4 <= 1.25 * slots) f = 4; }
+        else if (G0 * 2 <= 256 && (double)R * G0 * 2 <= 0.6 * slots) f = 2;
+    } else if ((uint32_t)width * G0 <= 256 && !(algo == CAO_FIREFLY && width == 4 && roww != 4)) f = (uint32_t)width;
+    L.wide = algo == CAO_FIREFLY && f == 4 ? 1 : 0;
+    if (algo == CAO_FIREFLY && f == 2) f = 1;                           // Firefly is either one warp-lane or four lanes per firefly
+    L.G = G0 * f;
     L.NG = L.G <= 256 ? 256 / L.G : 1;
     L.NB = 0;
     for (uint32_t d = 0; d < n; ++d) L.NB += (uint32_t)s->meta.m[d] - 1u;
@@ -354,7 +367,7 @@ int cao_runs_create_ex(const cao_space* s, int32_t algo, const cao_hparams* hp, 
     const uint64_t RP = (uint64_t)n_runs * pop;
     r->bytes_idx = RP * s->meta.rowB; r->bytes_pi = RP * 4; r->bytes_pn = RP * s->meta.n * 4;
     r->block = (unsigned)((pop + 31) / 32 * 32);
-    r->lay = gen_layout(s, algo, (uint32_t)pop);
+    r->lay = gen_layout(s, algo, (uint32_t)pop, n_runs, 0);
     r->gen_threads = r->lay.G * r->lay.NG;
     r->gen_smem = ((size_t)r->lay.cta_words + (size_t)r->lay.NG * r->lay.words) * 4;
     {   // default execution mode: how many invalid candidates will fall through the bitmap probes to the table scan?
@@ -482,6 +495,22 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
         CAO_LAUNCHED("k_finish");
         r->gen = g;
     }
+    return CAO_OK;
+}
+
+int cao_runs_set_fused_width(cao_runs* r, int32_t width) {
+    if (!r || (width != 0 && width != 1 && width != 2 && width != 4))
+        return cao_fail(CAO_E_INVALID_ARG, "cao_runs_set_fused_width: width must be 0 (automatic), 1, 2 or 4");
+    if (r->gen_grid != 0) return cao_fail(CAO_E_STATE, "cao_runs_set_fused_width: call before the first fused cao_runs_step");
+    const GenLayout L = gen_layout(r->s, r->rm.algo, r->rm.P, r->rm.R, width);
+    const size_t smem = ((size_t)L.cta_words + (size_t)L.NG * L.words) * 4;
+    if (smem > 227 * 1024) return cao_fail(CAO_E_TOO_LARGE, "cao_runs_set_fused_width: the groups do not fit the shared memory of one SM");
+    r->lay = L; r->gen_threads = L.G * L.NG; r->gen_smem = smem;
+    return CAO_OK;
+}
+int cao_runs_fused_width(const cao_runs* r, int32_t* width) {
+    if (!r || !width) return cao_fail(CAO_E_INVALID_ARG, "cao_runs_fused_width: NULL argument");
+    *width = (int32_t)(r->lay.G / ((r->rm.P + 31) / 32 * 32));
     return CAO_OK;
 }
 

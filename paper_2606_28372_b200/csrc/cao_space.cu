@@ -492,10 +492,20 @@ int cao_space_build_count(cao_space* s, void* d_bitmap, void* d_scratch, void* s
                 for (uint32_t t2 = s->probe.nb_first[(s->h_nb[t1] >> 8) + 1]; t2 < s->probe.NB; ++t2)
                     s->h_pairs.push_back(t1 | (t2 << 16));
         s->probe.C2 = (uint32_t)s->h_pairs.size();
+        // flat list of the Hamming-3 neighbour triples (the level that dominates the slow runs): every lane takes
+        // triples with eight independent bit tests in flight instead of walking the third neighbour serially per pair
+        s->h_triples.clear();
+        if (lv >= 3 && e[3] <= 131072.0)
+            for (uint32_t t1 = 0; t1 < s->probe.NB; ++t1)
+                for (uint32_t t2 = s->probe.nb_first[(s->h_nb[t1] >> 8) + 1]; t2 < s->probe.NB; ++t2)
+                    for (uint32_t t3 = s->probe.nb_first[(s->h_nb[t2] >> 8) + 1]; t3 < s->probe.NB; ++t3)
+                        s->h_triples.push_back(t1 | (t2 << 10) | (t3 << 20));
+        s->probe.C3 = (uint32_t)s->h_triples.size();
         s->probe.levels = lv;
     }
     s->off_tgt = off; off = align256(off + std::max<uint64_t>(1, s->h_nb.size()) * 2);
     s->off_pairs = off; off = align256(off + std::max<uint64_t>(1, s->h_pairs.size()) * 4);
+    s->off_triples = off; off = align256(off + std::max<uint64_t>(1, s->h_triples.size()) * 4);
     s->table_bytes = off;
     return CAO_OK;
 }
@@ -522,6 +532,9 @@ int cao_space_build_fill(cao_space* s, void* d_table, void* stream) {
     if (!s->h_pairs.empty())
         CAO_CUDA(cudaMemcpyAsync(tb + s->off_pairs, s->h_pairs.data(), s->h_pairs.size() * 4, cudaMemcpyHostToDevice, st));
     s->probe.pairs = (const uint32_t*)(tb + s->off_pairs);
+    if (!s->h_triples.empty())
+        CAO_CUDA(cudaMemcpyAsync(tb + s->off_triples, s->h_triples.data(), s->h_triples.size() * 4, cudaMemcpyHostToDevice, st));
+    s->probe.triples = (const uint32_t*)(tb + s->off_triples);
     s->meta.rows = rows; s->meta.Ltab = Ltab; s->meta.dir = dir;
     s->d_table = d_table;
     s->filled = true;

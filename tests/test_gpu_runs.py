@@ -71,7 +71,11 @@ def run_pair(cfg, algo, R, P, gens, budget=0, seed=0, first_run=0, step_sizes=No
     kw = dict(n_runs=R, pop=P, budget=budget, max_gens=gens, seed=seed, first_run=first_run)
     orr = O.OracleRuns(os_, algo, hparams=hp, **kw)
     ghp = None if hp is None else cao.HParams(*[getattr(hp, f[0]) for f in hp._fields_])
-    grs = [cao.Runs(g, algo, hparams=ghp, mode=m, **kw) for m in ("fused", "phased")]   # both execution modes
+    # both execution modes; fused at the automatic group width (small run counts: widened groups, Firefly with four lanes
+    # per firefly) and at width 1 (the shape of a filled GPU)
+    grs = [cao.Runs(g, algo, hparams=ghp, mode="fused", **kw), cao.Runs(g, algo, hparams=ghp, mode="fused", fused_width=1, **kw),
+           cao.Runs(g, algo, hparams=ghp, mode="phased", **kw)]
+    assert grs[1].fused_width == 1 and grs[0].fused_width == (4 if algo == "firefly" and sp.n <= 16 and P <= 64 else 2 if P <= 128 and not (algo == "firefly") else 1)
     for gr in grs:
         compare(gr, orr, sp.n)
     done = 0
