@@ -238,12 +238,20 @@ __global__ void __launch_bounds__(256) k_probe23(const __grid_constant__ SpaceMe
 // SMALL: every index < 128, so a byte of c^v is non-zero iff adding 0x7f carries into its bit 7.
 // KM: key layout.  0 = north_star's (Hamming << 13 + sum|didx|) << 32 | rank; 1 = NEXT-1 index distance (L215, L270):
 // sum|didx| << 32 | rank (the Hamming count is not computed).
+// 16-byte asynchronous global -> shared copy (LDGSTS; bypasses registers and L1) and its group fences.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 template <int WU, bool SMALL, int KM = 0>
 __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
                                                   const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
                                                   unsigned long long* key) {
     constexpr int ROWW = WU <= 4 ? 4 : 8;
-    __shared__ uint4 tile[SCAN_TR * (ROWW / 4)];
+    constexpr int TQ = SCAN_TR * (ROWW / 4);                             // 16-byte quads per tile
+    __shared__ uint4 tile[2][TQ];                                        // double buffer: tile rt+1 streams in (cp.async) while rt is scanned
     const uint32_t count = *wl_count;
     if (count == 0 || sm.V == 0) return;
     const uint32_t tid = threadIdx.x;
@@ -253,6 +261,13 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
     const uint32_t tpc = (nrt + nchunks - 1) / nchunks;                  // row tiles per chunk
     nchunks = (nrt + tpc - 1) / tpc;
     const uint64_t items = (uint64_t)ntiles * nchunks;
+    const uint4* table = (const uint4*)sm.rows;
+    auto stage = [&](uint32_t rt, int buf) {                             // issue the copies of row tile rt into buffer buf
+        const uint32_t r0 = rt * SCAN_TR, nr = min((uint32_t)SCAN_TR, sm.V - r0);
+        const uint4* src = table + (uint64_t)r0 * (ROWW / 4);
+        for (uint32_t q = tid; q < nr * (ROWW / 4); q += SCAN_TC) cp_async16(&tile[buf][q], &src[q]);
+        cp_async_commit();
+    };
     for (uint64_t item = blockIdx.x; item < items; item += gridDim.x) {
         const uint32_t ct = (uint32_t)(item / nchunks), rc = (uint32_t)(item - (uint64_t)ct * nchunks);
         const uint32_t ci = ct * SCAN_TC + tid;
@@ -263,18 +278,22 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
         else { for (int k = 0; k < ROWW; ++k) c[k] = 0; }
         uint32_t bestk = 0xFFFFFFFFu, bestr = 0xFFFFFFFFu;
         uint32_t rt1 = (rc + 1) * tpc; if (rt1 > nrt) rt1 = nrt;
-        for (uint32_t rt = rc * tpc; rt < rt1; ++rt) {
+        const uint32_t rt0 = rc * tpc;
+        __syncthreads();                                                 // the previous item's last tile is no longer read
+        if (rt0 < rt1) stage(rt0, 0);
+        for (uint32_t rt = rt0; rt < rt1; ++rt) {
+            const int buf = (int)((rt - rt0) & 1u);
+            if (rt + 1 < rt1) { stage(rt + 1, buf ^ 1); cp_async_wait<1>(); }   // (buf ^ 1 was released by the barrier below)
+            else cp_async_wait<0>();
+            __syncthreads();                                             // tile rt has landed for every thread
             const uint32_t r0 = rt * SCAN_TR;
             const uint32_t nr = min((uint32_t)SCAN_TR, sm.V - r0);
-            __syncthreads();
-            const uint4* src = (const uint4*)(sm.rows + (uint64_t)r0 * (ROWW * 4));
-            for (uint32_t q = tid; q < nr * (ROWW / 4); q += SCAN_TC) tile[q] = __ldg(&src[q]);
-            __syncthreads();
+            const uint4* tl = tile[buf];
 #pragma unroll 4
             for (uint32_t r = 0; r < nr; ++r) {
                 uint32_t v[ROWW];
-                { uint4 a = tile[r * (ROWW / 4)]; v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; }
-                if (ROWW == 8) { uint4 b = tile[r * 2 + 1]; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w; }
+                { uint4 a = tl[r * (ROWW / 4)]; v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; }
+                if (ROWW == 8) { uint4 b = tl[r * 2 + 1]; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w; }
                 uint32_t sad = 0, hb = 0, ham = 0;
 #pragma unroll
                 for (int k = 0; k < WU; ++k) {
@@ -290,6 +309,7 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
                 uint32_t k32 = KM == 1 ? sad : (ham << 13) + sad;
                 if (k32 < bestk) { bestk = k32; bestr = r0 + r; }         // ascending rank: ties keep the smallest L
             }
+            __syncthreads();                                             // everyone is done with tile rt: its buffer may be refilled
         }
         if (has && bestr != 0xFFFFFFFFu) atomicMin(&key[slot], ((unsigned long long)bestk << 32) | bestr);
     }

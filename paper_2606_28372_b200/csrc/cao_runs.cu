@@ -76,11 +76,13 @@ static int launch_pick_nb(const SpaceMeta& sm, const uint8_t* cand, const uint32
     return CAO_OK;
 }
 static int launch_present(const SpaceMeta& sm, uint8_t* present, cudaStream_t st) {
-    CAO_CUDA(cudaMemsetAsync(present, 0, (size_t)CAO_MAX_DIMS * 256, st));
+    CAO_CUDA(cudaMemsetAsync(present, 0, (size_t)CAO_MAX_DIMS * 256 + 256, st));
     const unsigned grid = (unsigned)((sm.V + 255) / 256);
     if (sm.rowB == 16) k_present<4><<<grid, 256, 0, st>>>(sm, present);
     else k_present<8><<<grid, 256, 0, st>>>(sm, present);
     CAO_LAUNCHED("k_present");
+    k_all_present<<<1, 256, 0, st>>>(sm, present, (uint32_t*)(present + CAO_MAX_DIMS * 256));
+    CAO_LAUNCHED("k_all_present");
     return CAO_OK;
 }
 
@@ -274,7 +276,7 @@ static RunsLayout runs_layout(const SpaceMeta& sm, int algo, uint64_t P, uint64_
         L.rule = take(RP);
         L.key3 = take(paper && cont ? RP * 24 : 0);
         L.cnt3 = take(paper && algo == CAO_GA ? RP * 12 : 0);
-        L.present = take(paper ? (uint64_t)CAO_MAX_DIMS * 256 : 0);
+        L.present = take(paper ? (uint64_t)CAO_MAX_DIMS * 256 + 256 : 0);
     }
     L.total = off;
     return L;
@@ -612,7 +614,7 @@ static ModeScratch mode_scratch(const cao_space* s, uint64_t count) {
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { uint64_t o = off; off = align256(off + bytes); return o; };
     L.key = take(c * 8); L.key3 = take(c * 24); L.cnt3 = take(c * 12); L.wl = take(c * 4); L.wl_count = take(256);
-    L.rule = take(c); L.present = take((uint64_t)CAO_MAX_DIMS * 256); L.clean = take(c * (uint64_t)s->meta.rowB);
+    L.rule = take(c); L.present = take((uint64_t)CAO_MAX_DIMS * 256 + 256); L.clean = take(c * (uint64_t)s->meta.rowB);
     L.total = off;
     return L;
 }

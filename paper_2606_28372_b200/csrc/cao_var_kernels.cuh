@@ -20,6 +20,14 @@ __global__ void __launch_bounds__(256) k_present(const __grid_constant__ SpaceMe
         if (d < sm.n) present[d * 256 + ((w[d >> 2] >> ((d & 3) * 8)) & 0xFFu)] = 1;
 }
 
+// all_present[0] = 1 iff present[d][k] = 1 for every d < n, k < m_d (then adjacent == strictly adjacent, A28).
+static __global__ void k_all_present(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ present, uint32_t* all_present) {
+    bool ok = true;
+    for (int d = 0; d < sm.n; ++d) for (uint32_t k = threadIdx.x; k < sm.m[d]; k += blockDim.x) ok = ok && present[d * 256 + k];
+    const int any_missing = __syncthreads_or(!ok);
+    if (threadIdx.x == 0) all_present[0] = any_missing ? 0u : 1u;
+}
+
 // Where the continuous position of candidate `slot` lives: x(slot, d) = base[(slot / P) * blk + d * sd + (slot % P) * si].
 // Runs (state layout [run][dim][ind]): P = pop, blk = n * pop, sd = pop, si = 1.  Standalone rows: P = 1, blk = n, sd = 1.
 struct XAddr { const float* base; uint32_t P; uint64_t blk; uint32_t sd, si; };
@@ -31,17 +39,22 @@ __device__ __forceinline__ uint32_t nz_bytes(uint32_t x) {              // 0x80 
 // Membership of valid row v in the three neighbour sets of candidate c (L139-143): bit 0 strictly-adjacent (every
 // |delta index| <= 1), bit 1 adjacent (every index equal to c's or to the nearest present index below / above it, rows lo /
 // hi; a missing side repeats c's own index), bit 2 Hamming (exactly one parameter differs).  c is invalid, so v != c.
-template <int WU>
+// ADJ_IS_SA: every value of every parameter occurs in some valid configuration, so "adjacent" and "strictly adjacent" are
+// the same set (the nearest present index is the neighbouring one) and the lo / hi rows are not looked at.
+template <int WU, bool ADJ_IS_SA>
 __device__ __forceinline__ uint32_t nb_member(const uint32_t* c, const uint32_t* lo, const uint32_t* hi, const uint32_t* v) {
-    uint32_t far = 0, notadj = 0, ham = 0;
+    uint32_t far = 0, notadj = 0, hb = 0, ham = 0;
 #pragma unroll
     for (int k = 0; k < WU; ++k) {
         const uint32_t zc = nz_bytes(c[k] ^ v[k]);
         far |= __vabsdiffu4(c[k], v[k]) & 0xFEFEFEFEu;
-        notadj |= zc & nz_bytes(lo[k] ^ v[k]) & nz_bytes(hi[k] ^ v[k]);
-        ham += __popc(zc);
+        if (!ADJ_IS_SA) notadj |= zc & nz_bytes(lo[k] ^ v[k]) & nz_bytes(hi[k] ^ v[k]);
+        if ((k & 3) == 0 && k) { ham += __popc(hb); hb = 0; }
+        hb |= zc >> (k & 3);                                           // one POPC per four words
     }
-    return (far == 0 ? 1u : 0u) | (notadj == 0 ? 2u : 0u) | (ham == 1 ? 4u : 0u);
+    ham += __popc(hb);
+    const uint32_t sa = far == 0 ? 1u : 0u;
+    return sa | (ADJ_IS_SA ? sa << 1 : (notadj == 0 ? 2u : 0u)) | (ham == 1 ? 4u : 0u);
 }
 
 // lo / hi rows of candidate c from the presence table.
@@ -68,14 +81,12 @@ __device__ __forceinline__ void near_rows(const SpaceMeta& sm, const uint8_t* __
 // (squared Euclidean distance to the continuous position, fp32 bits << 32 | rank) into key3[slot][rule] (atomicMin:
 // order-free; distance >= 0, so bit patterns order like values; equal distances keep the smallest rank = smallest L).
 // KIND 1 (Alg.3): the number of members per rule into cnt3[slot][rule].
-template <int WU, int KIND>
-__global__ void __launch_bounds__(SCAN_TC) k_scan_nb(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
-                                                     const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
-                                                     const uint8_t* __restrict__ present, const XAddr xa,
-                                                     unsigned long long* key3, uint32_t* cnt3) {
+template <int WU, int KIND, bool ADJ_IS_SA>
+__device__ __forceinline__ void scan_nb_body(const SpaceMeta& sm, const uint8_t* __restrict__ cand_rows,
+                                             const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
+                                             const uint8_t* __restrict__ present, const XAddr& xa,
+                                             unsigned long long* key3, uint32_t* cnt3, uint4* tile, float* s_coord) {
     constexpr int ROWW = WU <= 4 ? 4 : 8;
-    __shared__ uint4 tile[SCAN_TR * (ROWW / 4)];
-    __shared__ float s_coord[256];
     const uint32_t count = *wl_count;
     if (count == 0 || sm.V == 0) return;
     const uint32_t tid = threadIdx.x;
@@ -94,7 +105,8 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan_nb(const __grid_constant__ Spa
         uint32_t c[ROWW], lo[ROWW], hi[ROWW];
         if (has) load_row_rw<ROWW>(cand_rows + (uint64_t)slot * (ROWW * 4), c);
         else { for (int k = 0; k < ROWW; ++k) c[k] = 0; }
-        near_rows<ROWW>(sm, present, c, lo, hi);
+        if (!ADJ_IS_SA) near_rows<ROWW>(sm, present, c, lo, hi);
+        else { for (int k = 0; k < ROWW; ++k) { lo[k] = c[k]; hi[k] = c[k]; } }
         float xr[WU * 4];
         if (KIND == 0) {
             const float* xp = xa.base + (uint64_t)(slot / xa.P) * xa.blk + (uint64_t)(slot % xa.P) * xa.si;
@@ -116,7 +128,7 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan_nb(const __grid_constant__ Spa
                 uint32_t v[ROWW];
                 { uint4 a = tile[r * (ROWW / 4)]; v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; }
                 if (ROWW == 8) { uint4 b = tile[r * 2 + 1]; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w; }
-                const uint32_t mem = nb_member<WU>(c, lo, hi, v);
+                const uint32_t mem = nb_member<WU, ADJ_IS_SA>(c, lo, hi, v);
                 if (mem && has) {                                       // rare: a neighbour under some rule
                     if (KIND == 0) {
                         float acc = 0.0f;
@@ -145,6 +157,19 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan_nb(const __grid_constant__ Spa
             }
         }
     }
+}
+
+// present[CAO_MAX_DIMS * 256] (one word, written by k_all_present) selects the specialisation, uniformly for the grid.
+template <int WU, int KIND>
+__global__ void __launch_bounds__(SCAN_TC) k_scan_nb(const __grid_constant__ SpaceMeta sm, const uint8_t* __restrict__ cand_rows,
+                                                     const uint32_t* __restrict__ wl, const uint32_t* __restrict__ wl_count,
+                                                     const uint8_t* __restrict__ present, const XAddr xa,
+                                                     unsigned long long* key3, uint32_t* cnt3) {
+    constexpr int ROWW = WU <= 4 ? 4 : 8;
+    __shared__ uint4 tile[SCAN_TR * (ROWW / 4)];
+    __shared__ float s_coord[256];
+    if (*(const uint32_t*)(present + CAO_MAX_DIMS * 256)) scan_nb_body<WU, KIND, true>(sm, cand_rows, wl, wl_count, present, xa, key3, cnt3, tile, s_coord);
+    else scan_nb_body<WU, KIND, false>(sm, cand_rows, wl, wl_count, present, xa, key3, cnt3, tile, s_coord);
 }
 
 // Alg.3: one warp per worklist candidate.  The first non-empty rule (counts of k_scan_nb<.,1>) has K members;
@@ -177,7 +202,7 @@ __global__ void __launch_bounds__(256) k_pick_nb(const __grid_constant__ SpaceMe
             const uint32_t r = base + lane;
             uint32_t v[ROWW];
             load_row<ROWW>(sm.rows + (uint64_t)(r < sm.V ? r : base) * (ROWW * 4), v);
-            const bool mem = r < sm.V && ((nb_member<WU>(c, lo, hi, v) >> rule) & 1u);
+            const bool mem = r < sm.V && ((nb_member<WU, false>(c, lo, hi, v) >> rule) & 1u);
             const uint32_t bal = __ballot_sync(0xFFFFFFFFu, mem), n_here = (uint32_t)__popc(bal);
             if (pick < n_here) { found = base + (uint32_t)kth_set_bit32(bal, pick); break; }
             pick -= n_here;
