@@ -386,7 +386,7 @@ int cao_runs_create_ex(const cao_space* s, int32_t algo, const cao_hparams* hp, 
     if (r->var_on) r->mode = 0;                                         // SURVEY 8(f) variants run through the phased pipeline
     const size_t P = (size_t)pop, n = (size_t)s->meta.n;
     r->smem_init = P * 4;
-    r->smem_op = algo == CAO_GA ? P * 16 : algo == CAO_FIREFLY ? (P * n + P) * 4 : 0;
+    r->smem_op = algo == CAO_GA ? P * 16 : algo == CAO_FIREFLY ? (P * n + 2 * P) * 4 : 0;
     r->smem_fin = algo == CAO_DE ? P * 16 : 0;
     int rc2 = CAO_OK;
     do {

@@ -306,6 +306,7 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
     const uint32_t i = threadIdx.x, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
     const uint64_t q = (uint64_t)k * P + i;
+    uint64_t qt = q;                                                    // slot of the candidate this thread produces (Firefly remaps)
     uint32_t w[ROWW];
 #pragma unroll
     for (int z = 0; z < ROWW; ++z) w[z] = 0;
@@ -476,17 +477,31 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
     } else {                                                            // O7: Firefly (Yang's rule, synchronous)
         float* s_xo = (float*)s_dyn;                                    // [j][d]
         float* s_fo = s_xo + (size_t)P * n;                             // [j]
+        uint32_t* s_ord = (uint32_t*)(s_fo + P);                        // [brightness rank] -> firefly
         for (uint32_t e = i; e < P * (uint32_t)n; e += blockDim.x) {
             uint32_t j = e / n, d = e - j * n;
             s_xo[e] = rm.x[((uint64_t)k * n + d) * P + j];
         }
         if (i < P) s_fo[i] = rm.f[q];
         __syncthreads();
+        // Thread i takes the firefly of brightness RANK i (ties by index), not firefly i: a warp then holds fireflies of
+        // similar brightness, so for most attractors j its lanes agree on "j is brighter" -- whole warps skip the attractors
+        // dimmer than all their fireflies instead of idling half their lanes.  The update of a firefly does not depend on
+        // which thread computes it (draws are addressed by the firefly's index).
         if (i < P) {
+            const float fme = s_fo[i];
+            uint32_t pos = 0;
+            for (uint32_t j = 0; j < P; ++j) { const float fj = s_fo[j]; pos += (fj < fme) || (fj == fme && j < i); }
+            s_ord[pos] = i;
+        }
+        __syncthreads();
+        if (i < P) {
+            const uint32_t me = s_ord[i];
+            qt = (uint64_t)k * P + me;
             float xi[ROWW * 4];
 #pragma unroll
-            for (int d = 0; d < ROWW * 4; ++d) xi[d] = d < n ? s_xo[i * n + d] : 0.0f;
-            const float fi = s_fo[i];
+            for (int d = 0; d < ROWW * 4; ++d) xi[d] = d < n ? s_xo[me * n + d] : 0.0f;
+            const float fi = s_fo[me];
             for (uint32_t j = 0; j < P; ++j) {
                 if (!(s_fo[j] < fi)) continue;                          // only brighter (cheaper) fireflies attract
                 const float* xj = s_xo + (size_t)j * n;
@@ -503,7 +518,7 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
                 for (int qb = 0; qb < ROWW + 1; ++qb) {
                     uint4 rr = make_uint4(0, 0, 0, 0);
                     if ((uint32_t)(qb * 4) < o + (uint32_t)n)
-                        rr = philox4x32_10(make_uint4(run, g, i, (S_OP << 24) | (b0 + qb)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
+                        rr = philox4x32_10(make_uint4(run, g, me, (S_OP << 24) | (b0 + qb)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
                     nw[qb * 4] = rr.x; nw[qb * 4 + 1] = rr.y; nw[qb * 4 + 2] = rr.z; nw[qb * 4 + 3] = rr.w;
                 }
 #pragma unroll
@@ -522,13 +537,13 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
             for (int d = 0; d < ROWW * 4; ++d) {
                 if (d < n) {
                     float xx = clamp_pos(xi[d], coord_M(sm.M, (int)sm.m[d] - 1));
-                    rm.x[((uint64_t)k * n + d) * P + i] = xx;
+                    rm.x[((uint64_t)k * n + d) * P + me] = xx;
                     w[d >> 2] |= (uint32_t)snap_M(sm.M, (int)sm.m[d], xx) << ((d & 3) * 8);
                 }
             }
         }
     }
-    if (i < P) candidate_tail<ROWW>(sm, rm, q, w, wl, wl_count, count_scans, sh, use_cache);
+    if (i < P) candidate_tail<ROWW>(sm, rm, qt, w, wl, wl_count, count_scans, sh, use_cache);
     __syncthreads();
     if (i == 0 && sh.n_inv) atomicAdd(&rm.counters[0], (unsigned long long)sh.n_inv);
 }
