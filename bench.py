@@ -299,14 +299,13 @@ def gpu_arm(args):
     kept_w = None
     for _ in range(args.warmup):
         kept_w = one_step(False)
+    kept_w = None                                                         # both sets go back to the allocator's cache
     torch.cuda.synchronize()
     import gc
     gc.collect(); gc.disable()                                            # no cyclic-GC pause inside a timed step
     sampler = ClockSampler(local); sampler.start()
     ms, wall, _, launches, kept = timed(args.steps, False, False)
     sampler.stop_flag = True; sampler.join(timeout=2)
-    # per-kernel device times: the same step, serialised on one stream, events around every launch
-    ms_prof, _, prof, _, _ = timed(args.steps, False, True, concurrent=False)
     space, runs = kept
     stats = [r.stats() for r in runs]
     cands_step = sum(c["n_evaluated"] for c in stats)
@@ -314,13 +313,17 @@ def gpu_arm(args):
     repaired_step = sum(c["n_repaired"] for c in stats)
     gens_done = [int(r.best()["gens_done"].sum().item()) for r in runs]
     value = world * cands_step * args.steps / (ms / 1e3)
+    del space, runs, kept                                                 # never more than two buffer sets alive (see the warm-up)
+    # per-kernel device times: the same step, serialised on one stream, events around every launch
+    ms_prof, _, prof, _, _ = timed(args.steps, False, True, concurrent=False)
 
     for _ in range(max(args.warmup, 2)):
         kept_w = one_step(True)
+    kept_w = None
     torch.cuda.synchronize()
     ms_e, wall_e, _, _, _ = timed(args.steps, True, False)
     value_e = world * cands_step * args.steps / (ms_e / 1e3)
-    gc.enable(); del kept_w
+    gc.enable()
     h2d = obj.nbytes + sum(len(d) * 8 for d in sp.domains) + sum(len(p) * 4 for p in sp.rpn)
     d2h = len(wl["algos"]) * 16 * R + 8
 
