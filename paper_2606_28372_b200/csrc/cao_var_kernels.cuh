@@ -43,17 +43,19 @@ __device__ __forceinline__ uint32_t nz_bytes(uint32_t x) {              // 0x80 
 // the same set (the nearest present index is the neighbouring one) and the lo / hi rows are not looked at.
 template <int WU, bool ADJ_IS_SA>
 __device__ __forceinline__ uint32_t nb_member(const uint32_t* c, const uint32_t* lo, const uint32_t* hi, const uint32_t* v) {
-    uint32_t far = 0, notadj = 0, hb = 0, ham = 0;
+    // strictly adjacent <=> every differing byte differs by exactly 1 <=> sum |delta| == number of differing bytes: one
+    // VABSDIFF4 with accumulate per word (as in k_scan) instead of a per-byte absolute difference
+    uint32_t sad = 0, notadj = 0, hb = 0, ham = 0;
 #pragma unroll
     for (int k = 0; k < WU; ++k) {
         const uint32_t zc = nz_bytes(c[k] ^ v[k]);
-        far |= __vabsdiffu4(c[k], v[k]) & 0xFEFEFEFEu;
+        sad = sad4_acc(c[k], v[k], sad);
         if (!ADJ_IS_SA) notadj |= zc & nz_bytes(lo[k] ^ v[k]) & nz_bytes(hi[k] ^ v[k]);
         if ((k & 3) == 0 && k) { ham += __popc(hb); hb = 0; }
         hb |= zc >> (k & 3);                                           // one POPC per four words
     }
     ham += __popc(hb);
-    const uint32_t sa = far == 0 ? 1u : 0u;
+    const uint32_t sa = sad == ham ? 1u : 0u;
     return sa | (ADJ_IS_SA ? sa << 1 : (notadj == 0 ? 2u : 0u)) | (ham == 1 ? 4u : 0u);
 }
 
