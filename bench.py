@@ -36,8 +36,8 @@ N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum per k_gen launch of THIS workload (configs[1], 1000 runs per algorithm),
 # mean of the four launches of one step: a STORED constant from the ncu --set full capture summarised in
 # profiles/r2_kgen.md (it does not change with the run; the live numbers of this line are the CUDA-event times).
-NCU_KGEN_DRAM_BYTES_PER_LAUNCH = None
-NCU_KGEN_SOURCE = "profiles/r2_kgen.md"
+NCU_KGEN_DRAM_BYTES_PER_LAUNCH = 17.2e6
+NCU_KGEN_SOURCE = "profiles/r2b_kgen.md"
 SECTOR_BYTES_PER_CANDIDATE = 204          # state 2(n+8) + bitmap 32 + directory 32 + obj 32 + dedup 64
 
 

@@ -62,31 +62,42 @@ static __device__ __noinline__ uint32_t valid_rank(const uint64_t* __restrict__ 
 
 // Group-cooperative Hamming-1 probe (exact: Hamming is the primary key, |delta| the secondary, L the third).  The
 // `nopen` open candidates (list ol, linear indices Lc, rows8 = the group's candidate rows, RB bytes each) times their NB
-// neighbours form one flat index space that the threads stride over, four independent bit tests in flight each; hits
-// go to hkey[candidate] with a shared-memory atomicMin on (|delta| << 40 | L').  The caller synchronises afterwards.
+// neighbours form one flat index space that the threads stride over, four independent bit tests in flight each.  A hit
+// goes to the LOW WORD of hkey[candidate] with a native 32-bit shared-memory atomicMin on |delta| << 8 | ord (a 64-bit
+// shared atomicMin is a compare-and-swap loop).  ord orders the neighbours of one candidate that share |delta| = s exactly
+// like their linear indices L' = L -+ s * stride_d: the negative steps first (larger stride = smaller dimension first:
+// ord = d), then the positive steps (smaller stride first: ord = 63 - d); h1_decode rebuilds (|delta|, L').  hkey[.] must
+// hold ~0 on entry.  The caller synchronises afterwards.
 template <int RB>
 __device__ __forceinline__ void probe_h1_flat(const Grp& g, const uint64_t* __restrict__ bitmap, const CtaTabs& tb, const uint8_t* rows8,
                                               const uint32_t* ol, const uint64_t* Lc, unsigned long long* hkey, uint32_t nopen) {
     const uint32_t NB = tb.NB, total = nopen * NB;
     uint32_t jj = g.t / NB, t = g.t - jj * NB;
     const uint32_t sj = g.G / NB, st = g.G - sj * NB;
+    uint32_t* hk32 = (uint32_t*)hkey;
     for (uint32_t q0 = g.t; q0 < total; q0 += 4 * g.G) {
-        uint64_t Lp[4]; uint32_t sd[4], who[4]; bool bit[4];
+        uint32_t kv[4], who[4]; bool bit[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const bool live = q0 + u * g.G < total;
             const uint32_t i2 = ol[live ? jj : 0], e = tb.nb[live ? t : 0], d = e >> 8, kq = e & 255u, cd = rows8[(size_t)i2 * RB + d];
             const int dv = (int)(kq + (kq >= cd)) - (int)cd;
-            Lp[u] = Lc[i2] + (int64_t)dv * (int64_t)tb.stride[d];
-            sd[u] = (uint32_t)abs(dv); who[u] = i2;
-            bit[u] = bit_test(bitmap, Lp[u]) && live;
+            kv[u] = ((uint32_t)abs(dv) << 8) | (dv < 0 ? d : 63u - d); who[u] = i2;
+            bit[u] = bit_test(bitmap, Lc[i2] + (int64_t)dv * (int64_t)tb.stride[d]) && live;
             t += st; jj += sj;
             if (t >= NB) { t -= NB; ++jj; }
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u)
-            if (bit[u]) atomicMin(&hkey[who[u]], (unsigned long long)(((uint64_t)sd[u] << 40) | Lp[u]));
+            if (bit[u]) atomicMin(&hk32[2 * who[u]], kv[u]);
     }
+}
+// (|delta|, L') of the winning neighbour from the reduced word m != ~0 of a candidate with linear index L.
+__device__ __forceinline__ uint64_t h1_decode(const CtaTabs& tb, uint32_t m, uint64_t L, uint32_t* sad) {
+    const uint32_t sdv = m >> 8, ord = m & 63u, d = ord < 32u ? ord : 63u - ord;
+    const uint64_t step = (uint64_t)sdv * tb.stride[d];
+    *sad = sdv;
+    return ord < 32u ? L - step : L + step;
 }
 
 // Group-cooperative brute-force scan of the whole valid table for up to NB candidates (rows in shared memory); the
@@ -587,10 +598,11 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             probe_h1_flat<RB>(g, sm.bitmap, tb, (const uint8_t*)S.cand, ol, S.Lc, hkey, nopen);
             g.sync();
             if (open) {
-                const uint64_t hit = hkey[i];
-                if (hit != ~0ull) {
-                    uint32_t dummy;
-                    key = make_key(1u, (uint32_t)(hit >> 40), valid_rank(sm.bitmap, sm.dir, hit & ((1ull << 40) - 1), &dummy));
+                const uint32_t hit = (uint32_t)hkey[i];
+                if (hit != 0xFFFFFFFFu) {
+                    uint32_t dummy, sadv;
+                    const uint64_t Lh = h1_decode(tb, hit, L, &sadv);
+                    key = make_key(1u, sadv, valid_rank(sm.bitmap, sm.dir, Lh, &dummy));
                 }
             }
         }
