@@ -502,8 +502,15 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             uint32_t nw[(ROWW + 1) * 4];
             {
                 uint4 q5[ROWW + 1];
-                if (ROWW == 4) philox4x32_10_multi<ROWW + 1>(make_uint4(run, gen, i, (S_OP << 24) | (s0 >> 2)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), q5);
-                else {
+                if (ROWW == 4) {                                        // four blocks cover slots o .. o+15; the fifth only when o + n > 16
+                    uint4 q4[4];
+                    philox4x32_10_multi<4>(make_uint4(run, gen, i, (S_OP << 24) | (s0 >> 2)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), q4);
+#pragma unroll
+                    for (int z = 0; z < 4; ++z) q5[z] = q4[z];
+                    q5[4] = make_uint4(0, 0, 0, 0);
+                    if (o + (uint32_t)n > 16u)                          // warp-uniform
+                        q5[4] = philox4x32_10(make_uint4(run, gen, i, (S_OP << 24) | ((s0 >> 2) + 4)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
+                } else {
                     uint4 qa[5], qb[4];
                     philox4x32_10_multi<5>(make_uint4(run, gen, i, (S_OP << 24) | (s0 >> 2)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), qa);
                     philox4x32_10_multi<4>(make_uint4(run, gen, i, (S_OP << 24) | ((s0 >> 2) + 5)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32), qb);
