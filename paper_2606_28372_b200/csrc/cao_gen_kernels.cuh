@@ -894,7 +894,10 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
 
 // ---------------------------------------------------------------------------------------------
 template <int ALGO, int ROWW, int MAXT>
-__global__ void __launch_bounds__(MAXT, MAXT == 256 ? 3 : 1)
+// Resident CTAs per SM (register budget), measured on the 10^5-run sweep: PSO and Firefly keep their per-dimension state and
+// Philox chains in registers and run 8 % faster with 128 registers x 2 CTAs than with 80 x 3 (which spills ~140 bytes per
+// thread); DE and GA are 8 % / 4 % faster with 3 CTAs.  64 registers x 4 CTAs lost everywhere (spills).
+__global__ void __launch_bounds__(MAXT, MAXT == 256 ? ((ALGO == CAO_PSO || ALGO == CAO_FIREFLY) ? 2 : 3) : 1)
 k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm, const __grid_constant__ RunsMeta rm,
       const __grid_constant__ GenLayout lay, uint32_t g_first, uint32_t n_gens) {
     extern __shared__ __align__(16) uint32_t s_dyn[];
