@@ -168,14 +168,17 @@ def reference_arm(args):
         return
     wl = workload(args.config, None)
     sp = wl["space"]
-    sample = oracle_sample_text(wl, args.ref_runs)
+    # bounded sample: one step = the full space build (~0.7 s on configs[1]) + R_o runs of every algorithm (~6.6 s per run of
+    # the four); R_o is cut so that (steps + 1 warm-up) steps end within about three minutes
+    R_o = max(1, min(args.ref_runs, int((170.0 / (args.steps + 1) - 0.7) / 6.6)))
+    sample = oracle_sample_text(wl, R_o)
     obj = oracle_prepare(wl)
     with PinnedToOneCore():
         for _ in range(min(args.warmup, 1)):
-            oracle_sample_step(wl, args.ref_runs, obj)
+            oracle_sample_step(wl, R_o, obj)
         tot_c, tot_t = 0, 0.0
         for _ in range(args.steps):
-            c, t = oracle_sample_step(wl, args.ref_runs, obj)
+            c, t = oracle_sample_step(wl, R_o, obj)
             tot_c += c; tot_t += t
     val = tot_c / tot_t
     line = {"impl": "reference", "metric": "candidates_repaired_evaluated_per_s", "value": val, "unit": "candidates/s",

@@ -314,6 +314,11 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     // fork: the zero fill of the bitmap (N/8 bytes, HBM-bound) overlaps the table build (latency-bound)
     CAO_CUDA(cudaEventRecord(s->ev_fork, st));
     CAO_CUDA(cudaStreamWaitEvent(s->side, s->ev_fork, 0));
+    if (s->use_lut) {                                                   // the inner-digit LUT (needed by k_fill only) is off the critical path too
+        ProfScope ps(PK_TABLE, s->side);
+        k_inner_lut<<<(unsigned)((s->B + 255) / 256), 256, 0, s->side>>>(s->meta, (uint32_t*)(sc + s->off_lut), s->B, s->t, s->meta.rowB / 4);
+        CAO_LAUNCHED("k_inner_lut");
+    }
     CAO_CUDA(cudaMemsetAsync(d_bitmap, 0, s->bitmap_bytes, s->side));
     CAO_CUDA(cudaMemsetAsync(sc + s->off_V, 0, (s->off_cnt - s->off_V) + (s->nd + 1) * 4, s->side));   // V, tickets, counts
     for (int k = 0; k < s->n_rc; ++k) {                                 // class tables start empty
@@ -334,11 +339,6 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         if (tsm > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_build_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
         k_build_tables<<<grid, 256, tsm, st>>>(s->meta, d_dom, d_desc, d_tables, d_flags, s->B, s->Wb, s->t, ci_cap);
         CAO_LAUNCHED("k_build_tables");
-    }
-    if (s->use_lut) {
-        ProfScope ps(PK_TABLE, st);
-        k_inner_lut<<<(unsigned)((s->B + 255) / 256), 256, 0, st>>>(s->meta, (uint32_t*)(sc + s->off_lut), s->B, s->t, s->meta.rowB / 4);
-        CAO_LAUNCHED("k_inner_lut");
     }
     CAO_CUDA(cudaStreamWaitEvent(st, s->ev_join, 0));                   // join
     uint32_t* ctl = (uint32_t*)(sc + s->off_V);                         // [0..1] V, [2] scan ticket, [3] live count, [4] group count
