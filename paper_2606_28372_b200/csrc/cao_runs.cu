@@ -410,7 +410,8 @@ int cao_runs_create_ex(const cao_space* s, int32_t algo, const cao_hparams* hp, 
             if ((rc2 = launch_scan(r->sm, m.cand, levels >= 2 ? m.wl2 : m.wl, levels >= 2 ? m.wl2_count : m.wl_count, m.key, true, st))) break;
         }
 #define CALL_INIT(A, W) \
-        if (r->smem_op > 48 * 1024) cudaFuncSetAttribute(k_op<A, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
+        if (r->smem_op > 48 * 1024) { cudaFuncSetAttribute(k_op<A, W, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
+                                      cudaFuncSetAttribute(k_op<A, W, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); } \
         k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
         { ProfScope ps(PK_INIT, st); DISPATCH_ALGO_ROWW(algo, s->meta.rowB / 4, CALL_INIT); }
         ++g_cao_launches;
@@ -464,7 +465,8 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
     for (uint32_t it = 0; it < n_generations; ++it) {
         if (r->gen >= r->rm.max_gens) break;                            // g <= max_gens (O10)
         const uint32_t g = r->gen + 1;
-#define CALL_OP(A, W) k_op<A, W><<<r->rm.R, r->block, r->smem_op, st>>>(r->sm, r->rm, g)
+#define CALL_OP(A, W) if (r->block <= 256) k_op<A, W, 256><<<r->rm.R, r->block, r->smem_op, st>>>(r->sm, r->rm, g); \
+                      else k_op<A, W, 1024><<<r->rm.R, r->block, r->smem_op, st>>>(r->sm, r->rm, g)
         { ProfScope ps(PK_OP, st); DISPATCH_ALGO_ROWW(algo, roww, CALL_OP); }
         CAO_LAUNCHED("k_op");
         int rc = CAO_OK;

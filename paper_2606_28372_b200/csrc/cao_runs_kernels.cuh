@@ -514,12 +514,31 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
                 // front as independent chains, then word (o + d) is picked with selects (o = first slot & 3)
                 const uint32_t s0 = j * (uint32_t)n, b0 = s0 >> 2, o = s0 & 3;
                 uint32_t nw[(ROWW + 1) * 4];
+                {   // interleaved chains (the warp that holds the dimmest fireflies runs alone at the end of the launch:
+                    // its latency, not the issue rate, decides the kernel time)
+                    const uint32_t nblk = (o + (uint32_t)n + 3) >> 2;   // blocks that hold slots o .. o+n-1
+                    const uint32_t k0 = (uint32_t)rm.seed, k1 = (uint32_t)(rm.seed >> 32);
+                    uint4 q[ROWW + 1];
 #pragma unroll
-                for (int qb = 0; qb < ROWW + 1; ++qb) {
-                    uint4 rr = make_uint4(0, 0, 0, 0);
-                    if ((uint32_t)(qb * 4) < o + (uint32_t)n)
-                        rr = philox4x32_10(make_uint4(run, g, me, (S_OP << 24) | (b0 + qb)), (uint32_t)rm.seed, (uint32_t)(rm.seed >> 32));
-                    nw[qb * 4] = rr.x; nw[qb * 4 + 1] = rr.y; nw[qb * 4 + 2] = rr.z; nw[qb * 4 + 3] = rr.w;
+                    for (int z = 0; z < ROWW + 1; ++z) q[z] = make_uint4(0, 0, 0, 0);
+                    constexpr int K1 = ROWW == 4 ? 4 : 5;
+                    {
+                        uint4 qa[K1];
+                        philox4x32_10_multi<K1>(make_uint4(run, g, me, (S_OP << 24) | b0), k0, k1, qa);
+#pragma unroll
+                        for (int z = 0; z < K1; ++z) q[z] = qa[z];
+                    }
+                    if (nblk > (uint32_t)K1) {
+                        if (ROWW == 4 || nblk == (uint32_t)K1 + 1) q[K1] = philox4x32_10(make_uint4(run, g, me, (S_OP << 24) | (b0 + K1)), k0, k1);
+                        else {
+                            uint4 qb4[4];
+                            philox4x32_10_multi<4>(make_uint4(run, g, me, (S_OP << 24) | (b0 + K1)), k0, k1, qb4);
+#pragma unroll
+                            for (int z = 0; z < 4; ++z) if (K1 + z < ROWW + 1) q[K1 + z] = qb4[z];
+                        }
+                    }
+#pragma unroll
+                    for (int z = 0; z < ROWW + 1; ++z) { nw[z * 4] = q[z].x; nw[z * 4 + 1] = q[z].y; nw[z * 4 + 2] = q[z].z; nw[z * 4 + 3] = q[z].w; }
                 }
 #pragma unroll
                 for (int d = 0; d < ROWW * 4; ++d) {
@@ -548,8 +567,9 @@ __device__ __forceinline__ void gen_op(const SpaceMeta& sm, const RunsMeta& rm, 
     if (i == 0 && sh.n_inv) atomicAdd(&rm.counters[0], (unsigned long long)sh.n_inv);
 }
 
-template <int ALGO, int ROWW>
-__global__ void __launch_bounds__(1024) k_op(const __grid_constant__ SpaceMeta sm, const __grid_constant__ RunsMeta rm, uint32_t g) {
+// MAXT: 256 (populations up to 256: the register budget is not capped at 64) or 1024.
+template <int ALGO, int ROWW, int MAXT>
+__global__ void __launch_bounds__(MAXT) k_op(const __grid_constant__ SpaceMeta sm, const __grid_constant__ RunsMeta rm, uint32_t g) {
     extern __shared__ uint32_t s_dyn[];
     __shared__ RunShared sh;
     const uint32_t k = blockIdx.x;
