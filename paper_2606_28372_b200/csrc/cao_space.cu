@@ -375,13 +375,13 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
             k_enum<<<(unsigned)((threads + bd - 1) / bd), bd, smem_enum, st>>>(s->meta, ea);
         }
         CAO_LAUNCHED("k_enum");
-        if (s->use_keys) {
-            k_keys<<<(unsigned)std::min<uint64_t>((s->n_blocks + bd - 1) / bd, 148ull * 4), bd, smem_dig, st>>>(s->meta, ea);
-            CAO_LAUNCHED("k_keys");
-        }
         if (s->n_res) {                                                 // fork: the residual prefixes need the live list only
             CAO_CUDA(cudaEventRecord(s->ev_fork2, st));
             CAO_CUDA(cudaStreamWaitEvent(s->side2, s->ev_fork2, 0));
+        }
+        if (s->use_keys) {
+            k_keys<<<(unsigned)std::min<uint64_t>((s->n_blocks + bd - 1) / bd, 148ull * 4), bd, smem_dig, st>>>(s->meta, ea);
+            CAO_LAUNCHED("k_keys");
         }
         ProfScope ps(PK_PROBE, st);
         const uint64_t items = s->n_blocks * (uint64_t)s->Wb;
