@@ -556,3 +556,71 @@ __global__ void __launch_bounds__(256) k_cnt_apply(const uint32_t* __restrict__ 
         if (v[k]) groups[gbase++] = (uint32_t)(base + k);
     }
 }
+
+// Single-pass variant for cao_space_rebuild (the table address is known, so the two halves need no host round trip between
+// them): decoupled look-back over the chunk sums.  CTAs take chunk numbers from a ticket (so every predecessor has started),
+// publish state[b] = flag << 62 | value (flag 1: the chunk's own sum, 2: the inclusive prefix) and walk back over their
+// predecessors until they meet an inclusive prefix.  state[] and the ticket must be zero on entry.  Same outputs as
+// k_cnt_reduce + k_cnt_apply: directory, list of non-empty groups, V.
+__global__ void __launch_bounds__(256) k_cnt_scan1(const uint32_t* __restrict__ cnt, uint64_t nd, unsigned long long* state, uint32_t* ticket,
+                                                   uint32_t* dir, uint32_t* groups, uint32_t* group_count, uint64_t* V_out) {
+    __shared__ uint32_t ws[8];
+    __shared__ uint32_t s_b;
+    __shared__ unsigned long long s_excl;
+    if (threadIdx.x == 0) s_b = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const uint32_t b = s_b;
+    const uint64_t base = (uint64_t)b * SCAN_CHUNK + threadIdx.x * 16;
+    uint32_t v[16], s = 0;
+    if (base + 16 <= nd) {
+        const uint4* q = (const uint4*)(cnt + base);
+        const uint4 a0 = q[0], a1 = q[1], a2 = q[2], a3 = q[3];
+        v[0] = a0.x; v[1] = a0.y; v[2] = a0.z; v[3] = a0.w; v[4] = a1.x; v[5] = a1.y; v[6] = a1.z; v[7] = a1.w;
+        v[8] = a2.x; v[9] = a2.y; v[10] = a2.z; v[11] = a2.w; v[12] = a3.x; v[13] = a3.y; v[14] = a3.z; v[15] = a3.w;
+    } else {
+        for (int k = 0; k < 16; ++k) v[k] = (base + k < nd) ? cnt[base + k] : 0;
+    }
+    for (int k = 0; k < 16; ++k) s += v[k];
+    uint32_t inc = s;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o); if ((threadIdx.x & 31) >= o) inc += t; }
+    if ((threadIdx.x & 31) == 31) ws[threadIdx.x >> 5] = inc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long total = 0;
+        for (int k = 0; k < 8; ++k) total += ws[k];
+        volatile unsigned long long* vs = state;
+        if (b == 0) { vs[0] = (2ull << 62) | total; s_excl = 0; }
+        else {
+            vs[b] = (1ull << 62) | total;
+            __threadfence();
+            unsigned long long excl = 0;
+            for (uint32_t j = b; j-- > 0;) {
+                unsigned long long e;
+                do { e = vs[j]; } while ((e >> 62) == 0);
+                excl += e & ((1ull << 62) - 1);
+                if ((e >> 62) == 2) break;
+            }
+            vs[b] = (2ull << 62) | (excl + total);
+            s_excl = excl;
+        }
+        __threadfence();
+        if (b + 1 == gridDim.x) { *V_out = s_excl + total; *ticket = 0; }
+    }
+    __syncthreads();
+    uint32_t off = (uint32_t)s_excl;
+    for (uint32_t k = 0; k < (threadIdx.x >> 5); ++k) off += ws[k];
+    off += inc - s;
+    uint32_t mine = 0;
+    for (int k = 0; k < 16; ++k) mine += v[k] != 0;
+    uint32_t incl = mine;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xFFFFFFFFu, incl, o); if ((threadIdx.x & 31) >= o) incl += t; }
+    const uint32_t totalg = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    uint32_t gbase = 0;
+    if ((threadIdx.x & 31) == 0 && totalg) gbase = atomicAdd(group_count, totalg);
+    gbase = __shfl_sync(0xFFFFFFFFu, gbase, 0) + incl - mine;
+    for (int k = 0; k < 16; ++k) {
+        if (base + k < nd) dir[base + k] = off;
+        off += v[k];
+        if (v[k]) groups[gbase++] = (uint32_t)(base + k);
+    }
+}

@@ -276,7 +276,7 @@ static int plan_space(cao_space* s) {
     s->off_flags = off; off = align256(off + std::max<uint64_t>(1, total_flags));
     s->off_lut = off; off = align256(off + (s->use_lut ? B * (uint64_t)M.rowB : 1));
     s->n_part = (s->nd + 1 + SCAN_CHUNK - 1) / SCAN_CHUNK;
-    s->off_part = off; off = align256(off + s->n_part * 4);
+    s->off_part = off; off = align256(off + s->n_part * 8);      // chunk sums (u32) / look-back states (u64)
     s->off_V = off; off = align256(off + 32);                     // V (u64), scan ticket, live count, group count
     s->off_cnt = off; off = align256(off + (s->nd + 1) * 4);
     s->off_live = off; off = align256(off + s->n_blocks * 4);
@@ -301,7 +301,7 @@ int cao_space_build_workspace_bytes(cao_space* s, uint64_t* bitmap_bytes, uint64
 
 // S1 pass 1 on `st`: zero fill (side stream) || constraint tables, then block masks -> bitmap + per-512 counts,
 // residual constraints on the survivors, and the first half of the count scan (V).
-static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t st) {
+static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t st, bool with_reduce = true) {
     if (!s->side) {
         CAO_CUDA(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
         CAO_CUDA(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
@@ -320,7 +320,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         CAO_LAUNCHED("k_inner_lut");
     }
     CAO_CUDA(cudaMemsetAsync(d_bitmap, 0, s->bitmap_bytes, s->side));
-    CAO_CUDA(cudaMemsetAsync(sc + s->off_V, 0, (s->off_cnt - s->off_V) + (s->nd + 1) * 4, s->side));   // V, tickets, counts
+    CAO_CUDA(cudaMemsetAsync(sc + s->off_part, 0, (s->off_cnt - s->off_part) + (s->nd + 1) * 4, s->side));   // scan states, V, tickets, counts
     for (int k = 0; k < s->n_rc; ++k) {                                 // class tables start empty
         uint8_t* b = sc + s->off_rc[k];
         CAO_CUDA(cudaMemsetAsync(b, 0x80, (uint64_t)CAO_HS * 8, s->side));
@@ -408,7 +408,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         k_residual<<<(unsigned)((warps + 7) / 8), bd, smem_desc, st>>>(s->meta, ea, pre);
         CAO_LAUNCHED("k_residual");
     }
-    {
+    if (with_reduce) {
         ProfScope ps(PK_CSCAN, st);
         k_cnt_reduce<<<(unsigned)s->n_part, 256, 0, st>>>(ea.cnt, s->nd + 1, (uint32_t*)(sc + s->off_part), s->n_part, ctl + 2, (uint64_t*)ctl);
         CAO_LAUNCHED("k_cnt_reduce");
@@ -417,14 +417,18 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
 }
 
 // S1 pass 2 on `st`: rank directory + list of non-empty groups, then rows and Ltab.
-static int launch_fill(cao_space* s, uint8_t* tb, cudaStream_t st) {
+static int launch_fill(cao_space* s, uint8_t* tb, cudaStream_t st, bool single_pass = false) {
     uint8_t* sc = (uint8_t*)s->d_scratch;
     uint8_t* rows = tb + s->off_rows; void* Ltab = tb + s->off_Ltab; uint32_t* dir = (uint32_t*)(tb + s->off_dir);
     const uint32_t* cnt = (const uint32_t*)(sc + s->off_cnt);
     uint32_t* ctl = (uint32_t*)(sc + s->off_V);
     uint32_t* groups = (uint32_t*)(sc + s->off_groups);
     CAO_CUDA(cudaMemsetAsync(ctl + 4, 0, 4, st));
-    {
+    if (single_pass) {                                                  // rebuild: reduce + apply in one decoupled-look-back pass
+        ProfScope ps(PK_CSCAN, st);
+        k_cnt_scan1<<<(unsigned)s->n_part, 256, 0, st>>>(cnt, s->nd + 1, (unsigned long long*)(sc + s->off_part), ctl + 2, dir, groups, ctl + 4, (uint64_t*)ctl);
+        CAO_LAUNCHED("k_cnt_scan1");
+    } else {
         ProfScope ps(PK_CSCAN, st);
         k_cnt_apply<<<(unsigned)s->n_part, 256, 0, st>>>(cnt, s->nd + 1, (const uint32_t*)(sc + s->off_part), dir, groups, ctl + 4);
         CAO_LAUNCHED("k_cnt_apply");
@@ -549,11 +553,14 @@ int cao_space_rebuild(cao_space* s, void* stream) {
     // once into a CUDA graph and replayed.  Not on the legacy default stream (capture is illegal there) and not while
     // per-kernel profiling is on (its events must be real).
     const bool can_graph = st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread && !g_cao_prof_on.load();
+    // count scan: one look-back pass while the chain of chunks is short (measured: 2 us faster on configs[1] / [2], 4 us
+    // slower on configs[3]'s 274 chunks than reduce + apply)
+    const bool single = s->n_part <= 32;
     if (can_graph && !s->rebuild_exec) {
         const uint64_t l0 = g_cao_launches.load();
         if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-            int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st);
-            if (!rc) rc = launch_fill(s, (uint8_t*)s->d_table, st);
+            int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st, !single);
+            if (!rc) rc = launch_fill(s, (uint8_t*)s->d_table, st, single);
             cudaGraph_t graph = nullptr;
             const cudaError_t e = cudaStreamEndCapture(st, &graph);
             if (!rc && e == cudaSuccess && graph && cudaGraphInstantiate(&s->rebuild_exec, graph, 0) == cudaSuccess)
@@ -569,9 +576,9 @@ int cao_space_rebuild(cao_space* s, void* stream) {
         g_cao_launches += s->rebuild_launches;
         return CAO_OK;
     }
-    int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st);
+    int rc = launch_pass1(s, (void*)s->meta.bitmap, (uint8_t*)s->d_scratch, st, !single);
     if (rc) return rc;
-    return launch_fill(s, (uint8_t*)s->d_table, st);
+    return launch_fill(s, (uint8_t*)s->d_table, st, single);
 }
 
 int cao_space_build_stats(const cao_space* s, void* stream, uint64_t* h_out4) {

@@ -187,15 +187,25 @@ def test_exp_neg_spec_bit_exact():
     assert np.array_equal(got.view(np.uint32), O.exp_neg_spec_many(zb).view(np.uint32))
 
 
-@pytest.mark.parametrize("cfg", [0, 1, 2])
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
 def test_rebuild_reproduces_the_space(cfg):
-    """cao_space_rebuild: all of S1 again, asynchronously, into the same (wiped) buffers."""
+    """cao_space_rebuild: all of S1 again, asynchronously, into the same (wiped) buffers -- on the default stream (plain
+    launches) and twice on a side stream (captured CUDA graph, then its replay); the count scan of the rebuild is the
+    single-pass look-back variant (274 chunks on configs[3])."""
     sp, os_ = oracle_space(cfg, with_objective=False)
     gs = _gpu_space(sp)
     gs._bitmap.zero_(); gs.rows().zero_(); gs.Ltab().zero_(); gs.rank_dir().zero_()
     gs.rebuild()
     torch.cuda.synchronize()
     _check_space(sp, os_, gs)
+    side = torch.cuda.Stream()
+    for _ in range(2):
+        gs._bitmap.zero_(); gs.rows().zero_(); gs.Ltab().zero_(); gs.rank_dir().zero_()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            gs.rebuild()
+        torch.cuda.synchronize()
+        _check_space(sp, os_, gs)
     rows = np.stack([np.random.default_rng(1).integers(0, m, size=64) for m in sp.m], axis=1).astype(np.uint8)
     want = os_.repair(rows)
     rank, key = gs.repair(rows)                                         # probe tables survive the rebuild
