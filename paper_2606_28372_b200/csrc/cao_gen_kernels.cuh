@@ -308,9 +308,9 @@ __device__ __forceinline__ void store_state(const Grp& g, const SpaceMeta& sm, c
 // One generation `gen` of run k, state in shared memory.  last = write the parity taps of this generation.
 // Dimension loops are runtime loops over bytes in shared memory (compact code: the kernel is bound by instruction
 // issue and instruction fetch, not by memory).
-template <int ALGO, int ROWW>
+template <int ALGO, int ROWW, bool WIDE>
 __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, const ProbeMeta& pm, const CtaTabs& tb,
-                                           const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen, bool last, bool wide) {
+                                           const RunsMeta& rm, GrpMem& S, uint32_t k, uint32_t gen, bool last) {
     constexpr int RB = ROWW * 4;
     const uint32_t i = g.t, P = rm.P, run = rm.first_run + k;
     const int n = sm.n;
@@ -412,7 +412,7 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
                 PUT_DIM(d, (uint32_t)kq);
             }
         }
-    } else if (ROWW == 4 && wide) {                                     // O7: Firefly, FOUR LANES PER FIREFLY (underfilled GPU)
+    } else if (ROWW == 4 && WIDE) {                                     // O7: Firefly, FOUR LANES PER FIREFLY (underfilled GPU)
         // A lone warp per run is bound by the dependent chain r2 -> exp -> update of every attractor j.  Here lanes 4f..4f+3
         // share firefly f: lane `part` owns dimensions 4 part .. 4 part + 3, computes ONE Philox block per attractor instead
         // of five, and only the r2 sum is replicated: the 16 squared differences are gathered by shuffles and added in
@@ -893,11 +893,13 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int ALGO, int ROWW, int MAXT>
+template <int ALGO, int ROWW, int MAXT, bool WIDE = false>
 // Resident CTAs per SM (register budget), measured on the 10^5-run sweep: PSO and Firefly keep their per-dimension state and
 // Philox chains in registers and run 8 % faster with 128 registers x 2 CTAs than with 80 x 3 (which spills ~140 bytes per
 // thread); DE and GA are 8 % / 4 % faster with 3 CTAs.  64 registers x 4 CTAs lost everywhere (spills).
-__global__ void __launch_bounds__(MAXT, MAXT == 256 ? ((ALGO == CAO_PSO || ALGO == CAO_FIREFLY) ? 2 : 3) : 1)
+// WIDE (Firefly, four lanes per firefly, its own instantiation): the per-lane state is four dimensions and one Philox block, so
+// it keeps the 3-CTA budget.
+__global__ void __launch_bounds__(MAXT, MAXT == 256 ? (((ALGO == CAO_PSO || ALGO == CAO_FIREFLY) && !WIDE) ? 2 : 3) : 1)
 k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm, const __grid_constant__ RunsMeta rm,
       const __grid_constant__ GenLayout lay, uint32_t g_first, uint32_t n_gens) {
     extern __shared__ __align__(16) uint32_t s_dyn[];
@@ -939,7 +941,7 @@ k_gen(const __grid_constant__ SpaceMeta sm, const __grid_constant__ ProbeMeta pm
         for (; gen <= g_last; ++gen) {
             const bool active = rm.budget == 0 || gs->uniq < rm.budget;  // O10 (gen <= max_gens is enforced by the host)
             if (!active) break;
-            generation<ALGO, ROWW>(g, sm, pm, tb, rm, S, k, gen, gen == g_last, lay.wide != 0);
+            generation<ALGO, ROWW, WIDE>(g, sm, pm, tb, rm, S, k, gen, gen == g_last);
         }
         // a run that reached its budget stays frozen: its trajectory row repeats (O10)
         for (uint32_t q = gen + g.t; q <= g_last; q += g.G) {

@@ -9,7 +9,7 @@
 // Fused generation kernel, one object per algorithm (cao_gen_algo.cu).
 struct GenLayout;
 #define CAO_GEN_DECL(A)                                                                                                   \
-    int cao_gen_setup_##A(int roww, unsigned threads, size_t smem, int* occ);                                             \
+    int cao_gen_setup_##A(int roww, unsigned threads, size_t smem, int wide, int* occ);                                             \
     int cao_gen_launch_##A(int roww, unsigned grid, unsigned threads, size_t smem, cudaStream_t st, const SpaceMeta& sm,  \
                            const ProbeMeta& pm, const RunsMeta& rm, const GenLayout& lay, uint32_t g_first, uint32_t n_gens);
 CAO_GEN_DECL(0) CAO_GEN_DECL(1) CAO_GEN_DECL(2) CAO_GEN_DECL(3)
@@ -437,10 +437,10 @@ int cao_runs_step(cao_runs* r, uint32_t n_generations, void* stream) {
             CAO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             int rc = CAO_OK;
             switch (algo) {
-                case CAO_DE: rc = cao_gen_setup_0(roww, r->gen_threads, r->gen_smem, &occ); break;
-                case CAO_PSO: rc = cao_gen_setup_1(roww, r->gen_threads, r->gen_smem, &occ); break;
-                case CAO_FIREFLY: rc = cao_gen_setup_2(roww, r->gen_threads, r->gen_smem, &occ); break;
-                default: rc = cao_gen_setup_3(roww, r->gen_threads, r->gen_smem, &occ); break;
+                case CAO_DE: rc = cao_gen_setup_0(roww, r->gen_threads, r->gen_smem, (int)r->lay.wide, &occ); break;
+                case CAO_PSO: rc = cao_gen_setup_1(roww, r->gen_threads, r->gen_smem, (int)r->lay.wide, &occ); break;
+                case CAO_FIREFLY: rc = cao_gen_setup_2(roww, r->gen_threads, r->gen_smem, (int)r->lay.wide, &occ); break;
+                default: rc = cao_gen_setup_3(roww, r->gen_threads, r->gen_smem, (int)r->lay.wide, &occ); break;
             }
             if (rc) return rc;
             if (occ < 1) return cao_fail(CAO_E_TOO_LARGE, "cao_runs_step: the population state does not fit the shared memory of one SM");
