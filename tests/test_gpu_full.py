@@ -88,18 +88,20 @@ def same_everywhere(a, b):
 
 
 # ----------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("R", [1500, 20000])
+@pytest.mark.parametrize("R", [1000, 1500, 20000])
 @pytest.mark.parametrize("algo", ["de", "pso", "firefly", "ga"])
 def test_cfg1_many_runs_sampled_windows(algo, R):
     """More runs than resident groups: the persistent kernel's tickets wrap around; windows at both ends and across
-    the first wave boundary; fused against phased on ALL runs."""
+    the first wave boundary; fused against phased on ALL runs.  R = 1000 is the launch shape bench.py times: widened
+    groups (two warps per run; Firefly four lanes per firefly, its own instantiation); 1500 and 20000 run one warp per run."""
     import paper_2606_28372_b200 as cao
     sp, os_ = oracle_space(1)
     g = gpu_space(1, os_, sp)
     gens, width = 30, 8
-    windows = sorted({0, 1184, 1492, R - width})
+    windows = sorted({0, 1184, 1492, R - width} if R > 1492 + width else {0, 296, 500, R - width})
     kw = dict(pop=32, budget=0, seed=0)
     gf = cao.Runs(g, algo, n_runs=R, max_gens=gens, mode="fused", **kw)
+    assert gf.fused_width == ((4 if algo == "firefly" else 2) if R == 1000 else 1)
     gf.step(7); gf.step(gens - 7)                                       # two launches: state leaves and re-enters shared memory
     ors = oracle_windows(os_, algo, windows, width, gens, **kw)
     for k0, orr in zip(windows, ors):
