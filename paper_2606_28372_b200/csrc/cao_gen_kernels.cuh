@@ -365,7 +365,17 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
         g.sync();
         if (has) s_key[i] = ((unsigned long long)fbits(S.f[i]) << 32) | S.rank[i];
         g.sync();
-        if (has) {
+        if (g.G == 32) {
+            // One warp: position = keys below mine + equal keys in lower lanes (one MATCH for all the ties, so the loop
+            // is a bare 64-bit less-than).  Equal keys are identical configurations: their order is immaterial anyway.
+            const unsigned long long me = has ? s_key[i] : ~0ull - i;
+            const uint32_t ties = __match_any_sync(0xFFFFFFFFu, me);
+            if (has) {
+                uint32_t pos = (uint32_t)__popc(ties & ((1u << i) - 1u));
+                for (uint32_t j = 0; j < P; ++j) pos += s_key[j] < me;
+                s_order[pos] = i;
+            }
+        } else if (has) {
             const unsigned long long me = s_key[i];
             uint32_t pos = 0;
             for (uint32_t j = 0; j < P; ++j) { const unsigned long long o = s_key[j]; pos += (o < me) || (o == me && j < i); }
@@ -379,9 +389,19 @@ __device__ __forceinline__ void generation(const Grp& g, const SpaceMeta& sm, co
             for (uint32_t z = 0; z < B; ++z) sb = min(sb, below(dr(B + z), P));
             if (sb == sa) sb = sa + 1 == P ? 0 : sa + 1;
             const int cut = n > 1 ? 1 + (int)below(dr(2 * B), (uint32_t)(n - 1)) : 1;
-            const uint8_t* ra = idx8 + (size_t)s_order[sa] * RB; const uint8_t* rb = idx8 + (size_t)s_order[sb] * RB;
-#pragma unroll 2
-            for (int d = 0; d < n; ++d) PUT_DIM(d, d < cut ? (uint32_t)ra[d] : (uint32_t)rb[d]);
+            // the child is assembled a word at a time (bytes below the cut from A, the rest from B), compared with last
+            // generation's candidate and stored as words; only the linear index walks the dimensions
+            const uint32_t* wa = S.idx + (size_t)s_order[sa] * ROWW; const uint32_t* wb = S.idx + (size_t)s_order[sb] * ROWW;
+            uint32_t* cw = S.cand + (size_t)i * ROWW;
+#pragma unroll
+            for (int z = 0; z < ROWW; ++z) {
+                const int nb_a = min(max(cut - 4 * z, 0), 4);                    // bytes of this word that come from A
+                const uint32_t ma = nb_a >= 4 ? 0xFFFFFFFFu : ((1u << (8 * nb_a)) - 1u);
+                const uint32_t cwz = (wa[z] & ma) | (wb[z] & ~ma);
+                same = same && cw[z] == cwz;
+                cw[z] = cwz;
+            }
+            for (int d = 0; d < n; ++d) L += (uint64_t)cand8[d] * tb.stride[d];
         }
         g.sync();                                                       // every parent row is read before the population is replaced
     } else if (ALGO == CAO_PSO) {                                       // O6
