@@ -206,3 +206,25 @@ def test_default_execution_mode():
         sp, os_ = oracle_space(cfg)
         g = gpu_space(cfg, os_, sp)
         assert cao.Runs(g, "firefly", n_runs=2, pop=8, max_gens=1).mode == want, cfg
+
+
+def test_fused_width_api():
+    """cao_runs_set_fused_width: 0 / 1 / 2 / 4 only, before the first fused step; a width that does not apply falls back."""
+    import paper_2606_28372_b200 as cao
+    sp, os_ = oracle_space(0)
+    g = gpu_space(0, os_, sp)
+    r = cao.Runs(g, "ga", n_runs=4, pop=20, max_gens=4, mode="fused")
+    with pytest.raises(cao.CaoError) as e:
+        cao.lib().cao_runs_set_fused_width  # symbol exists
+        cao.api._check(cao.lib().cao_runs_set_fused_width(r._h, 3))
+    assert e.value.code == -1
+    cao.api._check(cao.lib().cao_runs_set_fused_width(r._h, 4))
+    assert r.fused_width == 4
+    r.step(1)
+    with pytest.raises(cao.CaoError) as e:
+        cao.api._check(cao.lib().cao_runs_set_fused_width(r._h, 1))
+    assert e.value.code == -2
+    sp3, os3 = oracle_space(3)                               # 32-byte rows: Firefly's four-lane operator does not apply
+    g3 = gpu_space(3, os3, sp3)
+    r3 = cao.Runs(g3, "firefly", n_runs=2, pop=16, max_gens=2, mode="fused", fused_width=4)
+    assert r3.fused_width == 1
