@@ -330,35 +330,55 @@ __global__ void __launch_bounds__(256) k_res_prefix(const __grid_constant__ Spac
         if (valid) out[e] = p;
     }
 }
-// k_res_class_table: one thread per (class constraint, hash slot, inner pattern) resumes the program from the class key.
-// Warps stride over (hash slot, 32 patterns) items; only the used slots (a few dozen) do any work.
+// k_res_class_table: one thread per (class constraint, used hash slot, inner pattern) resumes the program from the class
+// key.  Every CTA first compacts the used slots (a few dozen of 4096) into the same slot-ordered list in shared memory --
+// warp w reads slots [512 w, 512 w + 512) with 16 coalesced loads in flight, ballots, one barrier for the eight warp
+// counts -- so that the (used slot, 32 patterns) items can be dealt evenly to all the warps of the grid.
 __global__ void __launch_bounds__(256) k_res_class_table(const __grid_constant__ SpaceMeta sm, const __grid_constant__ EnumArgs a) {
-    const uint32_t lane = threadIdx.x & 31;
+    __shared__ uint16_t s_used[CAO_HS];
+    __shared__ uint32_t s_cnt[8];
+    const uint32_t lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const uint32_t wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     const int rc = blockIdx.y;
+    const long long* __restrict__ keys = a.rc[rc].keys;
+    uint32_t bal[CAO_HS / 256], mine = 0;
+    {
+        long long kv[CAO_HS / 256];
+#pragma unroll
+        for (int it = 0; it < CAO_HS / 256; ++it) kv[it] = keys[wl * (CAO_HS / 8) + it * 32 + lane];
+#pragma unroll
+        for (int it = 0; it < CAO_HS / 256; ++it) { bal[it] = __ballot_sync(0xFFFFFFFFu, kv[it] != CAO_CLS_EMPTY); mine += (uint32_t)__popc(bal[it]); }
+    }
+    if (lane == 0) s_cnt[wl] = mine;
+    __syncthreads();
+    uint32_t base = 0, n_used = 0;
+    for (uint32_t k = 0; k < 8; ++k) { if (k < wl) base += s_cnt[k]; n_used += s_cnt[k]; }
+#pragma unroll
+    for (int it = 0; it < CAO_HS / 256; ++it) {
+        if ((bal[it] >> lane) & 1u) s_used[base + __popc(bal[it] & ((1u << lane) - 1u))] = (uint16_t)(wl * (CAO_HS / 8) + it * 32 + lane);
+        base += (uint32_t)__popc(bal[it]);
+    }
+    __syncthreads();
     const int32_t* ds = a.desc + a.desc[a.n_tab + a.rc[rc].r];
     const uint32_t per_row = a.Wb * 64;
     const uint32_t chunks = per_row >> 5;                               // 32 patterns per warp item
-    for (uint32_t item = wid; item < CAO_HS * chunks; item += nwarps) {
-        const uint32_t slot = item / chunks, p0 = (item - slot * chunks) << 5;
-        const long long key = a.rc[rc].keys[slot];
-        if (key == CAO_CLS_EMPTY) continue;
-        {
-            const uint32_t p = p0 + lane;
-            int ok = 0;
-            if (p < a.B) {
-                int64_t x[CAO_MAX_DIMS];
-                for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
-                uint32_t q = p;
-                for (int d = sm.n - 1; d >= a.t; --d) { const uint32_t m = sm.m[d]; x[d] = a.dom[d * 256 + q % m]; q /= m; }
-                int64_t st[CAO_MAX_STACK];
-                st[0] = key;
-                int u0, u1;
-                ok = eval_core(ds + 1, ds[0], x, a.rc[rc].pc0, st, 1, -1, &u0, &u1);
-            }
-            const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
-            if (lane == 0) ((uint32_t*)a.rc[rc].table)[((uint64_t)slot * per_row + p0) >> 5] = word;
+    for (uint32_t item = wid; item < n_used * chunks; item += nwarps) {
+        const uint32_t slot = s_used[item / chunks], p0 = (item % chunks) << 5;
+        const long long key = keys[slot];
+        const uint32_t p = p0 + lane;
+        int ok = 0;
+        if (p < a.B) {
+            int64_t x[CAO_MAX_DIMS];
+            for (int d = 0; d < sm.n; ++d) x[d] = a.dom[d * 256];
+            uint32_t q = p;
+            for (int d = sm.n - 1; d >= a.t; --d) { const uint32_t m = sm.m[d]; x[d] = a.dom[d * 256 + q % m]; q /= m; }
+            int64_t st[CAO_MAX_STACK];
+            st[0] = key;
+            int u0, u1;
+            ok = eval_core(ds + 1, ds[0], x, a.rc[rc].pc0, st, 1, -1, &u0, &u1);
         }
+        const uint32_t word = __ballot_sync(0xFFFFFFFFu, ok);
+        if (lane == 0) ((uint32_t*)a.rc[rc].table)[((uint64_t)slot * per_row + p0) >> 5] = word;
     }
 }
 
