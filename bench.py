@@ -221,7 +221,7 @@ def gpu_arm(args):
     pk = peaks()
     wl = workload(args.config, args.runs)
     sp, R, P, G = wl["space"], wl["runs"], wl["pop"], wl["gens"]
-    from paper_2606_28372_b200.shard import shard_runs, max_over_ranks
+    from paper_2606_28372_b200.shard import shard_runs, max_over_ranks, sum_over_ranks
     first_run, _n_local = shard_runs(world * R, world, rank)         # weak scaling: R runs per rank, global run indices
     assert _n_local == R
 
@@ -315,7 +315,8 @@ def gpu_arm(args):
     scanned_step = sum(c["n_scanned"] for c in stats)
     repaired_step = sum(c["n_repaired"] for c in stats)
     gens_done = [int(r.best()["gens_done"].sum().item()) for r in runs]
-    value = world * cands_step * args.steps / (ms / 1e3)
+    cands_job = sum_over_ranks(cands_step, dev)                            # every rank ran its own runs: the job's count is the sum
+    value = cands_job * args.steps / (ms / 1e3)
     del space, runs, kept                                                 # never more than two buffer sets alive (see the warm-up)
     # per-kernel device times: the same step, serialised on one stream, events around every launch
     ms_prof, _, prof, _, _ = timed(args.steps, False, True, concurrent=False)
@@ -325,7 +326,7 @@ def gpu_arm(args):
     kept_w = None
     torch.cuda.synchronize()
     ms_e, wall_e, _, _, _ = timed(args.steps, True, False)
-    value_e = world * cands_step * args.steps / (ms_e / 1e3)
+    value_e = cands_job * args.steps / (ms_e / 1e3)
     gc.enable()
     h2d = obj.nbytes + sum(len(d) * 8 for d in sp.domains) + sum(len(p) * 4 for p in sp.rpn)
     d2h = len(wl["algos"]) * 16 * R + 8

@@ -24,6 +24,15 @@ def max_over_ranks(value: float, device="cpu") -> float:
     return float(t.item())
 
 
+def sum_over_ranks(value: int, device="cpu") -> int:
+    """Whole-job count of units (candidates) = the sum of every rank's."""
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return int(value)
+    t = torch.tensor([int(value)], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return int(t.item())
+
+
 def gather_runs(local: torch.Tensor, total_runs: int) -> torch.Tensor | None:
     """Gathers per-run rows (n_local, k) of every rank into global run order on rank 0 (None elsewhere)."""
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:

@@ -7,7 +7,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2606_28372_b200.shard import shard_runs, max_over_ranks, gather_runs
+from paper_2606_28372_b200.shard import shard_runs, max_over_ranks, sum_over_ranks, gather_runs
 
 
 def test_shard_runs_is_a_partition():
@@ -29,6 +29,7 @@ def _worker(rank, world, port, total):
         idx = torch.arange(first, first + n, dtype=torch.int64)
         local = torch.stack([idx, idx * idx % 1013], dim=1)
         assert max_over_ranks(10.0 + rank) == 10.0 + world - 1
+        assert sum_over_ranks(n) == total                        # whole-job unit count = the sum of the ranks' counts
         allr = gather_runs(local, total)
         if rank == 0:
             want = torch.arange(total, dtype=torch.int64)
