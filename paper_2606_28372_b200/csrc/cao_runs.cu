@@ -93,8 +93,8 @@ static int launch_probe23(const cao_space* s, const SpaceMeta& sm, const uint8_t
     ProbeMeta pm = s->probe;
     pm.levels = levels;
     ProfScope ps(PK_PROBE, st);
-    if (sm.rowB == 16) k_probe23<4><<<148 * 4, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
-    else k_probe23<8><<<148 * 4, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
+    if (sm.rowB == 16) k_probe23<4><<<148 * 8, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
+    else k_probe23<8><<<148 * 8, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
     CAO_LAUNCHED("k_probe23");
     return CAO_OK;
 }
