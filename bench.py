@@ -194,10 +194,9 @@ def reference_arm(args):
 # ----------------------------------------------------------------------------------------------------------
 def scan_ops_per_pair(n):
     """Integer instructions per (candidate, valid row) of k_scan, by kind, counted in the SASS of its inner loop
-    (n = 20: 5 VABSDIFF4 + 11 LOP3 + 6 IADD + 3 SHF + 2 POPC + 3 ISETP/SEL + 1 IMAD + 2 LDS)."""
+    (n = 20: 5 VABSDIFF4 + 5 LOP3 + 6 IADD + 10 IDP.4A + 1 IMAD + 3 ISETP/SEL + 2 LDS)."""
     wu = (n + 3) // 4
-    return {"vabsdiff4": wu, "lop3": 2 * wu + 1, "shf": (wu + 1) // 2, "iadd": wu + 1, "popc": (wu + 3) // 4, "setp_sel": 3,
-            "imad": 1, "lds": (wu + 3) // 4}
+    return {"vabsdiff4": wu, "lop3": wu, "iadd": wu + 1, "idp4a": 2 * wu, "setp_sel": 3, "imad": 1, "lds": (wu + 3) // 4}
 
 
 def enum_bytes(N, V, row_bytes, ltab_bytes):
@@ -361,21 +360,24 @@ def gpu_arm(args):
     # ---- measured integer issue peaks (lane-operations per second, one instruction kind each)
     int_peak = {}
     if not args.no_peak:
-        int_peak = {k: cao.int_peak(k) / 1e12 for k in ("imad", "lop3", "vabsdiff4", "popc", "iadd")}
+        int_peak = {k: cao.int_peak(k) / 1e12 for k in ("imad", "lop3", "vabsdiff4", "popc", "iadd", "idp4a")}
         int_peak["unit"] = "T lane-op/s"
 
     def scan_alu(n_dim, pairs, seconds):
         """Integer-pipe fractions of the repair scan against the MEASURED rates: (a) all its instructions against the
         issue rate (one warp instruction per scheduler per clock = the measured IADD rate), (b) the instructions of the
-        half-rate alu pipe (LOP3, VABSDIFF4, SHF, compare/select) against the measured LOP3 rate.  The larger binds."""
+        half-rate alu pipe (LOP3, VABSDIFF4, compare/select) against the measured LOP3 rate, (c) the IDP.4A / IMAD
+        instructions against the measured IDP.4A rate.  The largest binds."""
         if not int_peak or pairs == 0 or seconds <= 0:
             return None
         mix = scan_ops_per_pair(n_dim)
         total = sum(mix.values())
-        half = mix["vabsdiff4"] + mix["lop3"] + mix["shf"] + mix["setp_sel"]
+        half = mix["vabsdiff4"] + mix["lop3"] + mix["setp_sel"]
         return {"bound": "alu", "ops_per_pair": mix, "pairs": pairs, "achieved": total * pairs / seconds / 1e12,
                 "unit": "T lane-op/s", "peak_issue": int_peak["iadd"], "frac_of_issue": total * pairs / seconds / 1e12 / int_peak["iadd"],
-                "peak_alu_pipe": int_peak["lop3"], "frac_of_alu_pipe": half * pairs / seconds / 1e12 / int_peak["lop3"]}
+                "peak_alu_pipe": int_peak["lop3"], "frac_of_alu_pipe": half * pairs / seconds / 1e12 / int_peak["lop3"],
+                "peak_fma_pipe": int_peak["idp4a"],
+                "frac_of_fma_pipe": (mix["idp4a"] + mix["imad"]) * pairs / seconds / 1e12 / int_peak["idp4a"]}
 
     # ---- S1 alone (BASELINE metric "enumeration Gcfg/s"): configs[1..3], resident buffers
     enum = {}

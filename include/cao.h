@@ -275,7 +275,7 @@ int cao_test_curand_philox(const uint32_t* d_ctr_key /* count x 6 */, uint32_t* 
 int cao_test_exp_neg(const float* d_z, float* d_out, uint64_t count, void* stream);
 /* Integer-issue microbenchmark (the denominator of bench.py's "alu" roofline for the repair scan):
  * n_ctas x 256 threads, each runs `iters` x 8 independent chains of one instruction kind: 0 IMAD (mad.lo.u32),
- * 1 LOP3, 2 VABSDIFF4 (with accumulate), 3 POPC, 4 IADD.  d_out: n_ctas * 256 words.  The caller times it. */
+ * 1 LOP3, 2 VABSDIFF4 (with accumulate), 3 POPC, 4 IADD, 5 IDP.4A (dp4a with accumulate).  d_out: n_ctas * 256 words.  The caller times it. */
 int cao_test_int_peak(int32_t kind, uint32_t iters, uint32_t n_ctas, uint32_t* d_out, void* stream);
 
 const char* cao_last_error(void);

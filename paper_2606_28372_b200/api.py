@@ -533,7 +533,7 @@ def test_exp_neg(z: torch.Tensor) -> torch.Tensor:
     return out
 
 
-INT_PEAK_KINDS = {"imad": 0, "lop3": 1, "vabsdiff4": 2, "popc": 3, "iadd": 4}
+INT_PEAK_KINDS = {"imad": 0, "lop3": 1, "vabsdiff4": 2, "popc": 3, "iadd": 4, "idp4a": 5}
 
 
 def int_peak(kind: str, iters=4096, n_ctas=148 * 8, reps=5) -> float:

@@ -134,6 +134,7 @@ __global__ void __launch_bounds__(256) k_int_peak(uint32_t* out, uint32_t iters)
             if (KIND == 2) asm volatile("vabsdiff4.u32.u32.u32.add %0, %0, %1, %2;" : "+r"(a[j]) : "r"(b), "r"(c));
             if (KIND == 3) asm volatile("popc.b32 %0, %0;" : "+r"(a[j]));
             if (KIND == 4) asm volatile("add.u32 %0, %0, %1;" : "+r"(a[j]) : "r"(b));
+            if (KIND == 5) asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(a[j]) : "r"(b), "r"(c));
         }
     }
     uint32_t x = 0;
@@ -751,7 +752,8 @@ int cao_test_int_peak(int32_t kind, uint32_t iters, uint32_t n_ctas, uint32_t* d
         case 2: k_int_peak<2><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
         case 3: k_int_peak<3><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
         case 4: k_int_peak<4><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
-        default: return cao_fail(CAO_E_INVALID_ARG, "cao_test_int_peak: kind must be 0..4");
+        case 5: k_int_peak<5><<<n_ctas, 256, 0, st>>>(d_out, iters); break;
+        default: return cao_fail(CAO_E_INVALID_ARG, "cao_test_int_peak: kind must be 0..5");
     }
     CAO_LAUNCHED("k_int_peak");
     return CAO_OK;
