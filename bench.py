@@ -194,9 +194,9 @@ def reference_arm(args):
 # ----------------------------------------------------------------------------------------------------------
 def scan_ops_per_pair(n):
     """Integer instructions per (candidate, valid row) of k_scan, by kind, counted in the SASS of its inner loop
-    (n = 20: 5 VABSDIFF4 + 5 LOP3 + 6 IADD + 10 IDP.4A + 1 IMAD + 3 ISETP/SEL + 2 LDS)."""
+    (n = 20: 5 VABSDIFF4 + 6 IADD + 10 IDP.4A + 1 IMAD + 3 ISETP/SEL + 2 LDS)."""
     wu = (n + 3) // 4
-    return {"vabsdiff4": wu, "lop3": wu, "iadd": wu + 1, "idp4a": 2 * wu, "setp_sel": 3, "imad": 1, "lds": (wu + 3) // 4}
+    return {"vabsdiff4": wu, "lop3": 0, "iadd": wu + 1, "idp4a": 2 * wu, "setp_sel": 3, "imad": 1, "lds": (wu + 3) // 4}
 
 
 def enum_bytes(N, V, row_bytes, ltab_bytes):

@@ -294,27 +294,29 @@ __global__ void __launch_bounds__(SCAN_TC) k_scan(const __grid_constant__ SpaceM
                 uint32_t v[ROWW];
                 { uint4 a = tl[r * (ROWW / 4)]; v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; }
                 if (ROWW == 8) { uint4 b = tl[r * 2 + 1]; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w; }
-                // Hamming count without POPC (a quarter-rate instruction) and without the flag merging: the byte sums come
-                // from IDP.4A (dot product with 0x01010101), which does not issue on the alu pipe that bounds this loop.
-                //   SMALL (every index < 128): t = x + 0x7f7f7f7f has byte 127 for an equal byte and 128 + (x_b - 1) otherwise,
-                //   i.e. as SIGNED bytes t_b = x_b + 127 - 256 [x_b != 0]; so 256 * Hamming = sum x_b + 508 per word - sum s8(t_b).
-                //   general: flags f = 0x80 per differing byte, 128 * Hamming = sum f_b.
-                uint32_t sad = 0, xs = 0, fs = 0; int ts = 0;
+                // Per index word: ad = per-byte |c - v| (one VABSDIFF4), then both sums come from IDP.4A (dot product with
+                // 0x01010101), which issues on the fma pipe -- no POPC (quarter rate), no XOR, no flag merging:
+                //   sum |delta idx| = sum of the bytes of ad;
+                //   SMALL (every index < 128): t = ad + 0x7f7f7f7f has byte 127 where ad_b = 0 and 128 + (ad_b - 1) otherwise, i.e.
+                //   as SIGNED bytes t_b = ad_b + 127 - 256 [ad_b != 0], so 256 * Hamming = sum ad_b + 508 per word - sum s8(t_b).
+                //   general: flags f = 0x80 per differing byte from the carry trick on c ^ v, 128 * Hamming = sum f_b.
+                uint32_t sad = 0, fs = 0; int ts = 0;
 #pragma unroll
                 for (int k = 0; k < WU; ++k) {
-                    sad = sad4_acc(c[k], v[k], sad);
-                    if (KM == 0) {
-                        const uint32_t x = c[k] ^ v[k];
-                        if (SMALL) {
-                            xs = __dp4a(x, 0x01010101u, xs);
-                            ts = __dp4a((int)(x + 0x7f7f7f7fu), 0x01010101, ts);
-                        } else {
+                    if (KM == 0 && SMALL) {
+                        const uint32_t ad = __vabsdiffu4(c[k], v[k]);
+                        sad = __dp4a(ad, 0x01010101u, sad);
+                        ts = __dp4a((int)(ad + 0x7f7f7f7fu), 0x01010101, ts);
+                    } else {
+                        sad = sad4_acc(c[k], v[k], sad);
+                        if (KM == 0) {
+                            const uint32_t x = c[k] ^ v[k];
                             const uint32_t t = ((x & 0x7f7f7f7fu) + 0x7f7f7f7fu) | x;
                             fs = __dp4a(t & 0x80808080u, 0x01010101u, fs);
                         }
                     }
                 }
-                const uint32_t hamk = SMALL ? ((xs + 508u * WU - (uint32_t)ts) << 5) : (fs << 6);      // Hamming << 13
+                const uint32_t hamk = SMALL ? ((sad + 508u * WU - (uint32_t)ts) << 5) : (fs << 6);      // Hamming << 13
                 uint32_t k32 = KM == 1 ? sad : hamk + sad;
                 if (k32 < bestk) { bestk = k32; bestr = r0 + r; }         // ascending rank: ties keep the smallest L
             }
