@@ -158,6 +158,33 @@ int cao_space_is_valid(const cao_space* s, const uint8_t* d_idx_rows, uint64_t c
 int cao_space_repair_scratch_bytes(const cao_space* s, uint64_t count, uint64_t* bytes);
 int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
                      uint64_t* d_key_out, int32_t probe_levels, void* d_scratch, void* stream);
+/* cao_space_repair without a scratch argument, for callers that have no way to obtain device scratch at the moment of
+ * the call.  Everywhere else in this header the caller brings the scratch, which in practice means a cudaMalloc or a
+ * framework allocator somewhere up the call chain.  Some callers cannot do that: code that runs inside a memory pool's or
+ * an allocator's own callback (allocating there would re-enter it), a plugin whose host hands it input and output buffers
+ * and a stream but forbids allocation, a process whose whole device-memory budget was reserved up front by another
+ * component, or a latency-bound loop in which a cudaMalloc (it can synchronise the whole device) is not acceptable.
+ * For them the library carries its own scratch: one array inside its device image, CAO_REPAIR_NOALLOC_MAX_ROWS rows
+ * large (3 MiB + 256 bytes).  Every GPU on which the library's kernels get loaded holds that array until the process
+ * exits, whether or not this function is ever called.
+ *   - Same inputs, outputs, probe_levels meaning and results as cao_space_repair (S5: L143, L215, L270; O9); the caller
+ *     still owns d_idx_rows (16-byte aligned), d_rank_out and d_key_out (either may be NULL, not both).
+ *   - count > CAO_REPAIR_NOALLOC_MAX_ROWS returns CAO_E_TOO_LARGE and launches nothing: split the batch, or use
+ *     cao_space_repair.  count == 0 is a no-op.
+ *   - The function calls no cudaMalloc, cudaFree or other allocating routine.  That includes the optional per-kernel
+ *     timing, which creates CUDA events: while cao_profile_enable(1) is in force the call returns CAO_E_STATE.
+ *   - The first call on each device looks up the array's address on that device (cudaGetSymbolAddress, with the device
+ *     that holds the space's buffers current, as for every launching call) and remembers it.  Make that first call
+ *     before any stream capture is begun on that device; later calls only enqueue an 8-byte memset and the kernels.
+ *   - There is ONE array per device and every call uses it.  It still holds the previous call's data when the next one
+ *     starts; the function clears the part that must start at zero (the worklist counters) and overwrites the rest
+ *     before reading it, so back-to-back calls on one stream are independent.  Two calls whose kernels can overlap on
+ *     the GPU -- different streams without an event between them, or several host threads -- race on the array and give
+ *     wrong ranks: order them on one stream or with events.  That holds across cao_space handles too: the array belongs
+ *     to the library, not to a space. */
+#define CAO_REPAIR_NOALLOC_MAX_ROWS 65536
+int cao_space_repair_noalloc(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
+                             uint64_t* d_key_out, int32_t probe_levels, void* stream);
 /* NEXT-1 standalone (L139-143, L215, L270, Alg.2, Alg.3): the paper's own repairs for `count` rows.
  * mode 1 = index distance: d_rank_out[i] = argmin (sum |didx|, L);  2 = Alg.2 with d_x: count x n fp32 continuous
  * positions (row-major);  3 = Alg.3 with d_w: count 32-bit draws (member number floor(w K / 2^32) of the first non-empty

@@ -76,6 +76,7 @@ SIGNATURES = {
     "cao_space_is_valid": (C.c_int, [vp, vp, u64, vp, vp]),
     "cao_space_repair_scratch_bytes": (C.c_int, [vp, u64, pu64]),
     "cao_space_repair": (C.c_int, [vp, vp, u64, vp, vp, i32, vp, vp]),
+    "cao_space_repair_noalloc": (C.c_int, [vp, vp, u64, vp, vp, i32, vp]),
     "cao_space_set_objective": (C.c_int, [vp, vp]),
     "cao_runs_workspace_bytes": (C.c_int, [vp, i32, i32, u32, u32, pu64]),
     "cao_runs_create": (C.c_int, [vp, i32, C.POINTER(HParams), u32, u32, i32, u32, u32, u64, vp, vp, pvp]),
@@ -318,6 +319,30 @@ class Space:
                                       scratch.data_ptr(), _stream()))
         self._last_scratch = scratch
         return rank, key
+
+    REPAIR_NOALLOC_MAX_ROWS = 65536
+
+    def repair_noalloc(self, rows, rank_out=None, key_out=None, use_probe=True):
+        """cao_space_repair_noalloc: the repair of ``repair`` for code that may not allocate device memory when it runs
+        (an allocator or memory-pool callback, a plugin that is only lent buffers and a stream, a process whose device
+        memory is already fully reserved).  The scratch is a fixed 3 MiB array inside libcao.so, so at most
+        REPAIR_NOALLOC_MAX_ROWS rows per call (CaoError CAO_E_TOO_LARGE beyond), and calls must not overlap on the GPU.
+
+        This wrapper allocates nothing either, so everything is the caller's and already on the device:
+        rows (count, row_bytes) uint8, contiguous, padding bytes zero or not (they are ignored) -- see ``pack_rows``;
+        rank_out (count,) int32 and/or key_out (count,) int64 receive the results (uint32 / uint64 bit patterns)."""
+        use_probe = -1 if use_probe is True else 0 if use_probe is False else int(use_probe)
+        c = int(rows.shape[0])
+        if not (rows.is_cuda and rows.dtype == torch.uint8 and rows.is_contiguous() and rows.dim() == 2 and
+                rows.shape[1] == self.row_bytes):
+            raise ValueError("repair_noalloc: rows must be a contiguous (count, row_bytes) uint8 CUDA tensor (pack_rows)")
+        for t, dt in ((rank_out, torch.int32), (key_out, torch.int64)):
+            if t is not None and not (t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() >= c):
+                raise ValueError("repair_noalloc: outputs must be contiguous CUDA tensors, int32 ranks / int64 keys, count long")
+        _check(lib().cao_space_repair_noalloc(self._h, rows.data_ptr(), c,
+                                              rank_out.data_ptr() if rank_out is not None else None,
+                                              key_out.data_ptr() if key_out is not None else None, use_probe, _stream()))
+        return rank_out, key_out
 
     def repair_mode(self, mode, rows, x=None, w=None):
         """NEXT-1 standalone: mode 'index' (L270) | 'alg2' (x: continuous positions) | 'alg3' (w: 32-bit draws)

@@ -2,6 +2,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <curand_kernel.h>
 #include "cao_runs_kernels.cuh"
 #include "cao_var_kernels.cuh"
@@ -143,6 +144,39 @@ __global__ void __launch_bounds__(256) k_int_peak(uint32_t* out, uint32_t iters)
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = x;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Scratch of cao_space_repair_noalloc: one fixed array in the library's own device image, so the entry point never has to
+// ask the CUDA allocator for anything.  Sized for CAO_REPAIR_NOALLOC_MAX_ROWS rows of the wider row format (32 bytes):
+// packed keys + two worklists + their counters + the padding-cleaned copy of the rows -- the same regions, in the same
+// order, as cao_space_repair_scratch_bytes.  Every GPU on which the library's kernels get loaded keeps its own copy of
+// these 3 MiB until the process ends.
+#define CAO_NOALLOC_SCRATCH_BYTES ((size_t)CAO_REPAIR_NOALLOC_MAX_ROWS * (8 + 4 + 4 + 32) + 256)
+static_assert(CAO_NOALLOC_SCRATCH_BYTES % 256 == 0, "regions of the static scratch stay 256-byte aligned");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[CAO_NOALLOC_SCRATCH_BYTES];
+// In host code `g_noalloc_scratch` is only a handle for the runtime, not something a kernel can dereference: the real
+// device address differs per GPU and is looked up once per device with cudaGetSymbolAddress (noalloc_scratch_ptr).
+#define CAO_NOALLOC_MAX_DEVICES 64
+static std::mutex g_noalloc_mu;
+static void* g_noalloc_ptr[CAO_NOALLOC_MAX_DEVICES] = {};
+
+// Device address of the static scratch on the CURRENT device; resolved on the first call per device, cached afterwards.
+static int noalloc_scratch_ptr(void** out) {
+    int dev = -1;
+    CAO_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= CAO_NOALLOC_MAX_DEVICES)
+        return cao_fail(CAO_E_CUDA, "cao_space_repair_noalloc: device ordinal " + std::to_string(dev) + " is outside 0.." +
+                                        std::to_string(CAO_NOALLOC_MAX_DEVICES - 1));
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        CAO_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p || ((uintptr_t)p & 255)) return cao_fail(CAO_E_CUDA, "cao_space_repair_noalloc: the static scratch has no usable device address");
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return CAO_OK;
+}
+
 extern "C" {
 
 // ---------------------------------------------------------------------------------------------
@@ -189,6 +223,31 @@ int cao_space_repair(const cao_space* s, const uint8_t* d_idx_rows, uint64_t cou
     k_repair_finish<<<grid, 256, 0, st>>>(key, count, d_rank_out, d_key_out);
     CAO_LAUNCHED("k_repair_finish");
     return CAO_OK;
+}
+
+// cao_space_repair for callers that cannot bring scratch memory because they cannot allocate (who they are: include/cao.h).
+// Inputs and outputs stay the caller's; the scratch is g_noalloc_scratch.  Nothing on this path allocates:
+// cudaGetDevice / cudaGetSymbolAddress (first call per device only), one cudaMemsetAsync of the two worklist counters,
+// then the launches of cao_space_repair.  The per-kernel timing option creates CUDA events, so it has to be off.
+int cao_space_repair_noalloc(const cao_space* s, const uint8_t* d_idx_rows, uint64_t count, uint32_t* d_rank_out,
+                             uint64_t* d_key_out, int32_t use_probe, void* stream) {
+    if (!s) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_noalloc: NULL space");
+    if (!s->filled) return cao_fail(CAO_E_STATE, "cao_space_repair_noalloc: space not built");
+    if (count > CAO_REPAIR_NOALLOC_MAX_ROWS)
+        return cao_fail(CAO_E_TOO_LARGE, "cao_space_repair_noalloc: " + std::to_string(count) + " rows, the static scratch holds at most " +
+                                             std::to_string(CAO_REPAIR_NOALLOC_MAX_ROWS) + " per call (split the batch, or use cao_space_repair)");
+    if (count == 0) return CAO_OK;
+    if (!d_idx_rows || (!d_rank_out && !d_key_out)) return cao_fail(CAO_E_INVALID_ARG, "cao_space_repair_noalloc: NULL argument");
+    if (s->meta.V == 0) return cao_fail(CAO_E_EMPTY_SPACE, "cao_space_repair_noalloc: the space has no valid configuration");
+    if ((uintptr_t)d_idx_rows & 15) return cao_fail(CAO_E_WORKSPACE, "cao_space_repair_noalloc: rows must be 16-byte aligned");
+    if (g_cao_prof_on.load(std::memory_order_relaxed) != 0)
+        return cao_fail(CAO_E_STATE, "cao_space_repair_noalloc: cao_profile_enable is on, and its timing events are allocations; switch it off");
+    void* scratch = nullptr;
+    int rc = noalloc_scratch_ptr(&scratch);
+    if (rc) return rc;
+    // The worklist counters are cleared by cao_space_repair's cudaMemsetAsync and every key of rows 0..count-1 is written by
+    // k_repair_probe before anything reads it, so whatever the previous call left in the array cannot leak into this one.
+    return cao_space_repair(s, d_idx_rows, count, d_rank_out, d_key_out, use_probe, scratch, stream);
 }
 
 // Shared-memory slice of one group of the fused kernel (cao_gen_kernels.cuh): word offsets.
