@@ -8,16 +8,17 @@
 #define CAO_CAT_(a, b) a##b
 #define CAO_CAT(a, b) CAO_CAT_(a, b)
 
-// Opt-in shared memory + resident CTAs per SM of the variant that (roww, threads) selects.
+// Opt-in shared memory (always the device maximum, see cao_smem_optin_max: run sets that share an instantiation must not
+// lower the limit under one another) + resident CTAs per SM of the variant that (roww, threads) selects.
 int CAO_CAT(cao_gen_setup_, CAO_GEN_ALGO)(int roww, unsigned threads, size_t smem, int wide, int* occ) {
 #define SETUP(W, T)                                                                                                        \
     do {                                                                                                                   \
-        CAO_CUDA(cudaFuncSetAttribute(k_gen<CAO_GEN_ALGO, W, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        CAO_SMEM_OPTIN((k_gen<CAO_GEN_ALGO, W, T>));                                                                       \
         CAO_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_gen<CAO_GEN_ALGO, W, T>, (int)threads, smem));       \
     } while (0)
 #if CAO_GEN_ALGO == 2
     if (wide && roww == 4 && threads <= 256) {                         // Firefly, four lanes per firefly: its own instantiation
-        CAO_CUDA(cudaFuncSetAttribute(k_gen<2, 4, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CAO_SMEM_OPTIN((k_gen<2, 4, 256, true>));
         CAO_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_gen<2, 4, 256, true>, (int)threads, smem));
         return CAO_OK;
     }

@@ -27,6 +27,24 @@ struct ProfScope {
 
 static inline uint64_t align256(uint64_t x) { return (x + 255) & ~255ull; }
 
+// Opt-in to more than 48 KB of dynamic shared memory.  cudaFuncAttributeMaxDynamicSharedMemorySize REPLACES the kernel's
+// limit, it does not raise it: two live objects (two cao_runs, two cao_space) that share a kernel instantiation and each
+// set "their" size would lower the limit under one another, and the larger one's next launch would fail with
+// cudaErrorInvalidValue.  So every site sets the same value, the most the device grants this kernel (opt-in limit per
+// block minus the kernel's static shared memory).  The limit is only a permission: what a launch occupies, and hence the
+// residency, still follows the size given at launch.
+template <class K>
+static inline int cao_smem_optin_max(K* kernel, const char* what) {
+    int dev = 0, optin = 0;
+    cudaFuncAttributes fa{};
+    int rc = cao_cuda_check(cudaGetDevice(&dev), what);
+    if (!rc) rc = cao_cuda_check(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), what);
+    if (!rc) rc = cao_cuda_check(cudaFuncGetAttributes(&fa, kernel), what);
+    if (!rc) rc = cao_cuda_check(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes), what);
+    return rc;
+}
+#define CAO_SMEM_OPTIN(kernel) do { int rc_ = cao_smem_optin_max(kernel, "shared-memory opt-in of " #kernel); if (rc_) return rc_; } while (0)
+
 // Value classes of a residual constraint (cao_enum_kernels.cuh, pass 1c).
 #define CAO_MAX_RC 4
 struct ResClassArgs {

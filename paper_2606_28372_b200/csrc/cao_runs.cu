@@ -470,10 +470,11 @@ int cao_runs_create_ex(const cao_space* s, int32_t algo, const cao_hparams* hp, 
             if ((rc2 = launch_scan(r->sm, m.cand, levels >= 2 ? m.wl2 : m.wl, levels >= 2 ? m.wl2_count : m.wl_count, m.key, true, st))) break;
         }
 #define CALL_INIT(A, W) \
-        if (r->smem_op > 48 * 1024) { cudaFuncSetAttribute(k_op<A, W, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); \
-                                      cudaFuncSetAttribute(k_op<A, W, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r->smem_op); } \
-        k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
+        if (r->smem_op > 48 * 1024) { rc2 = cao_smem_optin_max(k_op<A, W, 256>, "shared-memory opt-in of k_op");               \
+                                      if (!rc2) rc2 = cao_smem_optin_max(k_op<A, W, 1024>, "shared-memory opt-in of k_op"); } \
+        if (!rc2) k_init<A, W><<<n_runs, r->block, r->smem_init, st>>>(r->sm, r->rm)
         { ProfScope ps(PK_INIT, st); DISPATCH_ALGO_ROWW(algo, s->meta.rowB / 4, CALL_INIT); }
+        if (rc2) break;
         ++g_cao_launches;
         rc2 = cao_cuda_check(cudaGetLastError(), "k_init");
     } while (0);

@@ -336,7 +336,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 8191) / 8192, 148 * 8), (unsigned)s->n_tab);
         const uint32_t ci_cap = s->B <= 8192 ? (uint32_t)((s->B + 7) & ~7ull) : 0;
         const size_t tsm = 2 * (size_t)ci_cap + (size_t)std::max<uint64_t>(256, s->max_table_ci);
-        if (tsm > 48 * 1024) CAO_CUDA(cudaFuncSetAttribute(k_build_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
+        if (tsm > 48 * 1024) CAO_SMEM_OPTIN(k_build_tables);
         k_build_tables<<<grid, 256, tsm, st>>>(s->meta, d_dom, d_desc, d_tables, d_flags, s->B, s->Wb, s->t, ci_cap);
         CAO_LAUNCHED("k_build_tables");
     }
@@ -367,8 +367,8 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     {
         const uint64_t threads = (s->n_blocks + s->CH - 1) / s->CH;
         if (smem_enum > 48 * 1024) {
-            CAO_CUDA(cudaFuncSetAttribute(k_enum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_enum));
-            CAO_CUDA(cudaFuncSetAttribute(k_masks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_dig));
+            CAO_SMEM_OPTIN(k_enum);
+            CAO_SMEM_OPTIN(k_masks);
         }
         {
             ProfScope ps(PK_ENUM, st);

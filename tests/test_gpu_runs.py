@@ -228,3 +228,31 @@ def test_fused_width_api():
     g3 = gpu_space(3, os3, sp3)
     r3 = cao.Runs(g3, "firefly", n_runs=2, pop=16, max_gens=2, mode="fused", fused_width=4)
     assert r3.fused_width == 1
+
+
+def test_two_live_run_sets_share_a_kernel_instantiation():
+    """Two run sets of one algorithm that need different amounts of opt-in shared memory, stepped in turn.  The opt-in
+    limit belongs to the kernel instantiation, not to a run set: the set with the LARGER need is stepped first, then the
+    smaller one, then the larger one again (the order in which a per-set limit would have been lowered under it)."""
+    import paper_2606_28372_b200 as cao
+    sp, os_ = oracle_space(1)
+    g = gpu_space(1, os_, sp)
+    # fused PSO, P=128: width 1 = two runs per CTA (~2x the shared memory of width 2 = one run per CTA), same k_gen<1,4,256>
+    kw = dict(n_runs=6, pop=128, max_gens=6, seed=11)
+    big = cao.Runs(g, "pso", mode="fused", fused_width=1, **kw)
+    small = cao.Runs(g, "pso", mode="fused", fused_width=2, **kw)
+    ref = cao.Runs(g, "pso", mode="phased", **kw)
+    assert (big.fused_width, small.fused_width) == (1, 2)
+    for k in (1, 2, 3):
+        big.step(k); small.step(k); ref.step(k)
+        torch.cuda.synchronize()
+        assert torch.equal(big.trajectory(), ref.trajectory()) and torch.equal(small.trajectory(), ref.trajectory())
+    # phased Firefly: k_op<2,4,1024> needs (P n + 2 P) 4 bytes: 64 KB at P=1024, 56 KB at P=896 -- both above the 48 KB default
+    a = cao.Runs(g, "firefly", n_runs=2, pop=1024, max_gens=3, seed=3, mode="phased")
+    b = cao.Runs(g, "firefly", n_runs=2, pop=896, max_gens=3, seed=3, mode="phased")
+    orr = O.OracleRuns(os_, "firefly", n_runs=2, pop=1024, max_gens=3, seed=3)
+    for _ in range(3):
+        a.step(1); b.step(1); orr.step(1)
+        torch.cuda.synchronize()
+    compare(a, orr, sp.n)
+    assert b.gen == 3
