@@ -66,18 +66,19 @@ __device__ __forceinline__ float evaluate(const SpaceMeta& sm, const RunsMeta& r
 }
 __device__ __forceinline__ void eval_begin(const RunsMeta& rm, uint32_t k, RunShared* sh) {     // thread 0, before a sync
     uint32_t br = rm.best_rank[k];
-    // nothing valid evaluated yet: (penalty, no rank) -- every objective value is below the penalty (A33)
-    sh->best = br == 0xFFFFFFFFu ? (((unsigned long long)fbits(rm.var.penalty) << 32) | 0xFFFFFFFFu)
-                                 : (((unsigned long long)fbits(rm.best_f[k]) << 32) | br);
+    // nothing valid evaluated yet: no key at all, so that the FIRST valid evaluation is recorded whatever its value -- also an
+    // objective at or above the penalty (the contract is only "> 0 and finite"); eval_end reports (penalty, no rank) meanwhile (A33)
+    sh->best = br == 0xFFFFFFFFu ? ~0ull : (((unsigned long long)fbits(rm.best_f[k]) << 32) | br);
     sh->n_new = 0; sh->flag = 0; sh->aux = ~0ull;
 }
 __device__ __forceinline__ void eval_end(const RunsMeta& rm, uint32_t k, uint32_t g, RunShared* sh) {   // thread 0, after a sync
     uint32_t u = rm.uniq[k] + sh->n_new;
     rm.uniq[k] = u;
-    rm.best_f[k] = __uint_as_float((uint32_t)(sh->best >> 32));
-    rm.best_rank[k] = (uint32_t)sh->best;
+    const unsigned long long best = sh->best == ~0ull ? (((unsigned long long)fbits(rm.var.penalty) << 32) | 0xFFFFFFFFu) : sh->best;
+    rm.best_f[k] = __uint_as_float((uint32_t)(best >> 32));
+    rm.best_rank[k] = (uint32_t)best;
     uint32_t* t = rm.traj + ((uint64_t)g * rm.R + k) * 3;
-    t[0] = (uint32_t)(sh->best >> 32); t[1] = (uint32_t)sh->best; t[2] = u;
+    t[0] = (uint32_t)(best >> 32); t[1] = (uint32_t)best; t[2] = u;
 }
 
 // O4: P distinct valid ranks, uniform with linear probing; fills the population and evaluates it.

@@ -248,3 +248,11 @@ def test_sorted_objective_baseline_and_score(cfg):
         osc, oper = orr.score(t)
         assert np.array_equal(_np(per).view(np.uint64), oper.view(np.uint64)), algo
         assert _np(sc).view(np.uint64)[0] == np.float64(osc).view(np.uint64)
+
+
+def test_unaware_penalty_below_objective_values():
+    """A penalty smaller than some objective values: the first valid configuration a run evaluates becomes its best-so-far
+    whatever its value (the oracle's rule, A33), it does not have to beat the penalty."""
+    gr, orr = run_pair(0, "pso", R=16, P=12, gens=8, seed=9, aware=False, penalty=0.5)
+    assert (orr.best()["best_f"][orr.best()["best_rank"] != 0xFFFFFFFF] > 0.5).any()
+    run_pair(0, "de", R=16, P=12, gens=8, seed=9, aware=False, repair_mode=1, penalty=0.5)

@@ -256,3 +256,17 @@ def test_two_live_run_sets_share_a_kernel_instantiation():
         torch.cuda.synchronize()
     compare(a, orr, sp.n)
     assert b.gen == 3
+
+
+@pytest.mark.parametrize("algo", ["de", "ga"])
+def test_objective_at_or_above_the_default_penalty(algo):
+    """The objective contract is "> 0 and finite": a table whose every value exceeds the default penalty (1e20, L107) still
+    has a best-so-far from generation 0 on, the same one in the fused kernel, the phased pipeline and the oracle."""
+    sp, os_ = oracle_space(0)
+    obj = (W.objective_table(os_.rows(), sp.m, 0).astype(np.float64) * 1e22).astype(np.float32)
+    assert obj.min() >= 1e20 and np.isfinite(obj).all()
+    try:
+        gr, orr = run_pair(0, algo, R=20, P=20, gens=8, step_sizes=[1, 3, 4], objective=obj)
+        assert (orr.best()["best_rank"] != 0xFFFFFFFF).all()
+    finally:
+        os_.set_objective(W.objective_table(os_.rows(), sp.m, 0))
