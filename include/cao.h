@@ -271,11 +271,12 @@ int cao_runs_stats(const cao_runs* r, void* stream, uint64_t* h_out32);
 /* NEXT-4 (Eq.2; A36): performance score of a set of runs against the calculated random-search baseline
  * B(t) = expected minimum of t draws without replacement from the V objective values (fp64).
  *   cao_space_sort_objective: d_sorted = the objective table in ascending order (V floats; d_scratch: the next power of
- *                             two >= V floats).
+ *                             two >= V floats).  CAO_E_TOO_LARGE when V > 2^31.
  *   cao_space_baseline:       d_B[q] = B(d_t[q]) for S sampling points (unique-evaluation counts, clamped to 1..V).
  *   cao_runs_score:           d_per_t[q] = mean over the runs of (B - best_r(t)) / (B - f_opt), best_r(t) = best-so-far at
  *                             the last recorded generation whose unique-evaluation count is <= t (generation 0 if none;
- *                             the worst objective if nothing valid was evaluated); d_score[0] = their mean over q.
+ *                             the worst objective if nothing valid was evaluated); where B(t) = f_opt (t >= V, or a constant
+ *                             table) the term is 1 for a run that holds the optimum, else 0; d_score[0] = their mean over q.
  *                             d_scratch: S * n_runs doubles.  Bit-identical to the oracle (same fp64 operation order). */
 int cao_space_sort_objective(const cao_space* s, float* d_sorted, void* d_scratch, void* stream);
 int cao_space_baseline(const cao_space* s, const float* d_sorted, const uint64_t* d_t, uint32_t S, double* d_B, void* stream);
@@ -287,8 +288,8 @@ uint64_t cao_launch_count(void);
 /* Optional device timing per kernel class (bench.py's roofline): while enabled, every launch is bracketed by
  * CUDA events on its stream.  enable(1) clears the totals.  read() synchronises the recorded events and
  * returns the summed milliseconds and the launch count of class `cls`: 0 k_build_tables + k_inner_lut, 1 k_enum,
- * 2 count scan, 3 k_fill, 4 k_init, 5 k_op, 6 k_scan, 7 k_finish, 8 queries, 9 k_probe23, 10 k_gen, 11 k_residual;
- * name() gives the kernel names. */
+ * 2 count scan, 3 k_fill, 4 k_init, 5 k_op, 6 k_scan, 7 k_finish, 8 queries, 9 k_probe23, 10 k_gen, 11 k_residual,
+ * 12 k_keys + k_masks, 13 k_res_prefix + k_res_class_table; name() gives the kernel names ("" beyond the last class). */
 int cao_profile_enable(int32_t on);
 int cao_profile_read(int32_t cls, double* h_ms_total, uint64_t* h_launches);
 const char* cao_profile_name(int32_t cls);

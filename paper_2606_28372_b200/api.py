@@ -156,11 +156,15 @@ def profile_enable(on=True):
 def profile_read():
     """{kernel class name: (total ms, launches)} since profile_enable(True)."""
     out = {}
-    for cls in range(12):
+    cls = 0
+    while True:
+        name = lib().cao_profile_name(cls).decode()
+        if not name:                                   # "" beyond the last class
+            return out
         ms, n = C.c_double(), u64()
         _check(lib().cao_profile_read(cls, C.byref(ms), C.byref(n)))
-        out[lib().cao_profile_name(cls).decode()] = (ms.value, n.value)
-    return out
+        out[name] = (ms.value, n.value)
+        cls += 1
 
 
 def _view(base: torch.Tensor, ptr: int, nbytes: int, dtype, shape):

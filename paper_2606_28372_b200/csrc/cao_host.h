@@ -16,7 +16,7 @@ int cao_cuda_check(cudaError_t e, const char* what);
 #define CAO_LAUNCHED(what) do { ++g_cao_launches; int rc_ = cao_cuda_check(cudaGetLastError(), what); if (rc_) return rc_; } while (0)
 
 // Optional per-kernel-class device timing (cao_profile_*): CUDA events on the launching stream around each launch.
-enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_GEN, PK_RESID, PK_N };
+enum { PK_TABLE = 0, PK_ENUM, PK_CSCAN, PK_FILL, PK_INIT, PK_OP, PK_SCAN, PK_FINISH, PK_QUERY, PK_PROBE, PK_GEN, PK_RESID, PK_MASKS, PK_RESPRE, PK_N };
 extern std::atomic<int> g_cao_prof_on;
 void cao_prof_mark(int cls, bool end, cudaStream_t st);
 struct ProfScope {

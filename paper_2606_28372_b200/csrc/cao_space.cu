@@ -89,7 +89,7 @@ int cao_profile_read(int32_t cls, double* ms_total, uint64_t* launches) {
 const char* cao_profile_name(int32_t cls) {
     static const char* names[PK_N] = {"k_build_tables+k_inner_lut", "k_enum", "k_cnt_reduce+k_cnt_apply", "k_fill", "k_init",
                                       "k_op", "k_scan", "k_finish", "k_is_valid/k_repair_probe/k_repair_finish", "k_probe23", "k_gen",
-                                      "k_residual"};
+                                      "k_residual", "k_keys+k_masks", "k_res_prefix+k_res_class_table"};
     return cls >= 0 && cls < PK_N ? names[cls] : "";
 }
 
@@ -380,10 +380,11 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
             CAO_CUDA(cudaStreamWaitEvent(s->side2, s->ev_fork2, 0));
         }
         if (s->use_keys) {
+            ProfScope ps(PK_MASKS, st);
             k_keys<<<(unsigned)std::min<uint64_t>((s->n_blocks + bd - 1) / bd, 148ull * 4), bd, smem_dig, st>>>(s->meta, ea);
             CAO_LAUNCHED("k_keys");
         }
-        ProfScope ps(PK_PROBE, st);
+        ProfScope ps(PK_MASKS, st);
         const uint64_t items = s->n_blocks * (uint64_t)s->Wb;
         k_masks<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 16), bd, smem_dig, st>>>(s->meta, ea);
         CAO_LAUNCHED("k_masks");
@@ -392,12 +393,12 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         ResPrefix* pre = (ResPrefix*)(sc + s->off_pre);
         const uint64_t items = s->n_blocks * (uint64_t)s->n_res;
         {
-            ProfScope ps(PK_QUERY, s->side2);
+            ProfScope ps(PK_RESPRE, s->side2);
             k_res_prefix<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 8), bd, smem_desc, s->side2>>>(s->meta, ea, pre);
         }
         CAO_LAUNCHED("k_res_prefix");
         if (s->n_rc) {
-            ProfScope ps(PK_QUERY, s->side2);
+            ProfScope ps(PK_RESPRE, s->side2);
             k_res_class_table<<<dim3(148 * 4, (unsigned)s->n_rc), 256, 0, s->side2>>>(s->meta, ea);
             CAO_LAUNCHED("k_res_class_table");
         }

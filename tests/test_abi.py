@@ -90,3 +90,16 @@ def test_product_does_not_import_oracle():
             if fn.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, fn)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "cao_oracle" not in txt, fn
+
+
+def test_profile_class_names(L):
+    """Every kernel class of cao_profile_read has a name that says which kernels it times; "" ends the list."""
+    names = []
+    while True:
+        nm = L.cao_profile_name(len(names)).decode()
+        if not nm:
+            break
+        names.append(nm)
+    assert len(names) == 14 and len(set(names)) == 14
+    assert "k_masks" in names[12] and "k_res_prefix" in names[13] and names[9] == "k_probe23"
+    assert L.cao_profile_name(-1) == b""

@@ -210,3 +210,20 @@ def test_rebuild_reproduces_the_space(cfg):
     want = os_.repair(rows)
     rank, key = gs.repair(rows)                                         # probe tables survive the rebuild
     assert np.array_equal(rank.cpu().numpy().view(np.uint32), want["rank"])
+
+
+def test_profile_classes_of_the_build():
+    """Per-kernel timing of S1: the mask / key and residual-prefix kernels are booked under their own classes, not under the
+    repair-probe and query classes that the generation step's analysis reads."""
+    import paper_2606_28372_b200 as cao
+    sp = W.space_cfg3()                                                 # has tabled and residual constraints
+    cao.profile_enable(True)
+    try:
+        cao.Space.from_space(sp).build()
+        torch.cuda.synchronize()
+        prof = cao.profile_read()
+    finally:
+        cao.profile_enable(False)
+    assert prof["k_keys+k_masks"][1] >= 1 and prof["k_enum"][1] == 1 and prof["k_fill"][1] == 1
+    assert prof["k_probe23"][1] == 0 and prof["k_is_valid/k_repair_probe/k_repair_finish"][1] == 0
+    assert len(prof) == 14
