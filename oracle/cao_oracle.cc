@@ -844,6 +844,7 @@ uint64_t baseline_budget(const std::vector<float>& sorted, double frac) {
 // P_t of one run (L359-361; A36): (B(t) - best_r(t)) / (B(t) - f_opt), best_r(t) = best-so-far objective at the last
 // recorded generation whose unique-evaluation count is <= t (generation 0 if none); a run that has not evaluated any
 // valid configuration by then counts as the worst feasible objective.  0 = baseline, 1 = optimum found at once.
+// Where the baseline has itself reached the optimum the quotient is undefined; see the guard below.
 double score_run_at(const Runs& rs, const std::vector<float>& sorted, uint32_t k, uint64_t t) {
     const uint32_t G = rs.gen;
     uint32_t gsel = 0;
@@ -856,6 +857,9 @@ double score_run_at(const Runs& rs, const std::vector<float>& sorted, uint32_t k
     std::memcpy(&br, &rs.traj[((size_t)gsel * rs.R + k) * 12 + 4], 4);
     const double best = br == RANK_NONE ? (double)sorted.back() : (double)bf;
     const double B = baseline_at(sorted, t), opt = sorted[0];
+    // B(t) = f_opt (t >= V, or every objective value equal): random search has reached the optimum itself and the ratio is
+    // 0/0 or x/0.  A36: the term is then 1 for a run that holds the optimum and 0 otherwise.
+    if (B - opt == 0.0) return best == opt ? 1.0 : 0.0;
     return (B - best) / (B - opt);
 }
 

@@ -728,13 +728,14 @@ int cao_space_repair_mode(const cao_space* s, int32_t mode, const uint8_t* d_idx
 
 // ---------------------------------------------------------------------------------------------
 // NEXT-4
-static uint32_t next_pow2(uint64_t v) { uint32_t p = 1; while (p < v) p <<= 1; return p; }
+static uint64_t next_pow2(uint64_t v) { uint64_t p = 1; while (p < v) p <<= 1; return p; }
 int cao_space_sort_objective(const cao_space* s, float* d_sorted, void* d_scratch, void* stream) {
     if (!s || !d_sorted || !d_scratch) return cao_fail(CAO_E_INVALID_ARG, "cao_space_sort_objective: NULL argument");
     if (!s->filled || !s->meta.obj) return cao_fail(CAO_E_STATE, "cao_space_sort_objective: build the space and set the objective first");
     if (s->meta.V == 0) return cao_fail(CAO_E_EMPTY_SPACE, "cao_space_sort_objective: the space has no valid configuration");
     cudaStream_t st = (cudaStream_t)stream;
-    const uint32_t V = s->meta.V, n2 = next_pow2(V);
+    if (s->meta.V > (1ull << 31)) return cao_fail(CAO_E_TOO_LARGE, "cao_space_sort_objective: more than 2^31 valid configurations");
+    const uint32_t V = s->meta.V, n2 = (uint32_t)next_pow2(V);
     uint32_t* buf = (uint32_t*)d_scratch;
     const unsigned grid = (n2 + 255) / 256;
     k_sort_load<<<grid, 256, 0, st>>>(s->meta.obj, V, buf, n2);

@@ -309,7 +309,9 @@ static __global__ void __launch_bounds__(256) k_score_runs(const uint32_t* __res
     const uint32_t fb = traj[((uint64_t)gsel * R + k) * 3], br = traj[((uint64_t)gsel * R + k) * 3 + 1];
     const double best = br == 0xFFFFFFFFu ? (double)sorted[V - 1] : (double)__uint_as_float(fb);
     const double b = B[q], opt = (double)sorted[0];
-    scratch[e] = __ddiv_rn(__dsub_rn(b, best), __dsub_rn(b, opt));
+    // B(t) = f_opt (t >= V, or a constant table): the quotient is undefined; A36: 1 for a run that holds the optimum, else 0
+    const double den = __dsub_rn(b, opt);
+    scratch[e] = den == 0.0 ? (best == opt ? 1.0 : 0.0) : __ddiv_rn(__dsub_rn(b, best), den);
 }
 // Means in the oracle's order: over the runs (k ascending) for every sampling point, then over the sampling points.
 static __global__ void __launch_bounds__(32) k_score_reduce(const double* __restrict__ scratch, uint32_t R, uint32_t S, double* per_t,

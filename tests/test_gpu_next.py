@@ -243,7 +243,7 @@ def test_sorted_objective_baseline_and_score(cfg):
         kw = dict(n_runs=40, pop=16, max_gens=12, seed=3)
         orr = O.OracleRuns(os_, algo, variant=O.Variant.make(**var), **kw); orr.step(12)
         gr = cao.Runs(g, algo, variant=cao.Variant.make(**var), **kw); gr.step(12)
-        t = [16, 20, 30, 50, 80, 120, 200] if cfg else [16, 20, 30, 50, 80]
+        t = [16, 20, 30, 50, 80, 120, 200] if cfg else [16, 20, 30, 50, 80, V, 3 * V]   # B(t >= V) = f_opt: guarded quotient (A36)
         sc, per = gr.score(srt, t)
         osc, oper = orr.score(t)
         assert np.array_equal(_np(per).view(np.uint64), oper.view(np.uint64)), algo

@@ -433,6 +433,14 @@ def test_score_special_cases_and_direct_evaluation():
             break
     else:
         pytest.skip("no seed starts at the optimum")
+    # t = V: B(V) is the optimum itself (every draw taken), the quotient would be x/0; A36: 1 for runs that hold the optimum, else 0
+    V = s.V
+    assert s.baseline(V) == fopt
+    scV, perV = r.score([V])
+    g_last = [max(gg for gg in range(11) if traj["uniq"][gg, k] <= V) for k in range(12)]
+    wantV = np.mean([1.0 if float(traj["best_f"][g_last[k], k]) == fopt else 0.0 for k in range(12)])
+    assert np.isfinite(perV).all() and perV[0] == wantV and scV == wantV
+    assert np.isfinite(r.score([8, V, 10 * V])[0])
     # a run stuck at the baseline value scores 0: uniform-random search itself averages to ~0 over many runs
     ru = O.OracleRuns(s, "ga", n_runs=400, pop=8, max_gens=0, seed=5)     # generation 0 = 8 uniform valid draws
     sc, _ = ru.score([8])
