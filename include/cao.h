@@ -76,6 +76,8 @@ typedef struct {
  *   de_crossover      0 binomial (default), 1 exponential (L272)
  *   ga_crossover      0 single_point (default), 1 two_point, 2 uniform, 3 disruptive_uniform (L288; A31)
  *   init_lhs          1 = DE's initial population by Latin Hypercube Sampling, repaired to valid (L223; A35)   [NEXT-3]
+ *                     The LHS points are always repaired with the unified key (Hamming, sum|didx|, L), also when
+ *                     repair_mode = 1 selects the paper's own repairs for the generations that follow.
  *   penalty           objective reported for an unevaluated invalid configuration, > 0 and finite (L107: 1e20)          */
 typedef struct {
     int32_t constraint_aware, repair_mode, de_mutation, de_crossover, ga_crossover, init_lhs;
@@ -263,7 +265,8 @@ int cao_runs_counters(const cao_runs* r, void* stream, uint64_t* n_repaired, uin
 /* All thirty-two 64-bit statistics words since create (synchronises `stream`): 0 n_repaired, 1 n_scanned (candidates
  * that needed the table scan), 2 n_evaluated; fused mode only: 3 candidates that went to the Hamming-2 probe, 4 ...
  * beyond it, 5 invalid candidates resolved by the previous generation's memo, 6 ... by the per-run repair cache
- * (L268: memoisation); 7 reserved; 8-13 clock cycles of thread 0 of every group in operator / tail / probe-2 /
+ * (L268: memoisation); 7 n_penalised: candidates that stayed invalid and received the static penalty instead of an
+ * evaluation (NEXT-1 / NEXT-2 variants only, L107; they are included in word 2); 8-13 clock cycles of thread 0 of every group in operator / tail / probe-2 /
  * deeper probes / scan / finish, 14-15 slowest run and most scan cycles in one run (only in builds with
  * -DCAO_GEN_STATS, else 0); 16-24 candidates of the stepped generations by Hamming distance of their repair
  * (16 = valid, 17 = Hamming 1, ..., 24 = eight or more; L143, L215); 25-31 reserved. */
