@@ -201,6 +201,65 @@ def test_cfg3_firefly_full_length():
             compare_window(gr, orr, sp.n, k0)
 
 
+# ---------------------------------------------------------------------------------------------------------- the shapes bench.py times
+def test_cfg3_firefly_timed_shape():
+    """bench.py's steps_cfg3: Firefly, P = 128, R = 1000, 100 generations, the library's default mode (phased).  The scan's
+    (candidate tiles, table chunks) split is chosen on the device from the worklist length, so R = 1000 takes a split that
+    the 8-run test above never takes; runs at the start, the middle and the end against the oracle."""
+    import paper_2606_28372_b200 as cao
+    sp, os_ = oracle_space(3)
+    g = gpu_space(3, os_, sp)
+    R, gens = 1000, 100
+    windows = [0, 499, R - 1]
+    kw = dict(pop=128, budget=0, seed=0)
+    ors = oracle_windows(os_, "firefly", windows, 1, gens, **kw)
+    gr = cao.Runs(g, "firefly", n_runs=R, max_gens=gens, **kw)
+    assert gr.mode == "phased"
+    gr.step(gens)
+    for k0, orr in zip(windows, ors):
+        compare_window(gr, orr, sp.n, k0)
+
+
+def test_cfg2_ga_timed_shape():
+    """bench.py's steps_cfg2: GA, P = 64, R = 10^4, 150 generations: 4 GB of per-run dedup bitmaps, byte offsets beyond 2^31."""
+    import paper_2606_28372_b200 as cao
+    sp, os_ = oracle_space(2)
+    g = gpu_space(2, os_, sp)
+    R, gens, width = 10_000, 150, 2
+    windows = [0, 5_000, R - width]
+    kw = dict(pop=64, budget=0, seed=0)
+    ors = oracle_windows(os_, "ga", windows, width, gens, **kw)
+    gr = cao.Runs(g, "ga", n_runs=R, max_gens=gens, **kw)
+    assert gr.workspace_bytes > 4_000_000_000
+    gr.step(gens)
+    for k0, orr in zip(windows, ors):
+        compare_window(gr, orr, sp.n, k0)
+    del gr
+    torch.cuda.empty_cache()
+
+
+_NEXT_ROWS = [(a, v) for a in ("de", "pso", "firefly", "ga") for v in ("unaware", "paper_repair")] + \
+             [("de", "rand1exp"), ("de", "lhs"), ("ga", "uniform")]
+
+
+@pytest.mark.parametrize("algo,name", _NEXT_ROWS)
+def test_cfg1_variant_rows_timed_shape(algo, name):
+    """bench.py's next_rows_cfg1: every SURVEY 8(f) variant at R = 1000, budget 1000, cap 200 generations; first and last runs."""
+    import paper_2606_28372_b200 as cao
+    var = {"unaware": dict(aware=False), "paper_repair": dict(repair_mode=1), "rand1exp": dict(de_mutation="rand1", de_crossover="exp"),
+           "lhs": dict(init_lhs=True), "uniform": dict(ga_crossover="uniform")}[name]
+    sp, os_ = oracle_space(1)
+    g = gpu_space(1, os_, sp)
+    R, gens, width = 1000, 200, 2
+    windows = [0, R - width]
+    kw = dict(pop=32, budget=1000, seed=0)
+    ors = oracle_windows(os_, algo, windows, width, gens, variant=O.Variant.make(**var), **kw)
+    gr = cao.Runs(g, algo, n_runs=R, max_gens=gens, variant=cao.Variant.make(**var), **kw)
+    gr.step(gens)
+    for k0, orr in zip(windows, ors):
+        compare_window(gr, orr, sp.n, k0)
+
+
 @pytest.mark.parametrize("algo", ["de", "pso", "firefly", "ga"])
 def test_cfg4_hundred_thousand_runs(algo):
     """BASELINE configs[4] at 10^5 runs, 200 generations, ONE launch: 3 GB of per-run dedup bitmaps (64-bit offsets),

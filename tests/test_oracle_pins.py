@@ -60,7 +60,7 @@ def test_exp_neg_spec_against_libm():
     got = O.exp_neg_spec_many(z).astype(np.float64)
     ref = np.exp(-z.astype(np.float64))
     rel = np.abs(got - ref) / ref
-    assert rel.max() < 4e-6, rel.max()                      # t = z*log2(e) rounding dominates (~z * 2^-24 relative)
+    assert rel.max() < 2e-6, rel.max()                      # SURVEY 8(c)'s bound (measured 1.8e-6 near z = 30: the rounding of t = z*log2(e), ~z * 2^-24 relative)
     small = z <= 1.0
     assert rel[small].max() < 3e-7
 
