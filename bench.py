@@ -6,16 +6,18 @@ One "step" = one pass of every S-row of the hot path over 
   S2  create R runs of each algorithm (generation 0)
   S3-S7  step every run until its budget of unique evaluations / the generation cap
   read best-so-far.
-Workload at N=1: BASELINE.json configs[1] (GEMM-like space, DE+PSO+Firefly+GA, pop 32, budget 1000 unique
-evaluations, cap 200 generations, 1000 runs each).  N>1: every rank processes its own 1000 runs per algorithm
-(run indices rank*1000..), no data-path collective (weak scaling).
+Workload at N=1: BASELINE.json names no config for its metric, so the default is the largest single-GPU one, configs[4]
+(GEMM-like space of configs[1], DE+PSO+Firefly+GA, pop 32, no budget, 200 generations, 10,000 runs each: 2.57e8 candidates
+per step); `--config 1` is the small budgeted workload rounds 1-2 reported (1000 runs, budget 1000 unique evaluations).
+N>1: every rank processes its own 10,000 runs per algorithm (run indices rank*10000..), no data-path collective (weak scaling).
 
 Besides the headline line the same JSON carries, as top-level keys: `enumeration` (S1 alone on configs[1..3]),
 `sweep_cfg4` (configs[4]: candidates/s against the run count), `steps_cfg2` / `steps_cfg3` (the generation step of
-configs[2] and configs[3] at their BASELINE sizes, fused and phased), `int_peak` (measured integer issue rates) and
-`cpu_baseline`.
+configs[2] and configs[3] at their BASELINE sizes, fused and phased), `next_rows_cfg1` (the SURVEY 8(f) variants on
+configs[1]), `int_peak` (measured integer issue rates) and `cpu_baseline`.  The headline figures of those legs are repeated
+as plain numbers inside `roofline` (enumeration Gcfg/s and HBM fraction, the sweep's HBM fractions, the cfg2 / cfg3 steps).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
 prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
@@ -38,6 +40,8 @@ N_SM = 148
 # profiles/r2_kgen.md (it does not change with the run; the live numbers of this line are the CUDA-event times).
 NCU_KGEN_DRAM_BYTES_PER_LAUNCH = 17.2e6
 NCU_KGEN_SOURCE = "profiles/r2b_kgen.md"
+# the same for the default workload, configs[4] at 10,000 runs per algorithm: (741.3 + 413.1 + 107.2 + 100.9) / 4 MB
+NCU_KGEN_TRAFFIC = {(1, 1000): (17.2e6, "profiles/r2b_kgen.md"), (4, 10000): (340.6e6, "profiles/r3_kgen_cfg4.md")}
 SECTOR_BYTES_PER_CANDIDATE = 204          # state 2(n+8) + bitmap 32 + directory 32 + obj 32 + dedup 64
 
 
@@ -161,6 +165,15 @@ def oracle_sample_text(wl, R_o):
             "every repair is a brute-force scan of the valid table (the oracle is the plain definition, not a tuned CPU program)")
 
 
+def oracle_seconds_per_run(wl):
+    """Rough oracle cost of ONE run of every algorithm of the workload (~2,400 candidates/s on one core, measured in rounds
+    1-2): with a budget of b unique evaluations a run evaluates about 4 b candidates before it stops (duplicates count)."""
+    per_algo = wl["pop"] * (wl["gens"] + 1)
+    if wl["budget"]:
+        per_algo = min(per_algo, 4 * wl["budget"])
+    return len(wl["algos"]) * per_algo / 2400.0
+
+
 def reference_arm(args):
     """The CPU oracle as it stands, on the host cores, on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -168,14 +181,16 @@ def reference_arm(args):
         return
     wl = workload(args.config, None)
     sp = wl["space"]
-    # bounded sample: one step = the full space build (~0.7 s on configs[1]) + R_o runs of every algorithm (~6.6 s per run of
-    # the four); R_o is cut so that (steps + 1 warm-up) steps end within about three minutes
-    R_o = max(1, min(args.ref_runs, int((170.0 / (args.steps + 1) - 0.7) / 6.6)))
-    sample = oracle_sample_text(wl, R_o)
+    # bounded sample: one step = the full space build (~0.7 s on configs[1] / [4]) + R_o runs of every algorithm (configs[1]:
+    # ~6.6 s per run of the four, configs[4]: ~11 s); R_o is cut so that (steps + 1 warm-up) steps end within a few minutes
+    R_o = max(1, min(args.ref_runs, int((170.0 / (args.steps + 1) - 0.7) / oracle_seconds_per_run(wl))))
     obj = oracle_prepare(wl)
     with PinnedToOneCore():
         for _ in range(min(args.warmup, 1)):
-            oracle_sample_step(wl, R_o, obj)
+            _, t_w = oracle_sample_step(wl, R_o, obj)
+            if R_o > 1 and t_w * args.steps > 240.0:                      # a slower host than the estimate assumed: fewer runs per step
+                R_o = max(1, int(R_o * 240.0 / (t_w * args.steps)))
+        sample = oracle_sample_text(wl, R_o)
         tot_c, tot_t = 0, 0.0
         for _ in range(args.steps):
             c, t = oracle_sample_step(wl, R_o, obj)
@@ -347,15 +362,18 @@ def gpu_arm(args):
     by = per * cands_step / max(top_n, 1)
     roof = {"kernel": top, "bound": "hbm", "achieved": by / dur_s / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
             "peak_source": pk["source"], "algorithmic_bytes_per_candidate": per,
-            "traffic": NCU_KGEN_DRAM_BYTES_PER_LAUNCH if (top == "k_gen" and args.config == 1 and R == 1000) else None,
-            "traffic_source": f"stored constant from the ncu --set full capture in {NCU_KGEN_SOURCE}, not measured by this run"}
+            "traffic": None, "traffic_source": "no ncu capture of this workload shape"}
+    ncu_src = NCU_KGEN_SOURCE
+    if top == "k_gen" and (args.config, R) in NCU_KGEN_TRAFFIC:
+        roof["traffic"], ncu_src = NCU_KGEN_TRAFFIC[(args.config, R)]
+        roof["traffic_source"] = f"stored constant from the ncu --set full capture in {ncu_src}, not measured by this run"
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_us"] = dur_s * 1e6
     roof["share_of_step"] = top_ms / (ms_prof / args.steps)
     roof["measured_in"] = ("the same step re-run in the timed loop on ONE stream with CUDA events around every launch "
                            f"({ms_prof / args.steps:.2f} ms/step serialised vs {ms / args.steps:.2f} ms/step with one stream per algorithm)")
     roof["note"] = ("sector-granular HBM model of SURVEY 8(d); the kernel is bound by instruction issue, not DRAM "
-                    f"(ncu: {NCU_KGEN_SOURCE}); sweep_cfg4 shows the same kernel with the GPU filled")
+                    f"(ncu: {ncu_src}); sweep_cfg4 shows the same kernel from 100 to 100,000 runs")
 
     # ---- measured integer issue peaks (lane-operations per second, one instruction kind each)
     int_peak = {}
@@ -479,10 +497,11 @@ def gpu_arm(args):
     # headline step, and the performance score (NEXT-4, Eq.2) of every variant against the calculated random-search
     # baseline -- score(aware) - score(unaware) is the quantity the paper's headline (+0.393 on its 24 spaces, L411) reports
     nxt = {}
-    if not args.no_next:
+    if not args.no_next and args.config in (1, 4):                        # configs[1] and [4] share the space (and obj_d)
+        wl1 = workload(1, None)
         spn = cao.Space.from_space(sp).build(); spn.set_objective(obj_d)
         srt = spn.sorted_objective()
-        ts = [int(t) for t in np.linspace(P, wl["budget"] or 1000, 32)]
+        ts = [int(t) for t in np.linspace(wl1["pop"], wl1["budget"], 32)]
         Bt = spn.baseline(srt, ts)
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -497,11 +516,11 @@ def gpu_arm(args):
             for name, kw in variants + extra.get(algo, []):
                 best_ms = None
                 for rep in range(2):
-                    rr = cao.Runs(spn, algo, n_runs=R, pop=P, budget=wl["budget"], max_gens=G, seed=wl["seed"],
-                                  variant=cao.Variant.make(**kw) if kw else None)
+                    rr = cao.Runs(spn, algo, n_runs=wl1["runs"], pop=wl1["pop"], budget=wl1["budget"], max_gens=wl1["gens"],
+                                  seed=wl1["seed"], variant=cao.Variant.make(**kw) if kw else None)
                     torch.cuda.synchronize(); flush.zero_()
                     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    e0.record(); rr.step(G); e1.record(); e1.synchronize()
+                    e0.record(); rr.step(wl1["gens"]); e1.record(); e1.synchronize()
                     t = e0.elapsed_time(e1); best_ms = t if best_ms is None else min(best_ms, t)
                     if rep == 1:
                         st = rr.stats()
@@ -525,11 +544,21 @@ def gpu_arm(args):
         import oracle as O
         obj_o = oracle_prepare(wl)
         assert np.array_equal(obj_o, obj)                                 # same input on both sides
+        R_cpu = max(1, min(args.ref_runs, int(25.0 / oracle_seconds_per_run(wl))))   # about 10-30 s of CPU work
         with PinnedToOneCore():
-            c, t = oracle_sample_step(wl, args.ref_runs, obj_o)
-        cpu = {"value": c / t, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": oracle_sample_text(wl, args.ref_runs),
+            c, t = oracle_sample_step(wl, R_cpu, obj_o)
+        cpu = {"value": c / t, "unit": "candidates/s", "cores": 1, "kind": "oracle", "sample": oracle_sample_text(wl, R_cpu),
                "seconds": t, **cpu_info()}
 
+    # BASELINE.json's metric has three parts (candidates/s, enumeration Gcfg/s, % of the HBM roofline): the other two, and the
+    # remaining legs' headline figures, as plain numbers inside the contract key (the bulky per-leg objects follow below)
+    roof["enumeration"] = {k: {"gcfg_s": round(v["gcfg_s"], 1), "us": round(v["ms"] * 1e3, 1), "hbm_frac": round(v["hbm_frac"], 4)}
+                           for k, v in enum.items()}
+    roof["sweep_cfg4_hbm_frac"] = {Rs: {a: round(v["hbm_frac_204B"], 4) for a, v in row.items()} for Rs, row in sweep.items()}
+    roof["sweep_cfg4_gcand_s"] = {Rs: {a: round(v["candidates_per_s"] / 1e9, 3) for a, v in row.items()} for Rs, row in sweep.items()}
+    for cfgk, leg in other.items():
+        roof["step_" + cfgk] = {m: {"ms": round(v["ms"], 2), "mcand_s": round(v["candidates_per_s"] / 1e6, 1)}
+                                for m, v in leg.items() if isinstance(v, dict) and "ms" in v}
     line = {
         "metric": "candidates_repaired_evaluated_per_s", "value": value, "unit": "candidates/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -568,7 +597,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs[k]; 4 = the largest single-GPU workload (default), 1 = the small budgeted one")
     ap.add_argument("--runs", type=int, default=None, help="runs per algorithm per GPU (default: the config's)")
     ap.add_argument("--ref-runs", type=int, default=3, help="runs per algorithm of the CPU-oracle sample")
     ap.add_argument("--streams", type=int, default=4, help="1 = all algorithms on one stream, >1 = one stream per algorithm")
