@@ -27,6 +27,11 @@ struct ProfScope {
 
 static inline uint64_t align256(uint64_t x) { return (x + 255) & ~255ull; }
 
+// Multiprocessors of the current device (cached per device ordinal): every persistent / grid-stride grid is sized as a
+// multiple of it.  Without a usable device (host-side planning on a CPU-only box) it answers 148, the B200's count; the
+// value only shapes grids and chunking, never results.
+unsigned cao_sm_count();
+
 // Opt-in to more than 48 KB of dynamic shared memory.  cudaFuncAttributeMaxDynamicSharedMemorySize REPLACES the kernel's
 // limit, it does not raise it: two live objects (two cao_runs, two cao_space) that share a kernel instantiation and each
 // set "their" size would lower the limit under one another, and the larger one's next launch would fail with

@@ -16,7 +16,7 @@ struct GenLayout;
 CAO_GEN_DECL(0) CAO_GEN_DECL(1) CAO_GEN_DECL(2) CAO_GEN_DECL(3)
 #include "cao_gen_layout.h"
 
-#define SCAN_GRID (148 * 8)
+#define SCAN_GRID (cao_sm_count() * 8)
 
 struct cao_runs {
     const cao_space* s = nullptr;
@@ -71,7 +71,7 @@ static int launch_pick_nb(const SpaceMeta& sm, const uint8_t* cand, const uint32
                           const uint32_t* cnt3, const uint32_t* w_arr, uint64_t seed, uint32_t first_run, uint32_t P, uint32_t gen,
                           unsigned long long* key, uint8_t* rule, cudaStream_t st) {
     ProfScope ps(PK_SCAN, st);
-#define CALL_PICK(W) k_pick_nb<W><<<148 * 4, 256, 0, st>>>(sm, cand, wl, wl_count, present, cnt3, w_arr, seed, first_run, P, gen, key, rule)
+#define CALL_PICK(W) k_pick_nb<W><<<cao_sm_count() * 4, 256, 0, st>>>(sm, cand, wl, wl_count, present, cnt3, w_arr, seed, first_run, P, gen, key, rule)
     DISPATCH_WU(sm.n, CALL_PICK);
     CAO_LAUNCHED("k_pick_nb");
     return CAO_OK;
@@ -94,8 +94,8 @@ static int launch_probe23(const cao_space* s, const SpaceMeta& sm, const uint8_t
     ProbeMeta pm = s->probe;
     pm.levels = levels;
     ProfScope ps(PK_PROBE, st);
-    if (sm.rowB == 16) k_probe23<4><<<148 * 8, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
-    else k_probe23<8><<<148 * 8, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
+    if (sm.rowB == 16) k_probe23<4><<<cao_sm_count() * 8, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
+    else k_probe23<8><<<cao_sm_count() * 8, 256, 0, st>>>(sm, pm, cand, wl, wl_count, key, wl2, wl2_count, n_scanned);
     CAO_LAUNCHED("k_probe23");
     return CAO_OK;
 }
@@ -272,7 +272,7 @@ static GenLayout gen_layout(const cao_space* s, int algo, uint32_t P, uint32_t R
     L.ptab = take(s->probe.levels >= 2 ? 2 * s->probe.NB : 0);
     L.words = off;
     const uint32_t G0 = (P + 31) / 32 * 32;
-    const double slots = 148.0 * 3 * 256;
+    const double slots = (double)cao_sm_count() * 3 * 256;
     uint32_t f = 1;
     if (width == 0) {
         if (algo == CAO_FIREFLY) { if (roww == 4 && G0 * 4 <= 256 && (double)R * G0 * 4 <= 1.25 * slots) f = 4; }

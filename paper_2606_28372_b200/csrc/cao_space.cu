@@ -39,6 +39,17 @@ void prof_drain() {
     g_prof_pending.clear();
 }
 }  // namespace
+unsigned cao_sm_count() {
+    static std::atomic<int> cache[64];                                   // zero-initialised: 0 = not asked yet
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return 148u; }
+    sms = cache[dev].load(std::memory_order_relaxed);
+    if (sms > 0) return (unsigned)sms;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) { cudaGetLastError(); return 148u; }
+    cache[dev].store(sms, std::memory_order_relaxed);
+    return (unsigned)sms;
+}
+
 void cao_prof_mark(int cls, bool end, cudaStream_t st) {
     std::lock_guard<std::mutex> lk(g_prof_mu);
     if (!end) {
@@ -174,7 +185,7 @@ static int plan_space(cao_space* s) {
     s->CH = 1; s->chunk_digits = 0;
     for (int d = t - 1; d >= 0; --d) {
         const uint64_t c2 = (uint64_t)s->CH * M.m[d];
-        if (c2 > 32 || s->n_blocks / c2 < 148ull * 256) break;
+        if (c2 > 32 || s->n_blocks / c2 < (uint64_t)cao_sm_count() * 256) break;
         s->CH = (uint32_t)c2; s->chunk_digits += 1;
     }
     // per-constraint plan
@@ -333,7 +344,7 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
     uint8_t* d_flags = sc + s->off_flags;
     if (s->n_tab) {
         ProfScope ps(PK_TABLE, st);
-        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 8191) / 8192, 148 * 8), (unsigned)s->n_tab);
+        dim3 grid((unsigned)std::min<uint64_t>((s->max_table_threads + 8191) / 8192, (uint64_t)cao_sm_count() * 8), (unsigned)s->n_tab);
         const uint32_t ci_cap = s->B <= 8192 ? (uint32_t)((s->B + 7) & ~7ull) : 0;
         const size_t tsm = 2 * (size_t)ci_cap + (size_t)std::max<uint64_t>(256, s->max_table_ci);
         if (tsm > 48 * 1024) CAO_SMEM_OPTIN(k_build_tables);
@@ -381,12 +392,12 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         }
         if (s->use_keys) {
             ProfScope ps(PK_MASKS, st);
-            k_keys<<<(unsigned)std::min<uint64_t>((s->n_blocks + bd - 1) / bd, 148ull * 4), bd, smem_dig, st>>>(s->meta, ea);
+            k_keys<<<(unsigned)std::min<uint64_t>((s->n_blocks + bd - 1) / bd, (uint64_t)cao_sm_count() * 4), bd, smem_dig, st>>>(s->meta, ea);
             CAO_LAUNCHED("k_keys");
         }
         ProfScope ps(PK_MASKS, st);
         const uint64_t items = s->n_blocks * (uint64_t)s->Wb;
-        k_masks<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 16), bd, smem_dig, st>>>(s->meta, ea);
+        k_masks<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, (uint64_t)cao_sm_count() * 16), bd, smem_dig, st>>>(s->meta, ea);
         CAO_LAUNCHED("k_masks");
     }
     if (s->n_res) {
@@ -394,18 +405,18 @@ static int launch_pass1(cao_space* s, void* d_bitmap, uint8_t* sc, cudaStream_t 
         const uint64_t items = s->n_blocks * (uint64_t)s->n_res;
         {
             ProfScope ps(PK_RESPRE, s->side2);
-            k_res_prefix<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, 148ull * 8), bd, smem_desc, s->side2>>>(s->meta, ea, pre);
+            k_res_prefix<<<(unsigned)std::min<uint64_t>((items + bd - 1) / bd, (uint64_t)cao_sm_count() * 8), bd, smem_desc, s->side2>>>(s->meta, ea, pre);
         }
         CAO_LAUNCHED("k_res_prefix");
         if (s->n_rc) {
             ProfScope ps(PK_RESPRE, s->side2);
-            k_res_class_table<<<dim3(148 * 4, (unsigned)s->n_rc), 256, 0, s->side2>>>(s->meta, ea);
+            k_res_class_table<<<dim3(cao_sm_count() * 4, (unsigned)s->n_rc), 256, 0, s->side2>>>(s->meta, ea);
             CAO_LAUNCHED("k_res_class_table");
         }
         CAO_CUDA(cudaEventRecord(s->ev_join2, s->side2));
         CAO_CUDA(cudaStreamWaitEvent(st, s->ev_join2, 0));              // join: k_residual needs the masks and the prefixes
         ProfScope ps(PK_RESID, st);
-        const uint64_t warps = std::min<uint64_t>(s->n_blocks, 148ull * 64);
+        const uint64_t warps = std::min<uint64_t>(s->n_blocks, (uint64_t)cao_sm_count() * 64);
         k_residual<<<(unsigned)((warps + 7) / 8), bd, smem_desc, st>>>(s->meta, ea, pre);
         CAO_LAUNCHED("k_residual");
     }
@@ -436,7 +447,7 @@ static int launch_fill(cao_space* s, uint8_t* tb, cudaStream_t st, bool single_p
     }
     const uint32_t* lut = s->use_lut ? (const uint32_t*)(sc + s->off_lut) : nullptr;
     const uint64_t magicB = s->B > 1 ? (uint64_t)((((unsigned __int128)1 << 64) + s->B - 1) / s->B) : 0;
-    const unsigned grid = (unsigned)std::min<uint64_t>((s->nd + 7) / 8, 148ull * 8);   // a warp per group, grid-stride over the list
+    const unsigned grid = (unsigned)std::min<uint64_t>((s->nd + 7) / 8, (uint64_t)cao_sm_count() * 8);   // a warp per group, grid-stride over the list
     {
         ProfScope ps(PK_FILL, st);
 #define CALL_FILL(W, L32) k_fill<W, L32><<<grid, 256, 0, st>>>(s->meta, s->n_words, rows, Ltab, dir, groups, ctl + 4, lut, s->B, magicB, s->t)
